@@ -1,0 +1,121 @@
+/*
+ * cuhpx.h -- C ABI of the B200-native HEALPix spherical harmonic transform (cuHPX hot path,
+ * arXiv 2510.01785; citations "P:n" are line n of the paper text, SURVEY.md section 8 is the scope table).
+ *
+ * The four operators on RING-ordered HEALPix maps, as real-linear maps between
+ *   map  : [batch][npix]  real (dtype),            npix = 12 nside^2
+ *   alm  : [batch][nalm]  complex interleaved (re,im) of dtype, m-major packed:
+ *          index(l, m) = m (2 lmax + 1 - m) / 2 + l,   0 <= m <= mmax <= lmax,  m <= l <= lmax (inclusive)
+ *
+ *   cuhpx_alm2map          S   : p_xy = sum_m sum_l a_lm lambda_lm(theta_y) exp(i m (phi0_y + 2 pi x / N_y))   Eq. 24
+ *                                (m < 0 terms implied by reality of the map; Im a_l0 is ignored)
+ *   cuhpx_map2alm          A   : a_lm = sum_y sum_x p_xy w_y lambda_lm(theta_y) exp(-i m (phi0_y + 2 pi x / N_y)) Eq. 26
+ *                                (a = Y^dagger W p, Eq. 27; output Im a_l0 is exactly 0)
+ *   cuhpx_alm2map_adjoint  S^T : "adjoint iSHT = Y^dagger"  P:287;  (S^T g)_lm = c_m sum_p g_p lambda_lm exp(-i m phi_p)
+ *   cuhpx_map2alm_adjoint  A^T : "adjoint SHT = W Y"        P:288;  (A^T b)_p = w_p [sum_l Re(b_l0) lambda_l0
+ *                                                                        + sum_{m>=1} sum_l Re(b_lm lambda_lm exp(i m phi_p))]
+ *   with c_0 = 1, c_m = 2 (m >= 1).  The transposes are taken w.r.t. <f,g> = sum_p f_p g_p and
+ *   <a,b> = sum_{l, m>=0} (Re a Re b + Im a Im b): the inner product autograd uses for the stored tensor, so
+ *   these are the analytic gradients of S and A.  A = D^-1 S^T W with D = diag(c_m).
+ *
+ * lambda_lm is the normalised associated Legendre function of Eq. 15 (Condon-Shortley phase included),
+ * generated on the fly by the three-term recurrence of Eq. 16; ring geometry follows Gorski et al.
+ * (ref [1] P:416): rings i = 1..4 nside - 1 north to south, polar caps N_i = 4 i, belt N_i = 4 nside.
+ *
+ * Conventions
+ *   - Every data pointer is a DEVICE pointer owned by the caller, 16-byte aligned.  The library allocates no
+ *     device memory: scratch and constant tables live in the caller's workspace (cuhpx_workspace_bytes).
+ *   - Inputs are const, outputs are fully overwritten (never accumulated); in/out must not alias.
+ *   - All work is enqueued on `stream`; the transform calls never synchronise with the host and can be captured
+ *     in a CUDA graph.  cuhpx_workspace_init enqueues table-building kernels and small host->device copies on
+ *     `stream` (it may block the host while it computes the tables); later calls on the same stream are ordered
+ *     after it.  A workspace serves one transform at a time (calls sharing one workspace must be stream-ordered).
+ *   - ring_weights: DEVICE pointer to 4 nside - 1 doubles (always fp64), rings north to south, the full
+ *     quadrature weight w_y of Eq. 26 (i.e. including the 4 pi / Npix factor); NULL = equal weights
+ *     4 pi / Npix (Eq. 1).
+ *   - Return value: a cuhpx_status_t.  Argument errors are detected on the host before any launch.  Nothing is
+ *     thrown across the ABI.  After CUHPX_ECUDA, cudaGetLastError() describes the launch failure.
+ *   - There is no CPU fallback: on a machine without a CUDA device every compute call returns CUHPX_ECUDA.
+ */
+#ifndef CUHPX_H_
+#define CUHPX_H_
+
+#include <stddef.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef enum { CUHPX_F32 = 0, CUHPX_F64 = 1 } cuhpx_dtype_t;
+
+typedef enum {
+    CUHPX_OK = 0,
+    CUHPX_EINVAL = 1,       /* bad nside / lmax / mmax / batch / dtype, null or misaligned pointer */
+    CUHPX_EWORKSPACE = 2,   /* workspace too small, not initialised, or initialised for other parameters */
+    CUHPX_EUNSUPPORTED = 3, /* valid request this build cannot serve (e.g. ring too long for one SM's shared memory) */
+    CUHPX_ECUDA = 4         /* CUDA runtime / launch error */
+} cuhpx_status_t;
+
+/* a cudaStream_t (CUstream_st*), declared here so the header needs no CUDA include */
+typedef struct CUstream_st* cuhpx_stream_t;
+
+/* ---- host-only helpers (no device work) */
+size_t cuhpx_npix(int nside);                      /* 12 nside^2; 0 if nside is not a power of two >= 1 */
+size_t cuhpx_nrings(int nside);                    /* 4 nside - 1 */
+size_t cuhpx_alm_count(int lmax, int mmax);        /* (mmax+1)(lmax+1) - mmax(mmax+1)/2; 0 on bad arguments */
+size_t cuhpx_alm_index(int lmax, int l, int m);    /* m (2 lmax + 1 - m)/2 + l */
+const char* cuhpx_status_string(int status);
+/* Ring table of Gorski et al. as the library uses it (ring = 1 .. 4 nside - 1): pixel count, RING index of the
+ * first pixel, cos(theta), phi0 of the first pixel.  Returns CUHPX_EINVAL on bad arguments. */
+int cuhpx_ring_info(int nside, int ring, long long* n_pix, long long* first_pix, double* cos_theta, double* phi0);
+
+/* ---- workspace */
+/* Bytes of device workspace needed for (nside, lmax, mmax, batch, dtype); 0 on invalid arguments. */
+size_t cuhpx_workspace_bytes(int nside, int lmax, int mmax, int batch, cuhpx_dtype_t dtype);
+/* Build the constant tables (ring geometry, recurrence seeds, twiddles, chirp filters) inside d_workspace.
+ * Must be called once before the transforms, and again if any of the five parameters changes. */
+int cuhpx_workspace_init(int nside, int lmax, int mmax, int batch, cuhpx_dtype_t dtype, void* d_workspace,
+                         size_t workspace_bytes, cuhpx_stream_t stream);
+/* Forget a workspace (host bookkeeping only; the memory stays the caller's). */
+int cuhpx_workspace_release(void* d_workspace);
+
+/* ---- the four operators */
+int cuhpx_map2alm(int nside, int lmax, int mmax, int batch, cuhpx_dtype_t dtype, const void* d_map, void* d_alm,
+                  const double* d_ring_weights, void* d_workspace, size_t workspace_bytes, cuhpx_stream_t stream);
+int cuhpx_alm2map(int nside, int lmax, int mmax, int batch, cuhpx_dtype_t dtype, const void* d_alm, void* d_map,
+                  void* d_workspace, size_t workspace_bytes, cuhpx_stream_t stream);
+int cuhpx_alm2map_adjoint(int nside, int lmax, int mmax, int batch, cuhpx_dtype_t dtype, const void* d_gmap,
+                          void* d_galm, void* d_workspace, size_t workspace_bytes, cuhpx_stream_t stream);
+int cuhpx_map2alm_adjoint(int nside, int lmax, int mmax, int batch, cuhpx_dtype_t dtype, const void* d_galm,
+                          void* d_gmap, const double* d_ring_weights, void* d_workspace, size_t workspace_bytes,
+                          cuhpx_stream_t stream);
+
+/* ---- the two stages of each direction, individually, for per-stage
+ * measurement and stage-level parity tests.  The ring spectra live inside the workspace:
+ *   spectra[b][ring][m], m = 0..m_cut(ring) (entries above m_cut(ring) are neither written nor read: there
+ *   lambda_lm(theta_ring) is below 2^-110 for every l <= lmax), row stride cuhpx_spectra_stride() complex values.
+ * analysis:  F_m(ring) = w_ring sum_x p_x exp(-i m (phi0 + 2 pi x / N))   (Eq. 13, phase and alias rule of Eq. 26)
+ * synthesis: p_x = Re G_0 + 2 sum_{m>=1} Re(G_m exp(+i m (phi0 + 2 pi x / N))), times w_ring if weights are given. */
+size_t cuhpx_spectra_stride(int mmax);
+/* device pointer to the spectra buffer inside an initialised workspace (NULL if unknown workspace) */
+void* cuhpx_workspace_spectra(void* d_workspace);
+/* m_cut of every ring (host array of 4 nside - 1 ints), from an initialised workspace */
+int cuhpx_workspace_mcut(void* d_workspace, int* h_mcut);
+int cuhpx_analysis_fft_stage(const void* d_map, const double* d_ring_weights, int use_weights, void* d_workspace,
+                             cuhpx_stream_t stream);
+/* adjoint != 0 multiplies by c_m (S^T) */
+int cuhpx_analysis_legendre_stage(void* d_alm, int adjoint, void* d_workspace, cuhpx_stream_t stream);
+/* adjoint != 0 divides the input by c_m (A^T) */
+int cuhpx_synthesis_legendre_stage(const void* d_alm, int adjoint, void* d_workspace, cuhpx_stream_t stream);
+int cuhpx_synthesis_fft_stage(void* d_map, const double* d_ring_weights, int use_weights, void* d_workspace,
+                              cuhpx_stream_t stream);
+
+/* Register-only FMA loop used by bench.py to measure the FP64 / FP32 FMA peak in the same run.
+ * Writes the elapsed milliseconds of `iters` dependent-chain FMAs per thread over the whole GPU to *ms and the
+ * number of FMA instructions executed to *fma_count.  Synchronises the stream. */
+int cuhpx_fma_peak_probe(cuhpx_dtype_t dtype, int iters, float* ms, double* fma_count, cuhpx_stream_t stream);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* CUHPX_H_ */

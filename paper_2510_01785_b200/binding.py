@@ -1,0 +1,280 @@
+"""Thin Python binding of libcuhpx.so (include/cuhpx.h): argument marshalling only.
+
+Every step of the transforms runs in the CUDA kernels behind the C ABI; PyTorch is used for device memory
+and streams.  There is no CPU fallback: if the shared library is missing the import fails, and the compute
+calls raise when no CUDA device is present.
+"""
+from __future__ import annotations
+
+import ctypes
+import os
+
+import torch
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_HERE, "libcuhpx.so")
+
+CUHPX_F32, CUHPX_F64 = 0, 1
+CUHPX_OK, CUHPX_EINVAL, CUHPX_EWORKSPACE, CUHPX_EUNSUPPORTED, CUHPX_ECUDA = 0, 1, 2, 3, 4
+
+#: every symbol include/cuhpx.h declares
+EXPORTS = [
+    "cuhpx_npix", "cuhpx_nrings", "cuhpx_alm_count", "cuhpx_alm_index", "cuhpx_status_string", "cuhpx_ring_info",
+    "cuhpx_workspace_bytes", "cuhpx_workspace_init", "cuhpx_workspace_release", "cuhpx_map2alm", "cuhpx_alm2map",
+    "cuhpx_alm2map_adjoint", "cuhpx_map2alm_adjoint", "cuhpx_spectra_stride", "cuhpx_workspace_spectra",
+    "cuhpx_workspace_mcut", "cuhpx_analysis_fft_stage", "cuhpx_analysis_legendre_stage",
+    "cuhpx_synthesis_legendre_stage", "cuhpx_synthesis_fft_stage", "cuhpx_fma_peak_probe",
+]
+
+
+class CuhpxError(RuntimeError):
+    def __init__(self, status: int, what: str):
+        self.status = status
+        super().__init__(f"{what}: {status_string(status)}")
+
+
+def _load() -> ctypes.CDLL:
+    if not os.path.exists(LIB_PATH):
+        raise ImportError(
+            f"{LIB_PATH} is missing: build it with `python -m paper_2510_01785_b200.build` "
+            "(there is no CPU fallback for the cuHPX transforms)")
+    lib = ctypes.CDLL(LIB_PATH)
+    i, sz, vp = ctypes.c_int, ctypes.c_size_t, ctypes.c_void_p
+    lib.cuhpx_npix.restype = sz
+    lib.cuhpx_npix.argtypes = [i]
+    lib.cuhpx_nrings.restype = sz
+    lib.cuhpx_nrings.argtypes = [i]
+    lib.cuhpx_alm_count.restype = sz
+    lib.cuhpx_alm_count.argtypes = [i, i]
+    lib.cuhpx_alm_index.restype = sz
+    lib.cuhpx_alm_index.argtypes = [i, i, i]
+    lib.cuhpx_status_string.restype = ctypes.c_char_p
+    lib.cuhpx_status_string.argtypes = [i]
+    lib.cuhpx_ring_info.argtypes = [i, i, vp, vp, vp, vp]
+    lib.cuhpx_workspace_bytes.restype = sz
+    lib.cuhpx_workspace_bytes.argtypes = [i, i, i, i, i]
+    lib.cuhpx_workspace_init.argtypes = [i, i, i, i, i, vp, sz, vp]
+    lib.cuhpx_workspace_release.argtypes = [vp]
+    lib.cuhpx_map2alm.argtypes = [i, i, i, i, i, vp, vp, vp, vp, sz, vp]
+    lib.cuhpx_alm2map.argtypes = [i, i, i, i, i, vp, vp, vp, sz, vp]
+    lib.cuhpx_alm2map_adjoint.argtypes = [i, i, i, i, i, vp, vp, vp, sz, vp]
+    lib.cuhpx_map2alm_adjoint.argtypes = [i, i, i, i, i, vp, vp, vp, vp, sz, vp]
+    lib.cuhpx_spectra_stride.restype = sz
+    lib.cuhpx_spectra_stride.argtypes = [i]
+    lib.cuhpx_workspace_spectra.restype = vp
+    lib.cuhpx_workspace_spectra.argtypes = [vp]
+    lib.cuhpx_workspace_mcut.argtypes = [vp, vp]
+    lib.cuhpx_analysis_fft_stage.argtypes = [vp, vp, i, vp, vp]
+    lib.cuhpx_analysis_legendre_stage.argtypes = [vp, i, vp, vp]
+    lib.cuhpx_synthesis_legendre_stage.argtypes = [vp, i, vp, vp]
+    lib.cuhpx_synthesis_fft_stage.argtypes = [vp, vp, i, vp, vp]
+    lib.cuhpx_fma_peak_probe.argtypes = [i, i, vp, vp, vp]
+    return lib
+
+
+_lib = _load()
+
+
+def lib() -> ctypes.CDLL:
+    return _lib
+
+
+def status_string(status: int) -> str:
+    return _lib.cuhpx_status_string(int(status)).decode()
+
+
+def _check(status: int, what: str) -> None:
+    if status != CUHPX_OK:
+        raise CuhpxError(status, what)
+
+
+def cuhpx_npix(nside: int) -> int:
+    return int(_lib.cuhpx_npix(nside))
+
+
+def cuhpx_nrings(nside: int) -> int:
+    return int(_lib.cuhpx_nrings(nside))
+
+
+def cuhpx_alm_count(lmax: int, mmax: int) -> int:
+    return int(_lib.cuhpx_alm_count(lmax, mmax))
+
+
+def cuhpx_alm_index(lmax: int, l: int, m: int) -> int:
+    return int(_lib.cuhpx_alm_index(lmax, l, m))
+
+
+def cuhpx_spectra_stride(mmax: int) -> int:
+    return int(_lib.cuhpx_spectra_stride(mmax))
+
+
+def cuhpx_ring_info(nside: int, ring: int):
+    n, s = ctypes.c_longlong(), ctypes.c_longlong()
+    c, p = ctypes.c_double(), ctypes.c_double()
+    _check(_lib.cuhpx_ring_info(nside, ring, ctypes.byref(n), ctypes.byref(s), ctypes.byref(c), ctypes.byref(p)),
+           "cuhpx_ring_info")
+    return n.value, s.value, c.value, p.value
+
+
+def cuhpx_workspace_bytes(nside: int, lmax: int, mmax: int, batch: int, dtype: int) -> int:
+    return int(_lib.cuhpx_workspace_bytes(nside, lmax, mmax, batch, dtype))
+
+
+def _dtype_code(t: torch.dtype) -> int:
+    if t in (torch.float32, torch.complex64):
+        return CUHPX_F32
+    if t in (torch.float64, torch.complex128):
+        return CUHPX_F64
+    raise TypeError(f"unsupported dtype {t}")
+
+
+def _stream_ptr(stream) -> int:
+    if stream is None:
+        stream = torch.cuda.current_stream()
+    return int(stream.cuda_stream)
+
+
+def _dev_ptr(t: torch.Tensor | None) -> int | None:
+    if t is None:
+        return None
+    if not t.is_cuda or not t.is_contiguous():
+        raise ValueError("cuhpx needs contiguous CUDA tensors")
+    return t.data_ptr()
+
+
+def cuhpx_workspace_init(nside, lmax, mmax, batch, dtype, workspace: torch.Tensor, stream=None) -> None:
+    _check(_lib.cuhpx_workspace_init(nside, lmax, mmax, batch, dtype, _dev_ptr(workspace),
+                                     workspace.numel() * workspace.element_size(), _stream_ptr(stream)),
+           "cuhpx_workspace_init")
+
+
+def cuhpx_workspace_release(workspace: torch.Tensor) -> None:
+    _lib.cuhpx_workspace_release(workspace.data_ptr())
+
+
+def _ws_args(ws: torch.Tensor):
+    return _dev_ptr(ws), ws.numel() * ws.element_size()
+
+
+def cuhpx_map2alm(nside, lmax, mmax, batch, dtype, d_map, d_alm, d_ring_weights, workspace, stream=None) -> None:
+    p, n = _ws_args(workspace)
+    _check(_lib.cuhpx_map2alm(nside, lmax, mmax, batch, dtype, _dev_ptr(d_map), _dev_ptr(d_alm),
+                              _dev_ptr(d_ring_weights), p, n, _stream_ptr(stream)), "cuhpx_map2alm")
+
+
+def cuhpx_alm2map(nside, lmax, mmax, batch, dtype, d_alm, d_map, workspace, stream=None) -> None:
+    p, n = _ws_args(workspace)
+    _check(_lib.cuhpx_alm2map(nside, lmax, mmax, batch, dtype, _dev_ptr(d_alm), _dev_ptr(d_map), p, n,
+                              _stream_ptr(stream)), "cuhpx_alm2map")
+
+
+def cuhpx_alm2map_adjoint(nside, lmax, mmax, batch, dtype, d_gmap, d_galm, workspace, stream=None) -> None:
+    p, n = _ws_args(workspace)
+    _check(_lib.cuhpx_alm2map_adjoint(nside, lmax, mmax, batch, dtype, _dev_ptr(d_gmap), _dev_ptr(d_galm), p, n,
+                                      _stream_ptr(stream)), "cuhpx_alm2map_adjoint")
+
+
+def cuhpx_map2alm_adjoint(nside, lmax, mmax, batch, dtype, d_galm, d_gmap, d_ring_weights, workspace,
+                          stream=None) -> None:
+    p, n = _ws_args(workspace)
+    _check(_lib.cuhpx_map2alm_adjoint(nside, lmax, mmax, batch, dtype, _dev_ptr(d_galm), _dev_ptr(d_gmap),
+                                      _dev_ptr(d_ring_weights), p, n, _stream_ptr(stream)), "cuhpx_map2alm_adjoint")
+
+
+def cuhpx_analysis_fft_stage(d_map, d_ring_weights, use_weights, workspace, stream=None) -> None:
+    _check(_lib.cuhpx_analysis_fft_stage(_dev_ptr(d_map), _dev_ptr(d_ring_weights), int(use_weights),
+                                         _dev_ptr(workspace), _stream_ptr(stream)), "cuhpx_analysis_fft_stage")
+
+
+def cuhpx_analysis_legendre_stage(d_alm, adjoint, workspace, stream=None) -> None:
+    _check(_lib.cuhpx_analysis_legendre_stage(_dev_ptr(d_alm), int(adjoint), _dev_ptr(workspace),
+                                              _stream_ptr(stream)), "cuhpx_analysis_legendre_stage")
+
+
+def cuhpx_synthesis_legendre_stage(d_alm, adjoint, workspace, stream=None) -> None:
+    _check(_lib.cuhpx_synthesis_legendre_stage(_dev_ptr(d_alm), int(adjoint), _dev_ptr(workspace),
+                                               _stream_ptr(stream)), "cuhpx_synthesis_legendre_stage")
+
+
+def cuhpx_synthesis_fft_stage(d_map, d_ring_weights, use_weights, workspace, stream=None) -> None:
+    _check(_lib.cuhpx_synthesis_fft_stage(_dev_ptr(d_map), _dev_ptr(d_ring_weights), int(use_weights),
+                                          _dev_ptr(workspace), _stream_ptr(stream)), "cuhpx_synthesis_fft_stage")
+
+
+def cuhpx_workspace_mcut(workspace: torch.Tensor, nside: int):
+    import numpy as np
+
+    out = np.zeros(4 * nside - 1, dtype=np.int32)
+    _check(_lib.cuhpx_workspace_mcut(_dev_ptr(workspace), out.ctypes.data_as(ctypes.c_void_p)),
+           "cuhpx_workspace_mcut")
+    return out
+
+
+def cuhpx_fma_peak_probe(dtype: int, iters: int, stream=None):
+    """(milliseconds, FMA instructions executed) of a register-only FMA loop over the whole GPU."""
+    ms, cnt = ctypes.c_float(), ctypes.c_double()
+    _check(_lib.cuhpx_fma_peak_probe(dtype, iters, ctypes.byref(ms), ctypes.byref(cnt), _stream_ptr(stream)),
+           "cuhpx_fma_peak_probe")
+    return ms.value, cnt.value
+
+
+class Transform:
+    """Convenience holder of a workspace for fixed (nside, lmax, mmax, batch, dtype): the call a user makes.
+
+    Tensors: maps are real [batch, npix]; alm are complex [batch, nalm] (m-major packed, see cuhpx.h).
+    """
+
+    def __init__(self, nside: int, lmax: int, mmax: int | None = None, batch: int = 1,
+                 dtype: torch.dtype = torch.float64, device="cuda", ring_weights: torch.Tensor | None = None):
+        if not torch.cuda.is_available():
+            raise RuntimeError("cuhpx needs a CUDA device (no CPU fallback)")
+        mmax = lmax if mmax is None else mmax
+        self.nside, self.lmax, self.mmax, self.batch = nside, lmax, mmax, batch
+        self.rdtype = dtype
+        self.cdtype = torch.complex64 if dtype == torch.float32 else torch.complex128
+        self.code = _dtype_code(dtype)
+        self.device = torch.device(device)
+        self.npix = cuhpx_npix(nside)
+        self.nalm = cuhpx_alm_count(lmax, mmax)
+        nbytes = cuhpx_workspace_bytes(nside, lmax, mmax, batch, self.code)
+        if nbytes == 0:
+            raise CuhpxError(CUHPX_EINVAL, "cuhpx_workspace_bytes")
+        self.workspace = torch.empty((nbytes + 7) // 8, dtype=torch.int64, device=self.device)
+        self.ring_weights = None
+        if ring_weights is not None:
+            self.ring_weights = ring_weights.to(device=self.device, dtype=torch.float64).contiguous()
+        with torch.cuda.device(self.device):
+            cuhpx_workspace_init(nside, lmax, mmax, batch, self.code, self.workspace)
+
+    def __del__(self):
+        try:
+            cuhpx_workspace_release(self.workspace)
+        except Exception:
+            pass
+
+    def _args(self):
+        return self.nside, self.lmax, self.mmax, self.batch, self.code
+
+    def map2alm(self, hmap: torch.Tensor, out: torch.Tensor | None = None) -> torch.Tensor:
+        assert hmap.shape == (self.batch, self.npix) and hmap.dtype == self.rdtype
+        alm = torch.empty(self.batch, self.nalm, dtype=self.cdtype, device=self.device) if out is None else out
+        cuhpx_map2alm(*self._args(), hmap, alm, self.ring_weights, self.workspace)
+        return alm
+
+    def alm2map(self, alm: torch.Tensor, out: torch.Tensor | None = None) -> torch.Tensor:
+        assert alm.shape == (self.batch, self.nalm) and alm.dtype == self.cdtype
+        hmap = torch.empty(self.batch, self.npix, dtype=self.rdtype, device=self.device) if out is None else out
+        cuhpx_alm2map(*self._args(), alm, hmap, self.workspace)
+        return hmap
+
+    def alm2map_adjoint(self, gmap: torch.Tensor, out: torch.Tensor | None = None) -> torch.Tensor:
+        assert gmap.shape == (self.batch, self.npix) and gmap.dtype == self.rdtype
+        galm = torch.empty(self.batch, self.nalm, dtype=self.cdtype, device=self.device) if out is None else out
+        cuhpx_alm2map_adjoint(*self._args(), gmap, galm, self.workspace)
+        return galm
+
+    def map2alm_adjoint(self, galm: torch.Tensor, out: torch.Tensor | None = None) -> torch.Tensor:
+        assert galm.shape == (self.batch, self.nalm) and galm.dtype == self.cdtype
+        gmap = torch.empty(self.batch, self.npix, dtype=self.rdtype, device=self.device) if out is None else out
+        cuhpx_map2alm_adjoint(*self._args(), galm, gmap, self.ring_weights, self.workspace)
+        return gmap

@@ -1,0 +1,526 @@
+// Legendre stage of the HEALPix SHT:
+//   analysis : a_lm = sum_j lambda_lm(theta_j) [F_m(N_j) + (-1)^(l+m) F_m(S_j)]          (Eq. 14, Eq. 26)
+//   synthesis: G_m(N_j) = E + O, G_m(S_j) = E - O,  E/O = sum_{l, (l+m) even/odd} a_lm lambda_lm(theta_j)  (Eq. 24)
+// lambda_lm is generated on the fly by the three-term recurrence of Eq. 16 from exponent-scaled
+// seeds lambda_mm (Eq. 15); nothing is precomputed per (l, m, ring) -- the paper's stored Legendre
+// tensor and its out-of-core streaming do not exist here.
+//
+// Thread mapping: one block = one m, one chunk of ring pairs, one group of BT channels.  Each thread owns R
+// ring pairs (lanes = adjacent rings) and walks l = m .. lmax carrying (lambda_{l}, lambda_{l-1}) in fp64
+// registers.  cos(theta) enters as x p = p - y p with y = 1 - cos(theta) (R3).
+#include <cuda_runtime.h>
+#include <math.h>
+
+#include "cuhpx_internal.h"
+
+namespace cuhpx {
+
+constexpr int LEG_THREADS = 256;
+constexpr int LEG_WARPS = LEG_THREADS / 32;
+constexpr int CT = 64;  // recurrence-coefficient tile (l values per __syncthreads)
+
+template <typename T> struct Vec2;
+template <> struct Vec2<float> { using type = float2; };
+template <> struct Vec2<double> { using type = double2; };
+
+// Exponent windows of the scaled recurrence.  true lambda = val * 2^(K * sc), sc <= 0.  A ring is "inactive"
+// while sc < 0; then |true lambda| < 2^(THR + 56 - K): 2^-200 (fp64) / 2^-44 (fp32 outputs), i.e. it cannot
+// change the result.  56 = log2 of the largest growth over the 8 steps between two checks.
+template <typename T> struct ScaleCfg;
+template <> struct ScaleCfg<double> { static constexpr int THR = 256, K = 512; };
+template <> struct ScaleCfg<float> { static constexpr int THR = 60, K = 160; };
+__host__ __device__ constexpr double pow2c(int e) {
+    double v = 1.0;
+    for (int i = 0; i < (e < 0 ? -e : e); ++i) v = e < 0 ? v * 0.5 : v * 2.0;
+    return v;
+}
+constexpr int CHECK_EVERY = 8;  // l steps between rescale checks (must divide CT and be a multiple of LT)
+
+// log2|lambda_mm(theta_j)| = pref[m] + m log2 sin(theta_j), evaluated in double-double so that the seed is
+// good to ~1e-16 relative even when the exponent is in the thousands.
+template <typename T>
+__device__ __forceinline__ void lambda_seed(int m, double pref_hi, double pref_lo, double ls_hi, double ls_lo,
+                                            double& val, int& sc) {
+    const double dm = (double)m;
+    const double p = dm * ls_hi;
+    const double pe = fma(dm, ls_hi, -p);
+    const double s = p + pref_hi;
+    const double bb = s - p;
+    const double se = (p - (s - bb)) + (pref_hi - bb);
+    const double lo = pe + se + fma(dm, ls_lo, pref_lo);
+    const double n = rint(s + lo);
+    const double f = (s - n) + lo;
+    const double mant = exp2(f);
+    int ni = (int)fmax(n, -2.0e9);
+    sc = 0;
+    constexpr int THR = ScaleCfg<T>::THR, K = ScaleCfg<T>::K;
+    if (ni < THR - K) {
+        // floor((ni - THR) / K) + 1, written for negative numerators
+        const int num = ni - THR;
+        const int fl = -((-num + K - 1) / K);
+        sc = fl + 1;
+        ni -= K * sc;
+    }
+    val = scalbn(mant, ni);
+    if (m & 1) val = -val;
+}
+
+// recurrence coefficients for degree l (>= m + 1):  lambda_l = A x lambda_{l-1} + B lambda_{l-2}
+__device__ __forceinline__ void recurrence_coeff(int l, int m, double& A, double& B) {
+    const double dl = (double)l, dm = (double)m;
+    const double l2m2 = (dl - dm) * (dl + dm);  // exact: < 2^53
+    A = sqrt((4.0 * dl * dl - 1.0) / l2m2);
+    const double num = (2.0 * dl + 1.0) * ((dl - 1.0 - dm) * (dl - 1.0 + dm));
+    const double den = (2.0 * dl - 3.0) * l2m2;
+    B = (num == 0.0) ? 0.0 : -sqrt(num / den);
+}
+
+struct LegArgs {
+    DevPlan p;
+    const void* in;  // analysis: unused (spectra from plan); synthesis: alm
+    void* out;       // analysis: alm or partial; synthesis: unused
+    int adjoint;
+    int to_partial;  // analysis: write [chunk][batch][nalm] partial sums
+};
+
+// sum NV per-thread values across the 32 lanes; afterwards lane L holds, in v[0 .. Q-1], the totals of the
+// values with index Q * (L >> SH) + q, Q = max(NV / 32, 1), SH = max(5 - log2 NV, 0).
+template <typename T, int NV>
+__device__ __forceinline__ void warp_transpose_reduce(T (&v)[NV], int lane) {
+    int n = NV;
+#pragma unroll
+    for (int mask = 16; mask >= 1; mask >>= 1) {
+        if (n > 1) {
+            const int h = n / 2;
+            const bool up = (lane & mask) != 0;
+#pragma unroll
+            for (int i = 0; i < NV / 2; ++i) {
+                if (i < h) {
+                    const T send = up ? v[i] : v[i + h];
+                    const T keep = up ? v[i + h] : v[i];
+                    v[i] = keep + __shfl_xor_sync(0xffffffffu, send, mask);
+                }
+            }
+            n = h;
+        } else {
+            v[0] += __shfl_xor_sync(0xffffffffu, v[0], mask);
+        }
+    }
+}
+
+// ------------------------------------------------------------------ analysis (row a3)
+template <typename T, int BT, int R, int LT>
+__global__ void __launch_bounds__(LEG_THREADS) legendre_analysis_kernel(LegArgs a) {
+    using T2 = typename Vec2<T>::type;
+    constexpr int NV = LT * BT * 2;
+    constexpr int Q = NV >= 32 ? NV / 32 : 1;
+    constexpr int SH = NV >= 32 ? 0 : (NV == 16 ? 1 : NV == 8 ? 2 : NV == 4 ? 3 : 4);
+    static_assert(CHECK_EVERY % LT == 0 && CT % CHECK_EVERY == 0, "tile sizes");
+    static_assert(NV <= LEG_THREADS && NV >= 2, "reduction tile");
+    const DevPlan& P = a.p;
+    const int m = blockIdx.x;
+    const int chunk = blockIdx.y;
+    const int ch0 = blockIdx.z * BT;
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const int jbase = P.jmin[m] + chunk * (LEG_THREADS * R);
+    if (jbase >= P.npairs) return;
+
+    __shared__ double sA[2][CT], sB[2][CT];
+    __shared__ T red[2][LEG_WARPS][NV];
+
+    const T2* spectra = reinterpret_cast<const T2*>(P.spectra);
+    double cur[R], prev[R], y[R];
+    int sc[R];
+    T fs[R][BT][2], fa[R][BT][2];  // F_N + F_S and F_N - F_S of the ACTIVE rings (zero while inactive)
+    int nact = 0;
+    const double pref_hi = P.pref_hi[m], pref_lo = P.pref_lo[m];
+
+    auto load_F = [&](int r) {
+        const int j = jbase + tid + LEG_THREADS * r;
+        const int rn = j, rs = P.nrings - 1 - j;
+#pragma unroll
+        for (int c = 0; c < BT; ++c) {
+            const int ch = min(ch0 + c, P.batch - 1);
+            const T2 fn = spectra[((size_t)ch * P.nrings + rn) * P.mstride + m];
+            T2 fsv;
+            fsv.x = 0;
+            fsv.y = 0;
+            if (rs != rn) fsv = spectra[((size_t)ch * P.nrings + rs) * P.mstride + m];
+            fs[r][c][0] = fn.x + fsv.x;
+            fs[r][c][1] = fn.y + fsv.y;
+            fa[r][c][0] = fn.x - fsv.x;
+            fa[r][c][1] = fn.y - fsv.y;
+        }
+    };
+
+#pragma unroll
+    for (int r = 0; r < R; ++r) {
+        const int j = jbase + tid + LEG_THREADS * r;
+#pragma unroll
+        for (int c = 0; c < BT; ++c) fs[r][c][0] = fs[r][c][1] = fa[r][c][0] = fa[r][c][1] = 0;
+        if (j < P.npairs) {
+            y[r] = P.y[j];
+            lambda_seed<T>(m, pref_hi, pref_lo, P.ls_hi[j], P.ls_lo[j], cur[r], sc[r]);
+            prev[r] = 0.0;
+            if (sc[r] == 0) {
+                load_F(r);
+                ++nact;
+            }
+        } else {  // padding lane: never active, recurrence on zeros
+            y[r] = 1.0;
+            cur[r] = 0.0;
+            prev[r] = 0.0;
+            sc[r] = -1;
+        }
+    }
+
+    const double outscale = (a.adjoint && m > 0) ? 2.0 : 1.0;
+    const long long abase = (long long)m * (2LL * P.lmax + 1 - m) / 2;  // index of (l = 0, m) in packed alm
+    T* out = reinterpret_cast<T*>(a.out);
+    if (a.to_partial) out += (size_t)chunk * P.batch * P.nalm * 2;
+
+    const int nl = P.lmax - m + 1;  // l values of this m
+    bool block_active = false;
+    int buf = 0;
+    for (int t0 = 0; t0 < nl; t0 += CT) {
+        // coefficients of degrees l = m + t0 + 1 + i (the step that produces lambda_{l}) for this tile
+        const int cb = (t0 / CT) & 1;
+        if (tid < CT) recurrence_coeff(m + t0 + 1 + tid, m, sA[cb][tid], sB[cb][tid]);
+        __syncthreads();
+        const int tend = min(CT, nl - t0);
+        for (int s0 = 0; s0 < tend; s0 += LT) {
+            if ((s0 % CHECK_EVERY) == 0) {
+#pragma unroll
+                for (int r = 0; r < R; ++r) {
+                    if (sc[r] < 0 && fabs(cur[r]) > pow2c(ScaleCfg<T>::THR)) {
+                        cur[r] *= pow2c(-ScaleCfg<T>::K);
+                        prev[r] *= pow2c(-ScaleCfg<T>::K);
+                        if (++sc[r] == 0) {
+                            load_F(r);
+                            ++nact;
+                        }
+                    }
+                }
+                if (!block_active) block_active = __syncthreads_or(nact > 0);
+            }
+            T acc[NV];
+#pragma unroll
+            for (int i = 0; i < NV; ++i) acc[i] = 0;
+            if (block_active) {
+#pragma unroll
+                for (int i = 0; i < LT; ++i) {
+                    const double A = sA[cb][s0 + i], B = sB[cb][s0 + i];
+#pragma unroll
+                    for (int r = 0; r < R; ++r) {
+                        const T lam = (T)cur[r];
+#pragma unroll
+                        for (int c = 0; c < BT; ++c) {
+                            // (t0 + s0 + i) = l - m; even -> symmetric combination
+                            if (((s0 + i) & 1) == 0) {
+                                acc[(i * BT + c) * 2 + 0] = fma(lam, fs[r][c][0], acc[(i * BT + c) * 2 + 0]);
+                                acc[(i * BT + c) * 2 + 1] = fma(lam, fs[r][c][1], acc[(i * BT + c) * 2 + 1]);
+                            } else {
+                                acc[(i * BT + c) * 2 + 0] = fma(lam, fa[r][c][0], acc[(i * BT + c) * 2 + 0]);
+                                acc[(i * BT + c) * 2 + 1] = fma(lam, fa[r][c][1], acc[(i * BT + c) * 2 + 1]);
+                            }
+                        }
+                        const double xl = fma(-y[r], cur[r], cur[r]);
+                        const double nx = fma(A, xl, B * prev[r]);
+                        prev[r] = cur[r];
+                        cur[r] = nx;
+                    }
+                }
+                warp_transpose_reduce<T, NV>(acc, lane);
+                if ((lane & ((1 << SH) - 1)) == 0) {
+#pragma unroll
+                    for (int q = 0; q < Q; ++q) red[buf][warp][Q * (lane >> SH) + q] = acc[q];
+                }
+            } else {
+#pragma unroll
+                for (int i = 0; i < LT; ++i) {
+                    const double A = sA[cb][s0 + i], B = sB[cb][s0 + i];
+#pragma unroll
+                    for (int r = 0; r < R; ++r) {
+                        const double xl = fma(-y[r], cur[r], cur[r]);
+                        const double nx = fma(A, xl, B * prev[r]);
+                        prev[r] = cur[r];
+                        cur[r] = nx;
+                    }
+                }
+            }
+            if (block_active) __syncthreads();
+            if (tid < NV) {
+                T sum = 0;
+                if (block_active) {
+#pragma unroll
+                    for (int w = 0; w < LEG_WARPS; ++w) sum += red[buf][w][tid];
+                }
+                const int i = tid / (BT * 2), c = (tid / 2) % BT, ri = tid & 1;
+                const int k = t0 + s0 + i;  // l - m
+                const int ch = ch0 + c;
+                if (k < nl && ch < P.batch) {
+                    T v = (T)(outscale * (double)sum);
+                    if (m == 0 && ri == 1) v = 0;  // Im a_l0 is exactly zero
+                    out[((size_t)ch * P.nalm + abase + m + k) * 2 + ri] = v;
+                }
+            }
+            buf ^= 1;
+        }
+    }
+}
+
+// sum the per-chunk partial results: alm[b][idx] = sum_c partial[c][b][idx], c < nchunks(m)
+template <typename T>
+__global__ void combine_partials_kernel(DevPlan P, const T* __restrict__ partial, T* __restrict__ alm) {
+    const int m = blockIdx.x;
+    const int b = blockIdx.y;
+    const int nch = (P.npairs - P.jmin[m] + P.chunk_pairs - 1) / P.chunk_pairs;
+    const long long base = ((long long)m * (2LL * P.lmax + 1 - m) / 2 + m) * 2;
+    const int n = (P.lmax - m + 1) * 2;
+    const size_t cstride = (size_t)P.batch * P.nalm * 2;
+    for (int i = threadIdx.x; i < n; i += blockDim.x) {
+        T s = 0;
+        for (int c = 0; c < nch; ++c) s += partial[c * cstride + (size_t)b * P.nalm * 2 + base + i];
+        alm[(size_t)b * P.nalm * 2 + base + i] = s;
+    }
+}
+
+// ------------------------------------------------------------------ synthesis (row s1)
+template <typename T, int BT, int R>
+__global__ void __launch_bounds__(LEG_THREADS) legendre_synthesis_kernel(LegArgs a) {
+    using T2 = typename Vec2<T>::type;
+    const DevPlan& P = a.p;
+    const int m = blockIdx.x;
+    const int chunk = blockIdx.y;
+    const int ch0 = blockIdx.z * BT;
+    const int tid = threadIdx.x;
+    const int jbase = P.jmin[m] + chunk * (LEG_THREADS * R);
+    if (jbase >= P.npairs) return;
+
+    __shared__ double sA[CT], sB[CT];
+    __shared__ T sAlm[CT][BT][2];
+
+    double cur[R], prev[R], y[R];
+    int sc[R];
+    T E[R][BT][2], O[R][BT][2];
+    const double pref_hi = P.pref_hi[m], pref_lo = P.pref_lo[m];
+#pragma unroll
+    for (int r = 0; r < R; ++r) {
+        const int j = jbase + tid + LEG_THREADS * r;
+#pragma unroll
+        for (int c = 0; c < BT; ++c) E[r][c][0] = E[r][c][1] = O[r][c][0] = O[r][c][1] = 0;
+        if (j < P.npairs) {
+            y[r] = P.y[j];
+            lambda_seed<T>(m, pref_hi, pref_lo, P.ls_hi[j], P.ls_lo[j], cur[r], sc[r]);
+            prev[r] = 0.0;
+        } else {
+            y[r] = 1.0;
+            cur[r] = 0.0;
+            prev[r] = 0.0;
+            sc[r] = -1;
+        }
+    }
+    const T inscale = (a.adjoint && m > 0) ? (T)0.5 : (T)1;
+    const long long abase = (long long)m * (2LL * P.lmax + 1 - m) / 2;
+    const T* alm = reinterpret_cast<const T*>(a.in);
+    const int nl = P.lmax - m + 1;
+
+    for (int t0 = 0; t0 < nl; t0 += CT) {
+        __syncthreads();  // previous tile fully consumed
+        if (tid < CT) recurrence_coeff(m + t0 + 1 + tid, m, sA[tid], sB[tid]);
+        for (int e = tid; e < CT * BT * 2; e += LEG_THREADS) {
+            const int i = e / (BT * 2), c = (e / 2) % BT, ri = e & 1;
+            const int k = t0 + i;
+            const int ch = ch0 + c;
+            T v = 0;
+            if (k < nl && ch < P.batch) v = inscale * alm[((size_t)ch * P.nalm + abase + m + k) * 2 + ri];
+            if (m == 0 && ri == 1) v = 0;  // Im a_l0 is ignored
+            sAlm[i][c][ri] = v;
+        }
+        __syncthreads();
+        const int tend = min(CT, nl - t0);
+        for (int s0 = 0; s0 < tend; s0 += CHECK_EVERY) {
+            bool any = false;
+#pragma unroll
+            for (int r = 0; r < R; ++r) {
+                if (sc[r] < 0) {
+                    if (fabs(cur[r]) > pow2c(ScaleCfg<T>::THR)) {
+                        cur[r] *= pow2c(-ScaleCfg<T>::K);
+                        prev[r] *= pow2c(-ScaleCfg<T>::K);
+                        ++sc[r];
+                    }
+                    // whatever was accumulated while the ring was inactive is noise below 2^-200 / 2^-44: drop it
+#pragma unroll
+                    for (int c = 0; c < BT; ++c) E[r][c][0] = E[r][c][1] = O[r][c][0] = O[r][c][1] = 0;
+                }
+                any |= (sc[r] == 0);
+            }
+            const bool warp_active = __any_sync(0xffffffffu, any);
+            if (warp_active) {
+#pragma unroll
+                for (int i = 0; i < CHECK_EVERY; ++i) {
+                    const double A = sA[s0 + i], B = sB[s0 + i];
+#pragma unroll
+                    for (int r = 0; r < R; ++r) {
+                        const T lam = (T)cur[r];
+#pragma unroll
+                        for (int c = 0; c < BT; ++c) {
+                            const T ar = sAlm[s0 + i][c][0], ai = sAlm[s0 + i][c][1];
+                            if ((i & 1) == 0) {
+                                E[r][c][0] = fma(lam, ar, E[r][c][0]);
+                                E[r][c][1] = fma(lam, ai, E[r][c][1]);
+                            } else {
+                                O[r][c][0] = fma(lam, ar, O[r][c][0]);
+                                O[r][c][1] = fma(lam, ai, O[r][c][1]);
+                            }
+                        }
+                        const double xl = fma(-y[r], cur[r], cur[r]);
+                        const double nx = fma(A, xl, B * prev[r]);
+                        prev[r] = cur[r];
+                        cur[r] = nx;
+                    }
+                }
+            } else {
+#pragma unroll
+                for (int i = 0; i < CHECK_EVERY; ++i) {
+                    const double A = sA[s0 + i], B = sB[s0 + i];
+#pragma unroll
+                    for (int r = 0; r < R; ++r) {
+                        const double xl = fma(-y[r], cur[r], cur[r]);
+                        const double nx = fma(A, xl, B * prev[r]);
+                        prev[r] = cur[r];
+                        cur[r] = nx;
+                    }
+                }
+            }
+        }
+    }
+
+    T2* spectra = reinterpret_cast<T2*>(P.spectra);
+#pragma unroll
+    for (int r = 0; r < R; ++r) {
+        const int j = jbase + tid + LEG_THREADS * r;
+        if (j >= P.npairs) continue;
+        const int rn = j, rs = P.nrings - 1 - j;
+        const bool live = sc[r] == 0;
+#pragma unroll
+        for (int c = 0; c < BT; ++c) {
+            const int ch = ch0 + c;
+            if (ch >= P.batch) continue;
+            T2 gn, gs;
+            gn.x = live ? E[r][c][0] + O[r][c][0] : (T)0;
+            gn.y = live ? E[r][c][1] + O[r][c][1] : (T)0;
+            gs.x = live ? E[r][c][0] - O[r][c][0] : (T)0;
+            gs.y = live ? E[r][c][1] - O[r][c][1] : (T)0;
+            spectra[((size_t)ch * P.nrings + rn) * P.mstride + m] = gn;
+            if (rs != rn) spectra[((size_t)ch * P.nrings + rs) * P.mstride + m] = gs;
+        }
+    }
+}
+
+// ------------------------------------------------------------------ launch configuration
+// R (ring pairs per thread) and LT (l values per reduction tile) per instantiation.
+template <typename T, int BT> struct LegCfg;
+template <> struct LegCfg<double, 1> { static constexpr int R = 4, LT = 8, RS = 4; };
+template <> struct LegCfg<float, 1> { static constexpr int R = 4, LT = 8, RS = 4; };
+template <> struct LegCfg<float, 4> { static constexpr int R = 2, LT = 4, RS = 2; };
+
+int legendre_chunk_pairs(cuhpx_dtype_t dt, int batch) {
+    if (dt == CUHPX_F64) return LEG_THREADS * LegCfg<double, 1>::R;
+    return batch >= 4 ? LEG_THREADS * LegCfg<float, 4>::R : LEG_THREADS * LegCfg<float, 1>::R;
+}
+
+template <typename T, int BT>
+static cudaError_t run_analysis(const HostPlan& hp, void* d_alm, int adjoint, cudaStream_t st) {
+    using C = LegCfg<T, BT>;
+    const DevPlan& P = hp.d;
+    LegArgs a;
+    a.p = P;
+    a.in = nullptr;
+    a.adjoint = adjoint;
+    a.to_partial = P.nchunk_max > 1;
+    a.out = a.to_partial ? P.partial : d_alm;
+    dim3 grid(P.mmax + 1, P.nchunk_max, (P.batch + BT - 1) / BT);
+    legendre_analysis_kernel<T, BT, C::R, C::LT><<<grid, LEG_THREADS, 0, st>>>(a);
+    cudaError_t e = cudaGetLastError();
+    if (e != cudaSuccess) return e;
+    if (a.to_partial) {
+        dim3 g2(P.mmax + 1, P.batch);
+        combine_partials_kernel<T><<<g2, 256, 0, st>>>(P, reinterpret_cast<const T*>(P.partial),
+                                                        reinterpret_cast<T*>(d_alm));
+        e = cudaGetLastError();
+    }
+    return e;
+}
+
+template <typename T, int BT>
+static cudaError_t run_synthesis(const HostPlan& hp, const void* d_alm, int adjoint, cudaStream_t st) {
+    using C = LegCfg<T, BT>;
+    const DevPlan& P = hp.d;
+    LegArgs a;
+    a.p = P;
+    a.in = d_alm;
+    a.out = nullptr;
+    a.adjoint = adjoint;
+    a.to_partial = 0;
+    const int chunk = LEG_THREADS * C::RS;
+    dim3 grid(P.mmax + 1, (P.npairs + chunk - 1) / chunk, (P.batch + BT - 1) / BT);
+    legendre_synthesis_kernel<T, BT, C::RS><<<grid, LEG_THREADS, 0, st>>>(a);
+    return cudaGetLastError();
+}
+
+cudaError_t launch_legendre_analysis(const HostPlan& hp, void* d_alm, int adjoint, cudaStream_t st) {
+    if (hp.dtype == CUHPX_F64) return run_analysis<double, 1>(hp, d_alm, adjoint, st);
+    if (hp.d.batch >= 4) return run_analysis<float, 4>(hp, d_alm, adjoint, st);
+    return run_analysis<float, 1>(hp, d_alm, adjoint, st);
+}
+
+cudaError_t launch_legendre_synthesis(const HostPlan& hp, const void* d_alm, int adjoint, cudaStream_t st) {
+    if (hp.dtype == CUHPX_F64) return run_synthesis<double, 1>(hp, d_alm, adjoint, st);
+    if (hp.d.batch >= 4) return run_synthesis<float, 4>(hp, d_alm, adjoint, st);
+    return run_synthesis<float, 1>(hp, d_alm, adjoint, st);
+}
+
+// ------------------------------------------------------------------ FMA peak probe
+template <typename T>
+__global__ void fma_probe_kernel(int iters, T* sink) {
+    T a0 = (T)threadIdx.x * (T)1e-3, a1 = a0 + 1, a2 = a0 + 2, a3 = a0 + 3, a4 = a0 + 4, a5 = a0 + 5, a6 = a0 + 6,
+      a7 = a0 + 7;
+    const T b = (T)0.999999, c = (T)1e-6;
+    for (int i = 0; i < iters; ++i) {
+        a0 = fma(a0, b, c); a1 = fma(a1, b, c); a2 = fma(a2, b, c); a3 = fma(a3, b, c);
+        a4 = fma(a4, b, c); a5 = fma(a5, b, c); a6 = fma(a6, b, c); a7 = fma(a7, b, c);
+    }
+    const T s = a0 + a1 + a2 + a3 + a4 + a5 + a6 + a7;
+    if (s == (T)-12345.678) sink[0] = s;
+}
+
+cudaError_t fma_peak_probe(cuhpx_dtype_t dt, int iters, float* ms, double* count, cudaStream_t st) {
+    int dev = 0, sms = 0;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e != cudaSuccess) return e;
+    e = cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+    if (e != cudaSuccess) return e;
+    const int blocks = sms * 8, threads = 256;
+    cudaEvent_t e0, e1;
+    if ((e = cudaEventCreate(&e0)) != cudaSuccess) return e;
+    if ((e = cudaEventCreate(&e1)) != cudaSuccess) return e;
+    for (int rep = 0; rep < 2; ++rep) {  // first launch warms up
+        cudaEventRecord(e0, st);
+        if (dt == CUHPX_F64) fma_probe_kernel<double><<<blocks, threads, 0, st>>>(iters, (double*)nullptr);
+        else fma_probe_kernel<float><<<blocks, threads, 0, st>>>(iters, (float*)nullptr);
+        cudaEventRecord(e1, st);
+        e = cudaEventSynchronize(e1);
+        if (e != cudaSuccess) break;
+    }
+    if (e == cudaSuccess) e = cudaGetLastError();
+    if (e == cudaSuccess) {
+        cudaEventElapsedTime(ms, e0, e1);
+        *count = (double)blocks * threads * 8.0 * (double)iters;
+    }
+    cudaEventDestroy(e0);
+    cudaEventDestroy(e1);
+    return e;
+}
+
+}  // namespace cuhpx

@@ -1,0 +1,224 @@
+"""GPU parity: the CUDA path (through the C ABI) against the CPU oracle, element by element, on the same
+seeded inputs.  Tolerances are north_star's: fp64 max|d|/max|ref| <= 1e-11, fp32 relative L2 <= 2e-5."""
+import numpy as np
+import pytest
+
+import oracle
+from paper_2510_01785_b200 import synth
+
+torch = pytest.importorskip("torch")
+pytestmark = pytest.mark.gpu
+
+TOL64 = 1e-11
+TOL32 = 2e-5
+
+
+def _binding():
+    from paper_2510_01785_b200 import binding
+
+    return binding
+
+
+def err64(got, ref):
+    return float(np.abs(got - ref).max() / np.abs(ref).max())
+
+
+def err32(got, ref):
+    return float(np.linalg.norm((got - ref).ravel()) / np.linalg.norm(ref.ravel()))
+
+
+def check(got, ref, dtype):
+    if dtype == "f64":
+        e = err64(got, ref)
+        assert e <= TOL64, f"fp64 max-norm relative error {e:.3e} > {TOL64}"
+    else:
+        e = err32(got, ref)
+        assert e <= TOL32, f"fp32 relative L2 error {e:.3e} > {TOL32}"
+    return e
+
+
+def make_transform(nside, lmax, mmax, batch, dtype, weights=None):
+    B = _binding()
+    tdt = torch.float64 if dtype == "f64" else torch.float32
+    w = None if weights is None else torch.from_numpy(weights)
+    return B.Transform(nside, lmax, mmax, batch, tdt, "cuda:0", ring_weights=w)
+
+
+def to_dev(a, dtype, complex_=False):
+    if complex_:
+        t = torch.from_numpy(np.ascontiguousarray(a)).to(torch.complex128 if dtype == "f64" else torch.complex64)
+    else:
+        t = torch.from_numpy(np.ascontiguousarray(a)).to(torch.float64 if dtype == "f64" else torch.float32)
+    return t.cuda()
+
+
+def rounded(a, dtype, complex_=False):
+    """What the oracle sees: the inputs after their one rounding to the transform's dtype."""
+    if dtype == "f64":
+        return a
+    return a.astype(np.complex64).astype(np.complex128) if complex_ else a.astype(np.float32).astype(np.float64)
+
+
+def run_all_four(nside, lmax, mmax, batch, dtype, seed, weights=None, channels_checked=None):
+    """All four operators against the full oracle; returns the four error figures."""
+    T = make_transform(nside, lmax, mmax, batch, dtype, weights)
+    fmap = synth.gaussian_map(seed, nside, batch)
+    alm = synth.powerlaw_alm(seed, lmax, mmax, batch)
+    galm = synth.white_alm(seed, lmax, mmax, batch)
+    chans = range(batch) if channels_checked is None else channels_checked
+    out = {}
+
+    got = T.map2alm(to_dev(fmap, dtype)).cpu().numpy().astype(np.complex128)
+    ref = np.stack([oracle.map2alm(nside, lmax, mmax, rounded(fmap[c], dtype), weights) for c in chans])
+    out["map2alm"] = check(got[list(chans)], ref, dtype)
+    assert np.all(got[:, : lmax + 1].imag == 0.0), "Im a_l0 must be exactly zero"
+
+    got = T.alm2map(to_dev(alm, dtype, True)).cpu().numpy().astype(np.float64)
+    ref = np.stack([oracle.alm2map(nside, lmax, mmax, rounded(alm[c], dtype, True)) for c in chans])
+    out["alm2map"] = check(got[list(chans)], ref, dtype)
+
+    got = T.alm2map_adjoint(to_dev(fmap, dtype)).cpu().numpy().astype(np.complex128)
+    ref = np.stack([oracle.alm2map_adjoint(nside, lmax, mmax, rounded(fmap[c], dtype)) for c in chans])
+    out["alm2map_adjoint"] = check(got[list(chans)], ref, dtype)
+
+    got = T.map2alm_adjoint(to_dev(galm, dtype, True)).cpu().numpy().astype(np.float64)
+    ref = np.stack([oracle.map2alm_adjoint(nside, lmax, mmax, rounded(galm[c], dtype, True), weights) for c in chans])
+    out["map2alm_adjoint"] = check(got[list(chans)], ref, dtype)
+    return out
+
+
+# ----------------------------------------------------------------------------- BASELINE configs 1-3
+
+def test_cfg1_all_four_fp64():
+    """configs[0]: nside 32, lmax = mmax = 64 (= equatorial Nyquist), batch 1, fp64; full oracle."""
+    errs = run_all_four(32, 64, 64, 1, "f64", 101)
+    print("cfg1", errs)
+
+
+def test_cfg1_weighted_fp64():
+    """Same with non-uniform, non-symmetric ring weights."""
+    errs = run_all_four(32, 64, 64, 1, "f64", 101, weights=synth.ring_weights(101, 32))
+    print("cfg1 weighted", errs)
+
+
+def test_cfg2_both_directions_fp64():
+    """configs[1]: nside 256, lmax = mmax = 511: alm -> map (both sides), then analysis of the ORACLE's map on
+    both sides, plus the adjoint dot-product identities on the GPU results."""
+    nside, lmax = 256, 511
+    T = make_transform(nside, lmax, lmax, 1, "f64")
+    alm = synth.powerlaw_alm(202, lmax, lmax, 1)
+    ref_map = oracle.alm2map(nside, lmax, lmax, alm[0])
+    got_map = T.alm2map(to_dev(alm, "f64", True)).cpu().numpy()[0]
+    check(got_map, ref_map, "f64")
+    ref_alm = oracle.map2alm(nside, lmax, lmax, ref_map)
+    got_alm = T.map2alm(to_dev(ref_map[None], "f64")).cpu().numpy()[0]
+    check(got_alm, ref_alm, "f64")
+    # adjoint dot products with fresh cotangents
+    g = synth.gaussian_map(203, nside, 1)
+    b = synth.white_alm(204, lmax, lmax, 1)
+    b[:, : lmax + 1] = b[:, : lmax + 1].real
+    a = alm.copy()
+    st_g = T.alm2map_adjoint(to_dev(g, "f64")).cpu().numpy()[0]
+    lhs = float(got_map @ g[0])
+    rhs = float((a[0].real * st_g.real + a[0].imag * st_g.imag).sum())
+    assert abs(lhs - rhs) <= 1e-11 * max(abs(lhs), 1.0)
+    at_b = T.map2alm_adjoint(to_dev(b, "f64", True)).cpu().numpy()[0]
+    lhs = float((got_alm.real * b[0].real + got_alm.imag * b[0].imag).sum())
+    rhs = float(ref_map @ at_b)
+    assert abs(lhs - rhs) <= 1e-11 * max(abs(lhs), 1.0)
+    check(st_g, oracle.alm2map_adjoint(nside, lmax, lmax, g[0]), "f64")
+    check(at_b, oracle.map2alm_adjoint(nside, lmax, lmax, b[0]), "f64")
+
+
+def test_cfg3_batched_fp32_training_step():
+    """configs[2]: nside 64, lmax = mmax = 128, 256 channels fp32: map2alm forward then map2alm_adjoint backward
+    with random upstream alm gradients; full oracle on every channel."""
+    nside, lmax, batch = 64, 128, 256
+    T = make_transform(nside, lmax, lmax, batch, "f32")
+    fmap = synth.gaussian_map(303, nside, batch)
+    galm = synth.white_alm(303, lmax, lmax, batch)
+    got = T.map2alm(to_dev(fmap, "f32")).cpu().numpy().astype(np.complex128)
+    ref = np.stack([oracle.map2alm(nside, lmax, lmax, rounded(fmap[c], "f32")) for c in range(batch)])
+    e1 = check(got, ref, "f32")
+    for c in (0, 17, 255):  # per-channel too: no channel hides behind the others
+        check(got[c], ref[c], "f32")
+    got = T.map2alm_adjoint(to_dev(galm, "f32", True)).cpu().numpy().astype(np.float64)
+    ref = np.stack([oracle.map2alm_adjoint(nside, lmax, lmax, rounded(galm[c], "f32", True)) for c in range(batch)])
+    e2 = check(got, ref, "f32")
+    print("cfg3", e1, e2)
+
+
+# ----------------------------------------------------------------------------- small, ragged and degenerate cases
+
+@pytest.mark.parametrize("nside,lmax,mmax,batch,dtype", [
+    (1, 0, 0, 1, "f64"), (1, 3, 3, 1, "f64"), (2, 8, 8, 2, "f64"), (4, 16, 16, 1, "f64"), (4, 11, 7, 3, "f64"),
+    (8, 16, 0, 1, "f64"), (16, 40, 33, 1, "f64"), (16, 47, 47, 5, "f32"), (8, 23, 23, 1, "f32"),
+    (64, 200, 150, 2, "f64"), (32, 95, 95, 7, "f32"), (128, 300, 300, 1, "f64"),
+])
+def test_small_and_ragged_cases(nside, lmax, mmax, batch, dtype):
+    """mmax < lmax, lmax far above 2 nside (every polar ring aliases), batch not a multiple of the channel
+    tile, lmax not a multiple of any l tile, single-coefficient transforms (lmax = 0)."""
+    w = synth.ring_weights(7, nside) if (nside + batch) % 2 == 0 else None
+    run_all_four(nside, lmax, mmax, batch, dtype, 1000 + nside + lmax, weights=w)
+
+
+def test_fft_stage_alone_matches_ring_dft():
+    """Stage-level parity: spectra written by the analysis FFT stage against the oracle's
+    direct ring DFT, ring by ring, for every m the stage is required to produce."""
+    B = _binding()
+    nside, lmax = 16, 40
+    T = make_transform(nside, lmax, lmax, 2, "f64")
+    fmap = synth.gaussian_map(55, nside, 2)
+    B.cuhpx_analysis_fft_stage(to_dev(fmap, "f64"), None, 0, T.workspace)
+    torch.cuda.synchronize()
+    mcut = B.cuhpx_workspace_mcut(T.workspace, nside)
+    stride = B.cuhpx_spectra_stride(lmax)
+    nrings = 4 * nside - 1
+    nbytes = 2 * nrings * stride * 16
+    ptr = B.lib().cuhpx_workspace_spectra(T.workspace.data_ptr())
+    off = (ptr - T.workspace.data_ptr()) // 8
+    spec = T.workspace[off: off + nbytes // 8].view(torch.float64).cpu().numpy().view(np.complex128)
+    spec = spec.reshape(2, nrings, stride)
+    for ring in range(1, nrings + 1):
+        n, start = oracle.ring_geometry(nside, ring)[:2]
+        assert mcut[ring - 1] >= min(lmax, 2)  # low orders are needed on every ring
+        for c in range(2):
+            ref = oracle.ring_dft(nside, ring, fmap[c, start:start + n], lmax)
+            mc = mcut[ring - 1]
+            np.testing.assert_allclose(spec[c, ring - 1, : mc + 1], ref[: mc + 1], atol=1e-12 * n)
+
+
+def test_outputs_are_overwritten_and_inputs_untouched():
+    nside, lmax = 8, 16
+    T = make_transform(nside, lmax, lmax, 1, "f64")
+    fmap = to_dev(synth.gaussian_map(1, nside, 1), "f64")
+    keep = fmap.clone()
+    out = torch.full((1, T.nalm), 7.0 + 3.0j, dtype=torch.complex128, device="cuda")
+    a1 = T.map2alm(fmap, out=out).clone()
+    a2 = T.map2alm(fmap, out=out).clone()
+    assert torch.equal(fmap, keep) and torch.equal(a1, a2)
+    m1 = T.alm2map(a1, out=torch.full((1, T.npix), 5.0, dtype=torch.float64, device="cuda"))
+    m2 = T.alm2map(a1)
+    assert torch.equal(m1, m2)
+
+
+def test_stream_ordering_and_error_codes():
+    B = _binding()
+    nside, lmax = 8, 16
+    T = make_transform(nside, lmax, lmax, 1, "f64")
+    fmap = to_dev(synth.gaussian_map(2, nside, 1), "f64")
+    s = torch.cuda.Stream()
+    ref = T.map2alm(fmap)
+    torch.cuda.synchronize()
+    with torch.cuda.stream(s):
+        got = T.map2alm(fmap)
+    s.synchronize()
+    assert torch.equal(ref, got)
+    # a workspace initialised for other parameters is refused
+    alm = torch.empty(1, T.nalm, dtype=torch.complex128, device="cuda")
+    with pytest.raises(B.CuhpxError) as ei:
+        B.cuhpx_map2alm(nside, lmax, lmax - 1, 1, B.CUHPX_F64, fmap, alm, None, T.workspace)
+    assert ei.value.status == B.CUHPX_EWORKSPACE
+    with pytest.raises(B.CuhpxError) as ei:
+        B.cuhpx_map2alm(nside, lmax, lmax, 1, B.CUHPX_F32, fmap, alm, None, T.workspace)
+    assert ei.value.status == B.CUHPX_EWORKSPACE
