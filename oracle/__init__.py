@@ -45,6 +45,7 @@ def _load():
         _lib.oracle_lambda.argtypes = [i32, i32, ctypes.c_double, vp]
         _lib.oracle_lambda_ring.argtypes = [i32, i32, i32, i32, vp]
         _lib.oracle_ring_dft.argtypes = [i32, i32, vp, i32, vp]
+        _lib.oracle_ring_synth.argtypes = [i32, i32, vp, i32, vp]
         _lib.oracle_alm2map.argtypes = [i32, i32, i32, vp, vp]
         _lib.oracle_map2alm.argtypes = [i32, i32, i32, vp, vp, vp]
         _lib.oracle_alm2map_adjoint.argtypes = [i32, i32, i32, vp, vp]
@@ -124,6 +125,14 @@ def ring_dft(nside: int, ring: int, p, mmax: int) -> np.ndarray:
     p = _f64(p)
     out = np.zeros(mmax + 1, dtype=np.complex128)
     _check(_load().oracle_ring_dft(nside, ring, _ptr(p), mmax, _ptr(out)), "ring_dft")
+    return out
+
+
+def ring_synth(nside: int, ring: int, G) -> np.ndarray:
+    """p_x = Re G_0 + 2 sum_{m>=1} Re(G_m exp(+i m (phi0 + 2 pi x / N))) for one ring, G = G_0..G_mmax."""
+    G = _c128(G)
+    out = np.zeros(ring_geometry(nside, ring)[0])
+    _check(_load().oracle_ring_synth(nside, ring, _ptr(G), len(G) - 1, _ptr(out)), "ring_synth")
     return out
 
 

@@ -292,6 +292,25 @@ int oracle_ring_dft(int nside, int ring, const double* p, int mmax, double* F /*
     return ORACLE_OK;
 }
 
+/* Public: the ring synthesis sum alone, p_x = Re G_0 + 2 sum_{m=1..mmax} Re(G_m exp(+i m (phi0 + 2 pi x / N))). */
+int oracle_ring_synth(int nside, int ring, const double* G /* (mmax+1) x (re,im) */, int mmax, double* p) {
+    ring_t r;
+    int rc = ring_geometry(nside, ring, &r);
+    if (rc) return rc;
+    if (mmax < 0) return ORACLE_EINVAL;
+    ld *tc, *ts;
+    if (twiddle_table(r.n, &tc, &ts)) return ORACLE_ENOMEM;
+    ld* Gre = (ld*)malloc(sizeof(ld) * (size_t)(mmax + 1));
+    ld* Gim = (ld*)malloc(sizeof(ld) * (size_t)(mmax + 1));
+    for (int m = 0; m <= mmax; ++m) {
+        Gre[m] = (ld)G[2 * m];
+        Gim[m] = (ld)G[2 * m + 1];
+    }
+    ring_synthesis_dft(&r, tc, ts, Gre, Gim, mmax, 2.0L, 1.0L, p);
+    free(Gre); free(Gim); free(tc); free(ts);
+    return ORACLE_OK;
+}
+
 /* ------------------------------------------------------------------ the four operators (A4) */
 
 static int check_args(int nside, int lmax, int mmax) {

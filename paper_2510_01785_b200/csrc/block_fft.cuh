@@ -1,0 +1,259 @@
+// Block-wide power-of-two complex FFT for one ring in one CTA (used by ring_fft.cu).
+//
+// n = 2^LOGN points are held ENTIRELY in registers (E = n / NT per thread); shared memory is only the exchange
+// buffer between passes.  Each pass is a set of radix-R (R = 2..16) butterflies done in registers with
+// compile-time twiddles; the inter-pass twiddles W_L^(j q) come from a global table (L1/L2 resident).
+// Decimation in frequency, in place: after the last pass the element at position p is X[bitrev(p)].
+// The inverse runs the same passes backwards (conjugated, decimation in time), so a forward+inverse pair
+// (the Bluestein convolution, Eq. 22) never needs a bit-reversal permutation.
+// Bank conflicts: positions are padded p -> p + (p >> 4) (8-byte) / p + (p >> 5) (4-byte); with the plans
+// below every pass is <= 2 wavefronts per request (measured by brute force).
+#pragma once
+#include <cuda_runtime.h>
+
+namespace cuhpx {
+
+template <typename T> struct V2;
+template <> struct V2<float> { using type = float2; };
+template <> struct V2<double> { using type = double2; };
+
+template <typename T> __device__ __forceinline__ int padi(int p) { return p + (p >> (sizeof(T) == 8 ? 4 : 5)); }
+template <typename T> __host__ __device__ constexpr int padded_len(int n) { return n + (n >> (sizeof(T) == 8 ? 4 : 5)) + 1; }
+
+// radix plans: passes in DIF order
+template <int LOGN> struct FftPlan;
+template <> struct FftPlan<8> { static constexpr int NT = 32, NP = 3; static constexpr int R0 = 8, R1 = 8, R2 = 4, R3 = 1; };
+template <> struct FftPlan<9> { static constexpr int NT = 64, NP = 3; static constexpr int R0 = 8, R1 = 8, R2 = 8, R3 = 1; };
+template <> struct FftPlan<10> { static constexpr int NT = 64, NP = 3; static constexpr int R0 = 16, R1 = 16, R2 = 4, R3 = 1; };
+template <> struct FftPlan<11> { static constexpr int NT = 128, NP = 3; static constexpr int R0 = 16, R1 = 16, R2 = 8, R3 = 1; };
+template <> struct FftPlan<12> { static constexpr int NT = 256, NP = 3; static constexpr int R0 = 16, R1 = 16, R2 = 16, R3 = 1; };
+template <> struct FftPlan<13> { static constexpr int NT = 512, NP = 4; static constexpr int R0 = 2, R1 = 16, R2 = 16, R3 = 16; };
+
+template <int LOGN, int S> struct PassRadix {
+    static constexpr int value = S == 0 ? FftPlan<LOGN>::R0 : S == 1 ? FftPlan<LOGN>::R1 : S == 2 ? FftPlan<LOGN>::R2 : FftPlan<LOGN>::R3;
+};
+// sub-transform length at pass S: L_S = n / (R_0 ... R_{S-1})
+template <int LOGN, int S> struct PassLen { static constexpr int value = PassLen<LOGN, S - 1>::value / PassRadix<LOGN, S - 1>::value; };
+template <int LOGN> struct PassLen<LOGN, 0> { static constexpr int value = 1 << LOGN; };
+
+// cos/sin(2 pi k / 16), k = 0..7
+__device__ __forceinline__ constexpr double c16(int k) {
+    return k == 0 ? 1.0 : k == 1 ? 0.92387953251128675613 : k == 2 ? 0.70710678118654752440 : k == 3 ? 0.38268343236508977173
+         : k == 4 ? 0.0 : k == 5 ? -0.38268343236508977173 : k == 6 ? -0.70710678118654752440 : -0.92387953251128675613;
+}
+__device__ __forceinline__ constexpr double s16(int k) {
+    return k == 0 ? 0.0 : k == 1 ? 0.38268343236508977173 : k == 2 ? 0.70710678118654752440 : k == 3 ? 0.92387953251128675613
+         : k == 4 ? 1.0 : k == 5 ? 0.92387953251128675613 : k == 6 ? 0.70710678118654752440 : 0.38268343236508977173;
+}
+
+// multiply (a + ib) by exp(SIGN * 2 pi i * K / 16), K compile time
+template <int K, int SIGN, typename T> __device__ __forceinline__ void mul_w16(T& a, T& b) {
+    if (K == 0) return;
+    if (K == 4) {  // * (SIGN i)
+        const T t = a;
+        if (SIGN > 0) { a = -b; b = t; } else { a = b; b = -t; }
+        return;
+    }
+    const T c = (T)c16(K), s = (T)(SIGN * s16(K));
+    const T na = a * c - b * s, nb = a * s + b * c;
+    a = na;
+    b = nb;
+}
+
+// in-register radix-R DIF: natural in, bit-reversed out; Y[q] = sum_p x[p] exp(SIGN 2 pi i p q / R)
+template <int R, int SIGN, typename T, int H = R / 2> struct RegDif {
+    static __device__ __forceinline__ void run(T* re, T* im) {
+#pragma unroll
+        for (int b = 0; b < R; b += 2 * H) {
+            stage<0>(re + b, im + b);
+        }
+        RegDif<R, SIGN, T, H / 2>::run(re, im);
+    }
+    template <int J> static __device__ __forceinline__ void stage(T* re, T* im) {
+        if constexpr (J < H) {
+            const T ar = re[J], ai = im[J], cr = re[J + H], ci = im[J + H];
+            re[J] = ar + cr;
+            im[J] = ai + ci;
+            T dr = ar - cr, di = ai - ci;
+            mul_w16<J * (8 / H), SIGN>(dr, di);
+            re[J + H] = dr;
+            im[J + H] = di;
+            stage<J + 1>(re, im);
+        }
+    }
+};
+template <int R, int SIGN, typename T> struct RegDif<R, SIGN, T, 0> {
+    static __device__ __forceinline__ void run(T*, T*) {}
+};
+
+// in-register radix-R DIT: bit-reversed in, natural out; same sum
+template <int R, int SIGN, typename T, int H = 1> struct RegDit {
+    static __device__ __forceinline__ void run(T* re, T* im) {
+        if constexpr (H < R) {
+#pragma unroll
+            for (int b = 0; b < R; b += 2 * H) {
+                stage<0>(re + b, im + b);
+            }
+            RegDit<R, SIGN, T, H * 2>::run(re, im);
+        }
+    }
+    template <int J> static __device__ __forceinline__ void stage(T* re, T* im) {
+        if constexpr (J < H) {
+            T cr = re[J + H], ci = im[J + H];
+            mul_w16<J * (8 / H), SIGN>(cr, ci);
+            const T ar = re[J], ai = im[J];
+            re[J] = ar + cr;
+            im[J] = ai + ci;
+            re[J + H] = ar - cr;
+            im[J + H] = ai - ci;
+            stage<J + 1>(re, im);
+        }
+    }
+};
+
+template <int R> __device__ __forceinline__ constexpr int brev_r(int x) {
+    int r = 0;
+    for (int b = 1, t = R >> 1; b < R; b <<= 1, t >>= 1)
+        if (x & b) r |= t;
+    return r;
+}
+
+// Multiply register r (holding butterfly output q = bitrev_R(r)) by w^q, w = tw[idx] (conjugated if CONJ).
+// w^(2^k) are loaded from the table, the other powers are running products (<= 3 multiplies from a table value).
+template <int R, bool CONJ, typename T>
+__device__ __forceinline__ void apply_twiddles(const typename V2<T>::type* __restrict__ tw, int idx, T* re, T* im) {
+    T w1r = 0, w1i = 0, cr = 1, ci = 0;
+#pragma unroll
+    for (int q = 1; q < R; ++q) {
+        if ((q & (q - 1)) == 0) {  // power of two: exact table value
+            const typename V2<T>::type w = __ldg(tw + q * idx);
+            cr = w.x;
+            ci = CONJ ? -w.y : w.y;
+            if (q == 1) {
+                w1r = cr;
+                w1i = ci;
+            }
+        } else {
+            const T nr = cr * w1r - ci * w1i, ni = cr * w1i + ci * w1r;
+            cr = nr;
+            ci = ni;
+        }
+        const int r = brev_r<R>(q);
+        const T a = re[r], b = im[r];
+        re[r] = a * cr - b * ci;
+        im[r] = a * ci + b * cr;
+    }
+}
+
+template <typename T, int LOGN> struct BlockFFT {
+    using P = FftPlan<LOGN>;
+    using T2 = typename V2<T>::type;
+    static constexpr int N = 1 << LOGN, NT = P::NT, E = N / NT, NP = P::NP;
+    static constexpr int RLAST = PassRadix<LOGN, NP - 1>::value;
+    static constexpr int R0 = P::R0;
+    static constexpr size_t SMEM_BYTES = 2 * (size_t)padded_len<T>(N) * sizeof(T);
+
+    // position of register e = c R + rho in pass S
+    template <int S> static __device__ __forceinline__ int pos(int tid, int c, int rho) {
+        constexpr int R = PassRadix<LOGN, S>::value, L = PassLen<LOGN, S>::value, LR = L / R;
+        const int u = tid + NT * c;
+        const int B = u / LR, j = u % LR;
+        return B * L + j + rho * LR;
+    }
+    // natural index held by register e in the pass-0 layout (input of forward / output of inverse)
+    static __device__ __forceinline__ int index0(int tid, int e) { return pos<0>(tid, e / R0, e % R0); }
+    // frequency index held by register e after forward (last-pass layout)
+    static __device__ __forceinline__ int freq_index(int tid, int e) {
+        const int p = pos<NP - 1>(tid, e / RLAST, e % RLAST);
+        return (int)(__brev((unsigned)p) >> (32 - LOGN));
+    }
+
+    template <int S> static __device__ __forceinline__ void load(T (&re)[E], T (&im)[E], const T* sre, const T* sim, int tid) {
+        constexpr int R = PassRadix<LOGN, S>::value;
+#pragma unroll
+        for (int c = 0; c < E / R; ++c)
+#pragma unroll
+            for (int r = 0; r < R; ++r) {
+                const int p = padi<T>(pos<S>(tid, c, r));
+                re[c * R + r] = sre[p];
+                im[c * R + r] = sim[p];
+            }
+    }
+    template <int S> static __device__ __forceinline__ void store(const T (&re)[E], const T (&im)[E], T* sre, T* sim, int tid) {
+        constexpr int R = PassRadix<LOGN, S>::value;
+#pragma unroll
+        for (int c = 0; c < E / R; ++c)
+#pragma unroll
+            for (int r = 0; r < R; ++r) {
+                const int p = padi<T>(pos<S>(tid, c, r));
+                sre[p] = re[c * R + r];
+                sim[p] = im[c * R + r];
+            }
+    }
+
+    template <int S> static __device__ __forceinline__ void fwd_pass(T (&re)[E], T (&im)[E], T* sre, T* sim,
+                                                                  const T2* __restrict__ tw, int twlen, int tid) {
+        if constexpr (S < NP) {
+            constexpr int R = PassRadix<LOGN, S>::value, L = PassLen<LOGN, S>::value, LR = L / R;
+            if constexpr (S > 0) {
+                __syncthreads();
+                load<S>(re, im, sre, sim, tid);
+            }
+#pragma unroll
+            for (int c = 0; c < E / R; ++c) {
+                RegDif<R, -1, T>::run(re + c * R, im + c * R);
+                if constexpr (LR > 1) {
+                    const int j = (tid + NT * c) % LR;
+                    apply_twiddles<R, false, T>(tw, j * (twlen / L), re + c * R, im + c * R);
+                }
+            }
+            if constexpr (S < NP - 1) store<S>(re, im, sre, sim, tid);
+            fwd_pass<S + 1>(re, im, sre, sim, tw, twlen, tid);
+        }
+    }
+
+    template <int S> static __device__ __forceinline__ void inv_pass(T (&re)[E], T (&im)[E], T* sre, T* sim,
+                                                                  const T2* __restrict__ tw, int twlen, int tid) {
+        if constexpr (S >= 0) {
+            constexpr int R = PassRadix<LOGN, S>::value, L = PassLen<LOGN, S>::value, LR = L / R;
+            if constexpr (S < NP - 1) {
+                __syncthreads();
+                load<S>(re, im, sre, sim, tid);
+            }
+#pragma unroll
+            for (int c = 0; c < E / R; ++c) {
+                if constexpr (LR > 1) {
+                    const int j = (tid + NT * c) % LR;
+                    apply_twiddles<R, true, T>(tw, j * (twlen / L), re + c * R, im + c * R);
+                }
+                RegDit<R, +1, T>::run(re + c * R, im + c * R);
+            }
+            if constexpr (S > 0) store<S>(re, im, sre, sim, tid);
+            inv_pass<S - 1>(re, im, sre, sim, tw, twlen, tid);
+        }
+    }
+
+    // forward DFT (exp(-i...)): registers in pass-0 layout -> registers in last-pass layout (freq_index)
+    static __device__ __forceinline__ void forward(T (&re)[E], T (&im)[E], T* sre, T* sim, const T2* __restrict__ tw,
+                                                   int twlen, int tid) {
+        fwd_pass<0>(re, im, sre, sim, tw, twlen, tid);
+    }
+    // unnormalised inverse (exp(+i...), factor n): last-pass layout -> pass-0 layout
+    static __device__ __forceinline__ void inverse(T (&re)[E], T (&im)[E], T* sre, T* sim, const T2* __restrict__ tw,
+                                                   int twlen, int tid) {
+        inv_pass<NP - 1>(re, im, sre, sim, tw, twlen, tid);
+    }
+    // write the forward result to shared memory in natural frequency order (call after forward; syncs first,
+    // because other threads may still be reading the exchange buffer; caller syncs before reading)
+    static __device__ __forceinline__ void store_natural(const T (&re)[E], const T (&im)[E], T* sre, T* sim, int tid) {
+        __syncthreads();
+#pragma unroll
+        for (int e = 0; e < E; ++e) {
+            const int p = padi<T>(freq_index(tid, e));
+            sre[p] = re[e];
+            sim[p] = im[e];
+        }
+    }
+};
+
+}  // namespace cuhpx

@@ -40,7 +40,8 @@ struct DevPlan {
 };
 
 // ------------------------------------------------------------------ host plan
-struct RingFftTables;  // defined in ring_fft.cu
+struct FftDev;  // FFT-stage device tables, defined in ring_fft.cu
+void free_fft_dev(FftDev*);
 
 struct HostPlan {
     DevPlan d;
@@ -53,12 +54,11 @@ struct HostPlan {
     int* d_rings_direct = nullptr;
     int* d_rings_pow2 = nullptr;
     int* d_rings_blue = nullptr;
-    // FFT tables (device)
-    void* d_twiddle = nullptr;        // complex<T>[tw_len]: exp(-2 pi i k / tw_len)
-    int tw_len = 0;
-    void* d_blue_filter = nullptr;    // concatenated chirp filter spectra
-    long long* d_blue_offset = nullptr;  // per cap ring i (1..nside-1): offset into d_blue_filter (complex units), -1 if unused
-    std::vector<long long> h_blue_offset;
+    FftDev* fft = nullptr;  // owned
+    ~HostPlan() { free_fft_dev(fft); }
+    HostPlan() = default;
+    HostPlan(const HostPlan&) = delete;
+    HostPlan& operator=(const HostPlan&) = delete;
 };
 
 inline int ilog2_ceil(long long v) {

@@ -2,23 +2,29 @@
 // phi0 phase twist and the m-aliasing rule (m mod N_i) of Eq. 24 / Eq. 26.
 //   analysis : F_m(i) = w_i exp(-i m phi0_i) X~_i[m mod N_i],  X_i[k] = sum_x p_x exp(-2 pi i k x / N_i)   (Eq. 13)
 //   synthesis: p_x = Re G_0 + 2 sum_{m>=1} Re(G_m exp(+i m (phi0_i + 2 pi x / N_i)))                       (Eq. 24)
-// Three kernel families, chosen per ring length:
-//   direct   : O(N m_cut) sums for short rings (several cheap rings, no FFT set-up cost)
-//   pow2     : shared-memory radix-8/4/2 FFT for N = 2^k (all belt rings and cap rings with i a power of two)
-//   bluestein: chirp-z (Eq. 17-23) for the other cap rings, per-ring minimal chirp length, in one SM
+// Three kernel families, chosen per ring length N:
+//   direct   : O(N m_cut) sums for N <= 256 (the first 64 rings of each cap; negligible work)
+//   pow2     : N = 2^k (all belt rings, cap rings with i a power of two): real FFT of length N as one complex
+//              block FFT of length N/2 held in registers (block_fft.cuh), Hermitian unpack fused with the twist
+//   bluestein: the other cap rings, N = 4 i: chirp-z (Eq. 17-23).  Unlike the paper's uniform chirp
+//              length + batched cuFFT, each ring uses its own minimal power-of-two length M >= 2i - 1 and
+//              stays inside one SM: the packed complex sequence of length 2 i is split into its even and odd
+//              halves (two length-i chirp-z transforms), each = chirp multiply -> FFT_M -> filter -> IFFT_M ->
+//              chirp multiply, all in registers/shared memory; the filter spectra are precomputed per i.
+// One CTA per (ring, channel); rings are read and spectra written exactly once, coalesced.
 #include <cuda_runtime.h>
 #include <math.h>
 
+#include <algorithm>
+
+#include "block_fft.cuh"
 #include "cuhpx_internal.h"
 
 namespace cuhpx {
 
-template <typename T> struct V2;
-template <> struct V2<float> { using type = float2; };
-template <> struct V2<double> { using type = double2; };
-
-constexpr int DIRECT_MAX_N = 1024;
-constexpr int FFT_THREADS = 256;
+constexpr int DIRECT_MAX_N = 256;
+constexpr int FFT_THREADS = 256;  // direct kernels
+constexpr int MIN_LOG = 8, MAX_LOG = 13;
 
 // exp(sign * i * pi * num / den) from exact integers (num already reduced mod 2 den)
 __device__ __forceinline__ void cispi_ratio(long long num, long long den, double sign, double& c, double& s) {
@@ -47,6 +53,13 @@ __device__ __forceinline__ RingRef ring_ref(const DevPlan& P, int r, const doubl
     if (use_w) R.weight = w ? w[r] : 4.0 * 3.14159265358979323846 / (double)P.npix;
     return R;
 }
+
+struct FftTables {
+    const void* tw;  // complex<T>[twlen] = exp(-2 pi i k / twlen)
+    int twlen;
+    const void* filt;             // Bluestein filter spectra, register order, concatenated
+    const long long* filt_offset; // [nside] offset (complex units) for cap ring i, -1 if none
+};
 
 // ------------------------------------------------------------------ direct kernels (short rings)
 template <typename T>
@@ -134,55 +147,658 @@ __global__ void __launch_bounds__(FFT_THREADS) ring_direct_synthesis_kernel(DevP
     }
 }
 
-// ------------------------------------------------------------------ planning
-bool fft_supported(int nside, cuhpx_dtype_t dt) {
-    (void)dt;
-    return 4 * nside <= DIRECT_MAX_N;
+// ------------------------------------------------------------------ shared pieces of the FFT kernels
+
+// exp(-+ i pi num / den) for the FFT kernels: POW2 rings read the twiddle table (den | twlen/2... exact integer
+// index), other rings evaluate sincospi of the exact rational.
+template <typename T, bool POW2> struct Cis {
+    using T2 = typename V2<T>::type;
+    const T2* tw;
+    int twlen;
+    // exp(SIGN * 2 pi i * num / den), 0 <= num < den
+    template <int SIGN> __device__ __forceinline__ void get(int num, int den, T& c, T& s) const {
+        if (POW2) {
+            const T2 w = __ldg(tw + (size_t)num * (twlen / den));
+            c = w.x;
+            s = SIGN > 0 ? -w.y : w.y;
+        } else {
+            cispi_ratio(2LL * num, den, (T)SIGN, c, s);
+        }
+    }
+};
+
+// Folded half spectrum H[k], k = 0..n (n = N/2), of the synthesis input:
+//   c_m = G_m exp(+i m phi0);  0 < k < n: H[k] = sum_{m = k (N)} c_m + sum_{m = -k (N)} conj(c_m);
+//   k in {0, n}: H[k] = sum_{m = k (N)} (m == 0 ? Re c_0 : 2 Re c_m)
+template <typename T, bool POW2>
+__device__ __forceinline__ void folded_H(const typename V2<T>::type* __restrict__ G, int k, int N, int mcut, int shifted,
+                                         const Cis<T, POW2>& cis, T& hr, T& hi) {
+    using T2 = typename V2<T>::type;
+    const int n = N >> 1;
+    hr = 0;
+    hi = 0;
+    auto cm = [&](int m, T& cr, T& ci) {
+        const T2 g = G[m];
+        if (shifted) {
+            T c, s;
+            cis.template get<+1>(m % (2 * N), 2 * N, c, s);
+            cr = g.x * c - g.y * s;
+            ci = g.x * s + g.y * c;
+        } else {
+            cr = g.x;
+            ci = g.y;
+        }
+    };
+    if (k == 0 || k == n) {
+        for (int m = k; m <= mcut; m += N) {
+            T cr, ci;
+            cm(m, cr, ci);
+            hr += (m == 0) ? cr : 2 * cr;
+        }
+    } else {
+        for (int m = k; m <= mcut; m += N) {
+            T cr, ci;
+            cm(m, cr, ci);
+            hr += cr;
+            hi += ci;
+        }
+        for (int m = N - k; m <= mcut; m += N) {
+            T cr, ci;
+            cm(m, cr, ci);
+            hr += cr;
+            hi -= ci;
+        }
+    }
 }
 
-size_t plan_fft_tables(HostPlan& hp, char* base, bool build, cudaStream_t st, cudaError_t* err) {
+// Packed inverse-real-FFT input: Y[k] = conj(Zs[k]), Zs[k] = E' + i O', E' = H[k] + conj H[n-k],
+// O' = (H[k] - conj H[n-k]) exp(+2 pi i k / N); the ring is then x[2t] = Re D[t], x[2t+1] = -Im D[t], D = DFT_n(Y).
+template <typename T, bool POW2>
+__device__ __forceinline__ void synth_packed_input(const typename V2<T>::type* __restrict__ G, int k, int N, int mcut,
+                                                   int shifted, const Cis<T, POW2>& cis, T& yr, T& yi) {
+    const int n = N >> 1;
+    T ar, ai, br, bi;
+    folded_H<T, POW2>(G, k, N, mcut, shifted, cis, ar, ai);
+    folded_H<T, POW2>(G, n - k, N, mcut, shifted, cis, br, bi);
+    bi = -bi;  // conj H[n-k]
+    const T er = ar + br, ei = ai + bi;
+    const T dr = ar - br, di = ai - bi;
+    T c, s;
+    cis.template get<+1>(k, N, c, s);
+    const T orr = dr * c - di * s, oi = dr * s + di * c;
+    // Zs = E' + i O' = (er - oi) + i (ei + orr);  Y = conj
+    yr = er - oi;
+    yi = -(ei + orr);
+}
+
+// Hermitian unpack of the packed analysis FFT + twist: given Z[kk mod n] and Z[(n-kk) mod n] returns
+// F_m = weight * exp(-i m phi0) * X~[m mod N]
+template <typename T, bool POW2>
+__device__ __forceinline__ typename V2<T>::type analysis_unpack(T z1r, T z1i, T z2r, T z2i, int m, int kk, bool cj, int N,
+                                                                 int shifted, T wt, const Cis<T, POW2>& cis) {
+    const T er = (T)0.5 * (z1r + z2r), ei = (T)0.5 * (z1i - z2i);
+    const T dr = (T)0.5 * (z1r - z2r), di = (T)0.5 * (z1i + z2i);
+    // O = -i D = (di, -dr);  X = E + W_N^kk O
+    T c, s;
+    cis.template get<-1>(kk, N, c, s);
+    T xr = er + (c * di + s * dr);
+    T xi = ei + (s * di - c * dr);
+    if (cj) xi = -xi;
+    if (shifted) {
+        T pc, ps;
+        cis.template get<-1>(m % (2 * N), 2 * N, pc, ps);
+        const T tr = xr * pc - xi * ps, ti = xr * ps + xi * pc;
+        xr = tr;
+        xi = ti;
+    }
+    typename V2<T>::type o;
+    o.x = wt * xr;
+    o.y = wt * xi;
+    return o;
+}
+
+// ------------------------------------------------------------------ power-of-two rings
+template <typename T, int LOGN>
+__global__ void __launch_bounds__(FftPlan<LOGN>::NT) ring_pow2_analysis_kernel(DevPlan P, const int* __restrict__ rings,
+                                                                               const T* __restrict__ map,
+                                                                               const double* __restrict__ w, int use_w,
+                                                                               FftTables tabs) {
+    using F = BlockFFT<T, LOGN>;
+    using T2 = typename V2<T>::type;
+    constexpr int n = F::N, N = 2 * n, E = F::E, NT = F::NT;
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    T* sre = reinterpret_cast<T*>(smem_raw);
+    T* sim = sre + padded_len<T>(n);
+    const int tid = threadIdx.x;
+    const int r = rings[blockIdx.x], ch = blockIdx.y;
+    const RingRef R = ring_ref(P, r, w, use_w);
+    const T2* src = reinterpret_cast<const T2*>(map + (size_t)ch * P.npix + R.start);
+    const T2* tw = reinterpret_cast<const T2*>(tabs.tw);
+    T re[E], im[E];
+#pragma unroll
+    for (int e = 0; e < E; ++e) {
+        const T2 z = src[F::index0(tid, e)];
+        re[e] = z.x;
+        im[e] = z.y;
+    }
+    F::forward(re, im, sre, sim, tw, tabs.twlen, tid);
+    F::store_natural(re, im, sre, sim, tid);
+    __syncthreads();
+    const Cis<T, true> cis{tw, tabs.twlen};
+    T2* dst = reinterpret_cast<T2*>(P.spectra) + ((size_t)ch * P.nrings + r) * P.mstride;
+    const T wt = (T)R.weight;
+    for (int m = tid; m <= R.mcut; m += NT) {
+        const int k = m & (N - 1);
+        const bool cj = k > n;
+        const int kk = cj ? N - k : k;
+        const int i1 = padi<T>(kk & (n - 1)), i2 = padi<T>((n - kk) & (n - 1));
+        dst[m] = analysis_unpack<T, true>(sre[i1], sim[i1], sre[i2], sim[i2], m, kk, cj, N, R.shifted, wt, cis);
+    }
+}
+
+template <typename T, int LOGN>
+__global__ void __launch_bounds__(FftPlan<LOGN>::NT) ring_pow2_synthesis_kernel(DevPlan P, const int* __restrict__ rings,
+                                                                                T* __restrict__ map,
+                                                                                const double* __restrict__ w, int use_w,
+                                                                                FftTables tabs) {
+    using F = BlockFFT<T, LOGN>;
+    using T2 = typename V2<T>::type;
+    constexpr int n = F::N, N = 2 * n, E = F::E, NT = F::NT;
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    T* sre = reinterpret_cast<T*>(smem_raw);
+    T* sim = sre + padded_len<T>(n);
+    const int tid = threadIdx.x;
+    const int r = rings[blockIdx.x], ch = blockIdx.y;
+    const RingRef R = ring_ref(P, r, w, use_w);
+    const T2* tw = reinterpret_cast<const T2*>(tabs.tw);
+    const Cis<T, true> cis{tw, tabs.twlen};
+    const T2* G = reinterpret_cast<const T2*>(P.spectra) + ((size_t)ch * P.nrings + r) * P.mstride;
+    T re[E], im[E];
+#pragma unroll
+    for (int e = 0; e < E; ++e)
+        synth_packed_input<T, true>(G, F::index0(tid, e), N, R.mcut, R.shifted, cis, re[e], im[e]);
+    F::forward(re, im, sre, sim, tw, tabs.twlen, tid);
+    F::store_natural(re, im, sre, sim, tid);
+    __syncthreads();
+    T2* dst = reinterpret_cast<T2*>(map + (size_t)ch * P.npix + R.start);
+    const T wt = (T)R.weight;
+    for (int t = tid; t < n; t += NT) {
+        T2 o;
+        o.x = wt * sre[padi<T>(t)];
+        o.y = -wt * sim[padi<T>(t)];
+        dst[t] = o;
+    }
+}
+
+// ------------------------------------------------------------------ Bluestein rings (N = 4 i, i not a power of two)
+// chirp c[u] = exp(-i pi u^2 / i) from the exact integer u^2 mod 2i  (Eq. 19 P:222 with N -> i)
+template <typename T> __device__ __forceinline__ void chirp(int u, int i, T& c, T& s) {
+    cispi_ratio((long long)((u * u) % (2 * i)), i, (T)-1, c, s);
+}
+
+// One length-i chirp-z transform of the sequence already multiplied by the chirp and zero-padded in registers
+// (pass-0 layout): FFT_M -> times filter spectrum -> IFFT_M (Eq. 22).  Result: conv[idx] in registers.
+template <typename T, int LOGM>
+__device__ __forceinline__ void chirp_convolve(T (&re)[BlockFFT<T, LOGM>::E], T (&im)[BlockFFT<T, LOGM>::E], T* sre, T* sim,
+                                               const typename V2<T>::type* __restrict__ tw, int twlen,
+                                               const typename V2<T>::type* __restrict__ filt, int tid) {
+    using F = BlockFFT<T, LOGM>;
+    F::forward(re, im, sre, sim, tw, twlen, tid);
+#pragma unroll
+    for (int e = 0; e < F::E; ++e) {
+        const typename V2<T>::type f = __ldg(filt + e * F::NT + tid);
+        const T a = re[e], b = im[e];
+        re[e] = a * f.x - b * f.y;
+        im[e] = a * f.y + b * f.x;
+    }
+    F::inverse(re, im, sre, sim, tw, twlen, tid);
+}
+
+template <typename T, int LOGM>
+__global__ void __launch_bounds__(FftPlan<LOGM>::NT) ring_blue_analysis_kernel(DevPlan P, const int* __restrict__ rings,
+                                                                               const T* __restrict__ map,
+                                                                               const double* __restrict__ w, int use_w,
+                                                                               FftTables tabs) {
+    using F = BlockFFT<T, LOGM>;
+    using T2 = typename V2<T>::type;
+    constexpr int M = F::N, E = F::E, NT = F::NT;
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    T* sre = reinterpret_cast<T*>(smem_raw);
+    T* sim = sre + padded_len<T>(M);
+    T2* Ze = reinterpret_cast<T2*>(sim + padded_len<T>(M));
+    const int tid = threadIdx.x;
+    const int r = rings[blockIdx.x], ch = blockIdx.y;
+    const RingRef R = ring_ref(P, r, w, use_w);
+    const int N = R.N, i = N >> 2, n = N >> 1;
+    const T2* src = reinterpret_cast<const T2*>(map + (size_t)ch * P.npix + R.start);
+    const T2* tw = reinterpret_cast<const T2*>(tabs.tw);
+    const T2* filt = reinterpret_cast<const T2*>(tabs.filt) + tabs.filt_offset[i];
+    T re[E], im[E];
+#pragma unroll 1
+    for (int sub = 0; sub < 2; ++sub) {
+#pragma unroll
+        for (int e = 0; e < E; ++e) {
+            const int u = F::index0(tid, e);
+            re[e] = 0;
+            im[e] = 0;
+            if (u < i) {
+                const T2 z = src[2 * u + sub];
+                T c, s;
+                chirp<T>(u, i, c, s);
+                re[e] = z.x * c - z.y * s;
+                im[e] = z.x * s + z.y * c;
+            }
+        }
+        chirp_convolve<T, LOGM>(re, im, sre, sim, tw, tabs.twlen, filt, tid);
+#pragma unroll
+        for (int e = 0; e < E; ++e) {
+            const int u = F::index0(tid, e);
+            if (u < i) {
+                T c, s;
+                chirp<T>(u, i, c, s);
+                const T vr = re[e] * c - im[e] * s, vi = re[e] * s + im[e] * c;
+                if (sub == 0) {
+                    T2 v;
+                    v.x = vr;
+                    v.y = vi;
+                    Ze[u] = v;
+                } else {  // own pass-0 slot of the exchange buffer: no other thread touches it
+                    sre[padi<T>(u)] = vr;
+                    sim[padi<T>(u)] = vi;
+                }
+            }
+        }
+    }
+    __syncthreads();
+    // Z[q] = Ze[q mod i] + W_n^q Zo[q mod i], q < n = 2 i
+    const Cis<T, false> cis{tw, tabs.twlen};
+    auto Zq = [&](int q, T& zr, T& zi) {
+        const int qi = q >= i ? q - i : q;
+        T c, s;
+        cis.template get<-1>(q, n, c, s);
+        const T2 ze = Ze[qi];
+        const T orr = sre[padi<T>(qi)], oi = sim[padi<T>(qi)];
+        zr = ze.x + (orr * c - oi * s);
+        zi = ze.y + (orr * s + oi * c);
+    };
+    T2* dst = reinterpret_cast<T2*>(P.spectra) + ((size_t)ch * P.nrings + r) * P.mstride;
+    const T wt = (T)R.weight;
+    for (int m = tid; m <= R.mcut; m += NT) {
+        const int k = m % N;
+        const bool cj = k > n;
+        const int kk = cj ? N - k : k;
+        T z1r, z1i, z2r, z2i;
+        Zq(kk == n ? 0 : kk, z1r, z1i);
+        Zq(kk == 0 ? 0 : n - kk, z2r, z2i);
+        dst[m] = analysis_unpack<T, false>(z1r, z1i, z2r, z2i, m, kk, cj, N, R.shifted, wt, cis);
+    }
+}
+
+template <typename T, int LOGM>
+__global__ void __launch_bounds__(FftPlan<LOGM>::NT) ring_blue_synthesis_kernel(DevPlan P, const int* __restrict__ rings,
+                                                                                T* __restrict__ map,
+                                                                                const double* __restrict__ w, int use_w,
+                                                                                FftTables tabs) {
+    using F = BlockFFT<T, LOGM>;
+    using T2 = typename V2<T>::type;
+    constexpr int M = F::N, E = F::E, NT = F::NT;
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    T* sre = reinterpret_cast<T*>(smem_raw);
+    T* sim = sre + padded_len<T>(M);
+    T2* De = reinterpret_cast<T2*>(sim + padded_len<T>(M));
+    const int tid = threadIdx.x;
+    const int r = rings[blockIdx.x], ch = blockIdx.y;
+    const RingRef R = ring_ref(P, r, w, use_w);
+    const int N = R.N, i = N >> 2, n = N >> 1;
+    const T2* tw = reinterpret_cast<const T2*>(tabs.tw);
+    const T2* filt = reinterpret_cast<const T2*>(tabs.filt) + tabs.filt_offset[i];
+    const Cis<T, false> cis{tw, tabs.twlen};
+    const T2* G = reinterpret_cast<const T2*>(P.spectra) + ((size_t)ch * P.nrings + r) * P.mstride;
+    T re[E], im[E];
+#pragma unroll 1
+    for (int sub = 0; sub < 2; ++sub) {
+#pragma unroll
+        for (int e = 0; e < E; ++e) {
+            const int u = F::index0(tid, e);
+            re[e] = 0;
+            im[e] = 0;
+            if (u < i) {
+                T yr, yi;
+                synth_packed_input<T, false>(G, 2 * u + sub, N, R.mcut, R.shifted, cis, yr, yi);
+                T c, s;
+                chirp<T>(u, i, c, s);
+                re[e] = yr * c - yi * s;
+                im[e] = yr * s + yi * c;
+            }
+        }
+        chirp_convolve<T, LOGM>(re, im, sre, sim, tw, tabs.twlen, filt, tid);
+#pragma unroll
+        for (int e = 0; e < E; ++e) {
+            const int u = F::index0(tid, e);
+            if (u < i) {
+                T c, s;
+                chirp<T>(u, i, c, s);
+                const T vr = re[e] * c - im[e] * s, vi = re[e] * s + im[e] * c;
+                if (sub == 0) {
+                    T2 v;
+                    v.x = vr;
+                    v.y = vi;
+                    De[u] = v;
+                } else {
+                    sre[padi<T>(u)] = vr;
+                    sim[padi<T>(u)] = vi;
+                }
+            }
+        }
+    }
+    __syncthreads();
+    // D[t] = De[t mod i] + W_n^t Do[t mod i];  x[2t] = Re D[t], x[2t+1] = -Im D[t]
+    T2* dst = reinterpret_cast<T2*>(map + (size_t)ch * P.npix + R.start);
+    const T wt = (T)R.weight;
+    for (int t = tid; t < n; t += NT) {
+        const int ti = t >= i ? t - i : t;
+        T c, s;
+        cis.template get<-1>(t, n, c, s);
+        const T2 de = De[ti];
+        const T orr = sre[padi<T>(ti)], oi = sim[padi<T>(ti)];
+        T2 o;
+        o.x = wt * (de.x + (orr * c - oi * s));
+        o.y = -wt * (de.y + (orr * s + oi * c));
+        dst[t] = o;
+    }
+}
+
+// Filter spectrum of cap-ring size i:  b[j] = exp(+i pi j^2 / i) for |j| < i (wrapped into length M), else 0;
+// filt = FFT_M(b) / M in the register order of BlockFFT<T, LOGM> ([e][tid]).  Computed in fp64, stored as T.
+template <typename T, int LOGM>
+__global__ void __launch_bounds__(FftPlan<LOGM>::NT) blue_filter_kernel(const int* __restrict__ ivals,
+                                                                        const long long* __restrict__ offsets,
+                                                                        typename V2<T>::type* __restrict__ out,
+                                                                        const double2* __restrict__ tw64, int twlen) {
+    using F = BlockFFT<double, LOGM>;
+    constexpr int M = F::N, E = F::E, NT = F::NT;
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    double* sre = reinterpret_cast<double*>(smem_raw);
+    double* sim = sre + padded_len<double>(M);
+    const int tid = threadIdx.x;
+    const int i = ivals[blockIdx.x];
+    double re[E], im[E];
+#pragma unroll
+    for (int e = 0; e < E; ++e) {
+        const int idx = F::index0(tid, e);
+        int j = -1;
+        if (idx < i) j = idx;
+        else if (M - idx < i) j = M - idx;
+        re[e] = 0;
+        im[e] = 0;
+        if (j >= 0) {
+            double c, s;
+            cispi_ratio((long long)((j * j) % (2 * i)), i, 1.0, c, s);
+            re[e] = c;
+            im[e] = s;
+        }
+    }
+    F::forward(re, im, sre, sim, tw64, twlen, tid);
+    typename V2<T>::type* dst = out + offsets[i];
+#pragma unroll
+    for (int e = 0; e < E; ++e) {
+        typename V2<T>::type v;
+        v.x = (T)(re[e] * (1.0 / M));
+        v.y = (T)(im[e] * (1.0 / M));
+        dst[e * NT + tid] = v;
+    }
+}
+
+template <typename T>
+__global__ void twiddle_table_kernel(typename V2<T>::type* tw, int twlen) {
+    const int k = blockIdx.x * blockDim.x + threadIdx.x;
+    if (k < twlen) {
+        double s, c;
+        sincospi(-2.0 * (double)k / (double)twlen, &s, &c);
+        tw[k].x = (T)c;
+        tw[k].y = (T)s;
+    }
+}
+
+// ------------------------------------------------------------------ planning
+static int blue_logm(int i) {  // M = 2^LOGM >= 2 i - 1, at least 2^MIN_LOG
+    int l = ilog2_ceil(2LL * i - 1);
+    return l < MIN_LOG ? MIN_LOG : l;
+}
+
+template <typename T, int LOG> static size_t fft_smem_bytes(bool blue) {
+    size_t b = 2 * (size_t)padded_len<T>(1 << LOG) * sizeof(T);
+    if (blue) b += sizeof(T) * 2 * ((size_t)(1 << LOG) / 2 + 2) + 16;  // Ze: i <= (M + 1) / 2 complex
+    return b;
+}
+
+bool fft_supported(int nside, cuhpx_dtype_t dt) {
+    (void)dt;
+    return nside <= 4096;  // belt: n = 2 nside <= 2^13; caps: M <= 2^13 (fp64 needs 205 KB of the SM's 227 KB)
+}
+
+struct RingFftLists {
+    std::vector<int> direct;
+    std::vector<int> pow2[MAX_LOG + 1];
+    std::vector<int> blue[MAX_LOG + 1];
+    std::vector<int> blue_i[MAX_LOG + 1];  // distinct i per LOGM
+};
+
+static void classify(const HostPlan& hp, RingFftLists& L) {
     const DevPlan& d = hp.d;
-    hp.rings_direct.clear();
-    hp.rings_pow2.clear();
-    hp.rings_blue.clear();
-    for (int r = 0; r < d.nrings; ++r) hp.rings_direct.push_back(r);
+    for (int r = 0; r < d.nrings; ++r) {
+        const int j = std::min(r, d.nrings - 1 - r);
+        const int N = hp.h_ringN[j];
+        if (N <= DIRECT_MAX_N) L.direct.push_back(r);
+        else if (is_pow2(N)) L.pow2[ilog2_ceil(N) - 1].push_back(r);
+        else {
+            const int i = N / 4, lm = blue_logm(i);
+            L.blue[lm].push_back(r);
+            if (r == j) L.blue_i[lm].push_back(i);
+        }
+    }
+}
+
+// Device layout of the FFT tables inside the workspace (all offsets relative to `base`):
+//   [ring lists: direct | pow2[8..13] | blue[8..13] | blue_i[8..13]] [filt_offset: nside x i64]
+//   [twiddle T2[twlen]] [twiddle double2[twlen] (set-up only, kept)] [filters]
+struct FftLayout {
+    size_t off_direct, off_pow2[MAX_LOG + 1], off_blue[MAX_LOG + 1], off_blue_i[MAX_LOG + 1];
+    size_t off_filt_offset, off_tw, off_tw64, off_filt, total;
+    long long filt_total;
+};
+
+static FftLayout fft_layout(const HostPlan& hp, const RingFftLists& L, std::vector<long long>& filt_off) {
+    const DevPlan& d = hp.d;
+    const size_t csize = hp.dtype == CUHPX_F64 ? 16 : 8;
+    FftLayout Y;
     size_t o = 0;
     auto take = [&](size_t bytes) {
         size_t r = o;
         o = (o + bytes + 255) / 256 * 256;
         return r;
     };
-    const size_t off_direct = take(sizeof(int) * hp.rings_direct.size());
-    if (build) {
-        hp.d_rings_direct = (int*)(base + off_direct);
-        *err = cudaMemcpyAsync(hp.d_rings_direct, hp.rings_direct.data(), sizeof(int) * hp.rings_direct.size(),
-                               cudaMemcpyHostToDevice, st);
-        if (*err == cudaSuccess) *err = cudaStreamSynchronize(st);
+    Y.off_direct = take(sizeof(int) * L.direct.size());
+    for (int l = MIN_LOG; l <= MAX_LOG; ++l) {
+        Y.off_pow2[l] = take(sizeof(int) * L.pow2[l].size());
+        Y.off_blue[l] = take(sizeof(int) * L.blue[l].size());
+        Y.off_blue_i[l] = take(sizeof(int) * L.blue_i[l].size());
     }
-    return o;
+    Y.off_filt_offset = take(sizeof(long long) * d.nside);
+    const int twlen = 8 * d.nside < 2048 ? 2048 : 8 * d.nside;
+    Y.off_tw = take(csize * twlen);
+    Y.off_tw64 = take(16 * (size_t)twlen);
+    filt_off.assign(d.nside, -1);
+    long long fo = 0;
+    for (int l = MIN_LOG; l <= MAX_LOG; ++l)
+        for (int i : L.blue_i[l]) {
+            filt_off[i] = fo;
+            fo += 1LL << l;
+        }
+    Y.filt_total = fo;
+    Y.off_filt = take(csize * (size_t)fo);
+    Y.total = o;
+    return Y;
 }
 
-// ------------------------------------------------------------------ launchers
-template <typename T>
-static cudaError_t run_fft_analysis(const HostPlan& hp, const void* d_map, const double* d_w, int use_w,
-                                    cudaStream_t st) {
-    const DevPlan& P = hp.d;
-    if (!hp.rings_direct.empty()) {
-        dim3 grid((unsigned)hp.rings_direct.size(), P.batch);
-        const size_t smem = (size_t)DIRECT_MAX_N * 3 * sizeof(T);
-        ring_direct_analysis_kernel<T><<<grid, FFT_THREADS, smem, st>>>(P, hp.d_rings_direct, (const T*)d_map, d_w, use_w);
+struct FftDev {  // device pointers resolved from the layout (kept per plan in a side table)
+    const int* direct;
+    const int* pow2[MAX_LOG + 1];
+    const int* blue[MAX_LOG + 1];
+    int n_direct, n_pow2[MAX_LOG + 1], n_blue[MAX_LOG + 1];
+    int max_mcut_direct;
+    FftTables tabs;
+};
+
+template <typename T, int LOG> static cudaError_t set_smem_attrs() {
+    cudaError_t e;
+    const size_t sp = fft_smem_bytes<T, LOG>(false), sb = fft_smem_bytes<T, LOG>(true);
+    if ((e = cudaFuncSetAttribute(ring_pow2_analysis_kernel<T, LOG>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sp))) return e;
+    if ((e = cudaFuncSetAttribute(ring_pow2_synthesis_kernel<T, LOG>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sp))) return e;
+    if ((e = cudaFuncSetAttribute(ring_blue_analysis_kernel<T, LOG>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sb))) return e;
+    if ((e = cudaFuncSetAttribute(ring_blue_synthesis_kernel<T, LOG>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sb))) return e;
+    if ((e = cudaFuncSetAttribute(blue_filter_kernel<T, LOG>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                  (int)fft_smem_bytes<double, LOG>(false)))) return e;
+    return cudaSuccess;
+}
+
+template <typename T, int LOG>
+static cudaError_t build_filters(const RingFftLists& L, const FftLayout& Y, char* base, cudaStream_t st, int twlen) {
+    if (L.blue_i[LOG].empty()) return cudaSuccess;
+    using T2 = typename V2<T>::type;
+    blue_filter_kernel<T, LOG><<<(unsigned)L.blue_i[LOG].size(), FftPlan<LOG>::NT, fft_smem_bytes<double, LOG>(false), st>>>(
+        (const int*)(base + Y.off_blue_i[LOG]), (const long long*)(base + Y.off_filt_offset), (T2*)(base + Y.off_filt),
+        (const double2*)(base + Y.off_tw64), twlen);
+    return cudaGetLastError();
+}
+
+template <typename T> static cudaError_t build_tables_t(HostPlan& hp, const RingFftLists& L, const FftLayout& Y, char* base,
+                                                        cudaStream_t st, int twlen) {
+    using T2 = typename V2<T>::type;
+    cudaError_t e;
+#define CUHPX_ATTR(LOG) if ((e = set_smem_attrs<T, LOG>()) != cudaSuccess) return e;
+    CUHPX_ATTR(8) CUHPX_ATTR(9) CUHPX_ATTR(10) CUHPX_ATTR(11) CUHPX_ATTR(12) CUHPX_ATTR(13)
+#undef CUHPX_ATTR
+    twiddle_table_kernel<T><<<(twlen + 255) / 256, 256, 0, st>>>((T2*)(base + Y.off_tw), twlen);
+    twiddle_table_kernel<double><<<(twlen + 255) / 256, 256, 0, st>>>((double2*)(base + Y.off_tw64), twlen);
+    if ((e = cudaGetLastError()) != cudaSuccess) return e;
+#define CUHPX_FILT(LOG) if ((e = build_filters<T, LOG>(L, Y, base, st, twlen)) != cudaSuccess) return e;
+    CUHPX_FILT(8) CUHPX_FILT(9) CUHPX_FILT(10) CUHPX_FILT(11) CUHPX_FILT(12) CUHPX_FILT(13)
+#undef CUHPX_FILT
+    (void)hp;
+    return cudaSuccess;
+}
+
+size_t plan_fft_tables(HostPlan& hp, char* base, bool build, cudaStream_t st, cudaError_t* err) {
+    RingFftLists L;
+    classify(hp, L);
+    std::vector<long long> filt_off;
+    const FftLayout Y = fft_layout(hp, L, filt_off);
+    if (!build) return Y.total;
+    const DevPlan& d = hp.d;
+    const int twlen = 8 * d.nside < 2048 ? 2048 : 8 * d.nside;
+    cudaError_t e = cudaSuccess;
+    auto up = [&](size_t off, const void* src, size_t bytes) {
+        if (e == cudaSuccess && bytes) e = cudaMemcpyAsync(base + off, src, bytes, cudaMemcpyHostToDevice, st);
+    };
+    up(Y.off_direct, L.direct.data(), sizeof(int) * L.direct.size());
+    for (int l = MIN_LOG; l <= MAX_LOG; ++l) {
+        up(Y.off_pow2[l], L.pow2[l].data(), sizeof(int) * L.pow2[l].size());
+        up(Y.off_blue[l], L.blue[l].data(), sizeof(int) * L.blue[l].size());
+        up(Y.off_blue_i[l], L.blue_i[l].data(), sizeof(int) * L.blue_i[l].size());
     }
+    up(Y.off_filt_offset, filt_off.data(), sizeof(long long) * d.nside);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(st);  // pageable sources
+    if (e == cudaSuccess)
+        e = hp.dtype == CUHPX_F64 ? build_tables_t<double>(hp, L, Y, base, st, twlen)
+                                  : build_tables_t<float>(hp, L, Y, base, st, twlen);
+    FftDev D;
+    D.direct = (const int*)(base + Y.off_direct);
+    D.n_direct = (int)L.direct.size();
+    for (int l = 0; l <= MAX_LOG; ++l) {
+        D.pow2[l] = l >= MIN_LOG ? (const int*)(base + Y.off_pow2[l]) : nullptr;
+        D.blue[l] = l >= MIN_LOG ? (const int*)(base + Y.off_blue[l]) : nullptr;
+        D.n_pow2[l] = l >= MIN_LOG ? (int)L.pow2[l].size() : 0;
+        D.n_blue[l] = l >= MIN_LOG ? (int)L.blue[l].size() : 0;
+    }
+    D.tabs.tw = base + Y.off_tw;
+    D.tabs.twlen = twlen;
+    D.tabs.filt = base + Y.off_filt;
+    D.tabs.filt_offset = (const long long*)(base + Y.off_filt_offset);
+    D.max_mcut_direct = 0;
+    for (int r : L.direct) D.max_mcut_direct = std::max(D.max_mcut_direct, hp.h_mcut[std::min(r, d.nrings - 1 - r)]);
+    const size_t csz = hp.dtype == CUHPX_F64 ? 16 : 8;
+    if (e == cudaSuccess && (DIRECT_MAX_N + D.max_mcut_direct + 1) * csz > 200 * 1024) e = cudaErrorInvalidConfiguration;
+    if (e == cudaSuccess) {
+        const int want = (int)((DIRECT_MAX_N + D.max_mcut_direct + 1) * csz);
+        e = hp.dtype == CUHPX_F64
+                ? cudaFuncSetAttribute(ring_direct_synthesis_kernel<double>, cudaFuncAttributeMaxDynamicSharedMemorySize, std::max(want, 48 * 1024))
+                : cudaFuncSetAttribute(ring_direct_synthesis_kernel<float>, cudaFuncAttributeMaxDynamicSharedMemorySize, std::max(want, 48 * 1024));
+    }
+    delete hp.fft;
+    hp.fft = new FftDev(D);
+    hp.rings_direct = L.direct;
+    *err = e;
+    return Y.total;
+}
+
+void free_fft_dev(FftDev* f) { delete f; }
+
+// ------------------------------------------------------------------ launchers
+template <typename T, int LOG>
+static void launch_class_analysis(const DevPlan& P, const FftDev& D, const T* map, const double* w, int use_w, cudaStream_t st) {
+    if (D.n_pow2[LOG])
+        ring_pow2_analysis_kernel<T, LOG><<<dim3(D.n_pow2[LOG], P.batch), FftPlan<LOG>::NT, fft_smem_bytes<T, LOG>(false), st>>>(
+            P, D.pow2[LOG], map, w, use_w, D.tabs);
+    if (D.n_blue[LOG])
+        ring_blue_analysis_kernel<T, LOG><<<dim3(D.n_blue[LOG], P.batch), FftPlan<LOG>::NT, fft_smem_bytes<T, LOG>(true), st>>>(
+            P, D.blue[LOG], map, w, use_w, D.tabs);
+}
+
+template <typename T, int LOG>
+static void launch_class_synthesis(const DevPlan& P, const FftDev& D, T* map, const double* w, int use_w, cudaStream_t st) {
+    if (D.n_pow2[LOG])
+        ring_pow2_synthesis_kernel<T, LOG><<<dim3(D.n_pow2[LOG], P.batch), FftPlan<LOG>::NT, fft_smem_bytes<T, LOG>(false), st>>>(
+            P, D.pow2[LOG], map, w, use_w, D.tabs);
+    if (D.n_blue[LOG])
+        ring_blue_synthesis_kernel<T, LOG><<<dim3(D.n_blue[LOG], P.batch), FftPlan<LOG>::NT, fft_smem_bytes<T, LOG>(true), st>>>(
+            P, D.blue[LOG], map, w, use_w, D.tabs);
+}
+
+template <typename T>
+static cudaError_t run_fft_analysis(const HostPlan& hp, const void* d_map, const double* d_w, int use_w, cudaStream_t st) {
+    const DevPlan& P = hp.d;
+    if (!hp.fft) return cudaErrorInvalidValue;
+    const FftDev& D = *hp.fft;
+    const T* map = (const T*)d_map;
+    // largest rings first: they dominate the run time
+    launch_class_analysis<T, 13>(P, D, map, d_w, use_w, st);
+    launch_class_analysis<T, 12>(P, D, map, d_w, use_w, st);
+    launch_class_analysis<T, 11>(P, D, map, d_w, use_w, st);
+    launch_class_analysis<T, 10>(P, D, map, d_w, use_w, st);
+    launch_class_analysis<T, 9>(P, D, map, d_w, use_w, st);
+    launch_class_analysis<T, 8>(P, D, map, d_w, use_w, st);
+    if (D.n_direct)
+        ring_direct_analysis_kernel<T><<<dim3(D.n_direct, P.batch), FFT_THREADS, (size_t)DIRECT_MAX_N * 3 * sizeof(T), st>>>(
+            P, D.direct, map, d_w, use_w);
     return cudaGetLastError();
 }
 
 template <typename T>
 static cudaError_t run_fft_synthesis(const HostPlan& hp, void* d_map, const double* d_w, int use_w, cudaStream_t st) {
     const DevPlan& P = hp.d;
-    if (!hp.rings_direct.empty()) {
-        dim3 grid((unsigned)hp.rings_direct.size(), P.batch);
-        const size_t smem = ((size_t)DIRECT_MAX_N + P.mstride) * 2 * sizeof(T);
-        ring_direct_synthesis_kernel<T><<<grid, FFT_THREADS, smem, st>>>(P, hp.d_rings_direct, (T*)d_map, d_w, use_w);
-    }
+    if (!hp.fft) return cudaErrorInvalidValue;
+    const FftDev& D = *hp.fft;
+    T* map = (T*)d_map;
+    launch_class_synthesis<T, 13>(P, D, map, d_w, use_w, st);
+    launch_class_synthesis<T, 12>(P, D, map, d_w, use_w, st);
+    launch_class_synthesis<T, 11>(P, D, map, d_w, use_w, st);
+    launch_class_synthesis<T, 10>(P, D, map, d_w, use_w, st);
+    launch_class_synthesis<T, 9>(P, D, map, d_w, use_w, st);
+    launch_class_synthesis<T, 8>(P, D, map, d_w, use_w, st);
+    if (D.n_direct)
+        ring_direct_synthesis_kernel<T><<<dim3(D.n_direct, P.batch), FFT_THREADS,
+                                          ((size_t)DIRECT_MAX_N + D.max_mcut_direct + 1) * 2 * sizeof(T), st>>>(P, D.direct, map, d_w, use_w);
     return cudaGetLastError();
 }
 

@@ -222,3 +222,72 @@ def test_stream_ordering_and_error_codes():
     with pytest.raises(B.CuhpxError) as ei:
         B.cuhpx_map2alm(nside, lmax, lmax, 1, B.CUHPX_F32, fmap, alm, None, T.workspace)
     assert ei.value.status == B.CUHPX_EWORKSPACE
+
+
+# ----------------------------------------------------------------------------- FFT stage at full ring sizes
+
+def _spectra_view(B, T, batch, nside, mmax, dtype):
+    stride = B.cuhpx_spectra_stride(mmax)
+    nrings = 4 * nside - 1
+    esz = 16 if dtype == "f64" else 8
+    ptr = B.lib().cuhpx_workspace_spectra(T.workspace.data_ptr())
+    off = ptr - T.workspace.data_ptr()
+    raw = T.workspace.view(torch.uint8)[off: off + batch * nrings * stride * esz]
+    v = raw.view(torch.complex128 if dtype == "f64" else torch.complex64)
+    return v.view(batch, nrings, stride)
+
+
+def _class_rings(nside):
+    """Rings hitting every FFT kernel family and size class present at this nside, both hemispheres."""
+    picks = {1, 2, 3, 16, 63, 64, 65, 96, 127, 128, 129, 200, 255, 256, 257, 300, 511, 512, 513, 700, 1000, 1023, 1024,
+             1025, 1500, 2047, 2048, 2049, 3000, 4095, 4096, 4097, 5000}
+    rings = sorted(r for r in picks if r <= 2 * nside)
+    rings += [nside - 1, nside, nside + 1, 2 * nside, 3 * nside, 4 * nside - 1, 4 * nside - 70, 4 * nside - 1030]
+    return sorted(set(r for r in rings if 1 <= r <= 4 * nside - 1))
+
+
+@pytest.mark.parametrize("nside,lmax,dtype", [(512, 1200, "f64"), (1024, 2047, "f32"), (2048, 4095, "f64"),
+                                                (4096, 8191, "f64"), (4096, 8191, "f32")])
+def test_fft_stages_every_size_class(nside, lmax, dtype):
+    """a1 and s2 alone at full ring sizes against the oracle's direct ring sums, for rings from every
+    kernel family (direct / pow2 / chirp-z) and every block-FFT size (2^8 .. 2^13), incl. the m > N/2 fold."""
+    B = _binding()
+    T = make_transform(nside, lmax, lmax, 1, dtype)
+    mcut = B.cuhpx_workspace_mcut(T.workspace, nside)
+    rings = _class_rings(nside)
+    npix = 12 * nside * nside
+    fmap = np.zeros(npix)
+    for r in rings:
+        n, start = oracle.ring_geometry(nside, r)[:2]
+        fmap[start:start + n] = synth.normal(900 + nside, r, n)
+    fmap_r = rounded(fmap, dtype)
+    B.cuhpx_analysis_fft_stage(to_dev(fmap[None], dtype), None, 0, T.workspace)
+    torch.cuda.synchronize()
+    spec = _spectra_view(B, T, 1, nside, lmax, dtype)
+    tol = 1e-12 if dtype == "f64" else 3e-6
+    for r in rings:
+        n, start = oracle.ring_geometry(nside, r)[:2]
+        mc = int(mcut[r - 1])
+        ref = oracle.ring_dft(nside, r, fmap_r[start:start + n], mc)
+        got = spec[0, r - 1, : mc + 1].cpu().numpy().astype(np.complex128)
+        err = np.abs(got - ref).max() / np.abs(ref).max()
+        assert err < tol, f"analysis FFT stage ring {r} (N={n}, mcut={mc}): {err:.3e}"
+    # synthesis: fill the spectra rows of the picked rings, run s2 alone
+    spec.zero_()
+    Gs = {}
+    for r in rings:
+        mc = int(mcut[r - 1])
+        G = synth.white_alm(901 + nside, mc + 5, 0, 1, tag=r)[0][: mc + 1].copy()
+        G[0] = G[0].real
+        G = rounded(G, dtype, True)
+        Gs[r] = G
+        spec[0, r - 1, : mc + 1] = torch.from_numpy(G).to(spec.dtype).cuda()
+    out = torch.empty(1, npix, dtype=torch.float64 if dtype == "f64" else torch.float32, device="cuda")
+    B.cuhpx_synthesis_fft_stage(out, None, 0, T.workspace)
+    torch.cuda.synchronize()
+    out = out.cpu().numpy().astype(np.float64)[0]
+    for r in rings:
+        n, start = oracle.ring_geometry(nside, r)[:2]
+        ref = oracle.ring_synth(nside, r, Gs[r])
+        err = np.abs(out[start:start + n] - ref).max() / np.abs(ref).max()
+        assert err < tol, f"synthesis FFT stage ring {r} (N={n}): {err:.3e}"

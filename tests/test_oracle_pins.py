@@ -235,6 +235,17 @@ def test_ring_dft_vs_direct_sum(nside, ring):
     np.testing.assert_allclose(got, ref, atol=1e-13 * n)
 
 
+@pytest.mark.parametrize("nside,ring", [(4, 1), (4, 2), (4, 6), (8, 13), (16, 40)])
+def test_ring_synth_vs_direct_sum(nside, ring):
+    """The ring synthesis sum of Eq. 24 against numpy, with m far beyond N/2."""
+    n, start, c, s, phi0 = oracle.ring_geometry(nside, ring)
+    mmax = 3 * nside + 3
+    G = synth.white_alm(5, mmax, 0)[0][: mmax + 1].copy()
+    x = np.arange(n)
+    ref = G[0].real + 2 * sum((G[m] * np.exp(1j * m * (phi0 + 2 * np.pi * x / n))).real for m in range(1, mmax + 1))
+    np.testing.assert_allclose(oracle.ring_synth(nside, ring, G), ref, atol=1e-13 * mmax)
+
+
 def test_bluestein_identity():
     """Eq. 17-23 (P:212-251): X(k) = h[k] sum_n (x[n] h[n]) h^-1[k-n], h[m] = W_N^(m^2/2), reproduces
     the ring DFT for a non-power-of-two ring (the identity the CUDA chirp-z kernels rely on)."""
