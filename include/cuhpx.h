@@ -110,6 +110,13 @@ int cuhpx_synthesis_legendre_stage(const void* d_alm, int adjoint, void* d_works
 int cuhpx_synthesis_fft_stage(void* d_map, const double* d_ring_weights, int use_weights, void* d_workspace,
                               cuhpx_stream_t stream);
 
+/* Host-side statistics of an initialised workspace, for measurement (doubles, `count` of them are written, at most 8):
+ *  [0] kernel launches of one FFT-stage call   [1] of one Legendre analysis call   [2] of one Legendre synthesis call
+ *  [3] Legendre terms executed per channel = sum_m (lmax - m + 1) * (ring pairs processed at order m)
+ *  [4] Legendre terms of the full triangle = nalm * 2 nside          [5] spectra entries per channel = sum_rings (m_cut + 1)
+ *  [6] bytes of constant tables read by one FFT-stage call (chirp filters + twiddles)   [7] workspace bytes */
+int cuhpx_workspace_stats(void* d_workspace, double* h_stats, int count);
+
 /* Register-only FMA loop used by bench.py to measure the FP64 / FP32 FMA peak in the same run.
  * Writes the elapsed milliseconds of `iters` dependent-chain FMAs per thread over the whole GPU to *ms and the
  * number of FMA instructions executed to *fma_count.  Synchronises the stream. */

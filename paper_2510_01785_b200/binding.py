@@ -23,7 +23,7 @@ EXPORTS = [
     "cuhpx_workspace_bytes", "cuhpx_workspace_init", "cuhpx_workspace_release", "cuhpx_map2alm", "cuhpx_alm2map",
     "cuhpx_alm2map_adjoint", "cuhpx_map2alm_adjoint", "cuhpx_spectra_stride", "cuhpx_workspace_spectra",
     "cuhpx_workspace_mcut", "cuhpx_analysis_fft_stage", "cuhpx_analysis_legendre_stage",
-    "cuhpx_synthesis_legendre_stage", "cuhpx_synthesis_fft_stage", "cuhpx_fma_peak_probe",
+    "cuhpx_synthesis_legendre_stage", "cuhpx_synthesis_fft_stage", "cuhpx_fma_peak_probe", "cuhpx_workspace_stats",
 ]
 
 
@@ -69,6 +69,7 @@ def _load() -> ctypes.CDLL:
     lib.cuhpx_synthesis_legendre_stage.argtypes = [vp, i, vp, vp]
     lib.cuhpx_synthesis_fft_stage.argtypes = [vp, vp, i, vp, vp]
     lib.cuhpx_fma_peak_probe.argtypes = [i, i, vp, vp, vp]
+    lib.cuhpx_workspace_stats.argtypes = [vp, vp, i]
     return lib
 
 
@@ -208,6 +209,15 @@ def cuhpx_workspace_mcut(workspace: torch.Tensor, nside: int):
     _check(_lib.cuhpx_workspace_mcut(_dev_ptr(workspace), out.ctypes.data_as(ctypes.c_void_p)),
            "cuhpx_workspace_mcut")
     return out
+
+
+def cuhpx_workspace_stats(workspace: torch.Tensor) -> dict:
+    """Host-side statistics of an initialised workspace (see cuhpx.h)."""
+    arr = (ctypes.c_double * 8)()
+    _check(_lib.cuhpx_workspace_stats(_dev_ptr(workspace), arr, 8), "cuhpx_workspace_stats")
+    keys = ["fft_stage_launches", "legendre_analysis_launches", "legendre_synthesis_launches", "legendre_terms_executed",
+            "legendre_terms_full", "spectra_entries", "fft_table_bytes", "workspace_bytes"]
+    return dict(zip(keys, [float(v) for v in arr]))
 
 
 def cuhpx_fma_peak_probe(dtype: int, iters: int, stream=None):

@@ -80,6 +80,9 @@ size_t plan_fft_tables(HostPlan& hp, char* base, bool build, cudaStream_t st, cu
 // largest supported ring for this dtype (shared-memory bound); used by argument validation
 bool fft_supported(int nside, cuhpx_dtype_t dt);
 
+// launches per FFT-stage call and bytes of constant tables it reads
+void fft_stage_stats(const HostPlan& hp, int* launches, double* table_bytes);
+
 cudaError_t fma_peak_probe(cuhpx_dtype_t dt, int iters, float* ms, double* count, cudaStream_t st);
 
 }  // namespace cuhpx

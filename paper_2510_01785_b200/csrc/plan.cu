@@ -364,6 +364,26 @@ int cuhpx_workspace_mcut(void* ws, int* h_mcut) {
     return CUHPX_OK;
 }
 
+int cuhpx_workspace_stats(void* ws, double* out, int count) {
+    HostPlan* hp = find_plan(ws);
+    if (!hp || !out || count < 1) return CUHPX_EWORKSPACE;
+    const DevPlan& d = hp->d;
+    double st[8] = {0};
+    int fl = 0;
+    double tb = 0;
+    fft_stage_stats(*hp, &fl, &tb);
+    st[0] = fl;
+    st[1] = d.nchunk_max > 1 ? 2 : 1;
+    st[2] = 1;
+    for (int m = 0; m <= d.mmax; ++m) st[3] += (double)(d.lmax - m + 1) * (double)(d.npairs - hp->h_jmin[m]);
+    st[4] = (double)d.nalm * (double)d.npairs;
+    for (int r = 0; r < d.nrings; ++r) st[5] += hp->h_mcut[r < d.nrings - 1 - r ? r : d.nrings - 1 - r] + 1;
+    st[6] = tb;
+    st[7] = (double)hp->workspace_bytes;
+    for (int i = 0; i < count && i < 8; ++i) out[i] = st[i];
+    return CUHPX_OK;
+}
+
 #define CUDA_OR_FAIL(expr)                         \
     do {                                           \
         if ((expr) != cudaSuccess) return CUHPX_ECUDA; \

@@ -744,6 +744,23 @@ size_t plan_fft_tables(HostPlan& hp, char* base, bool build, cudaStream_t st, cu
 
 void free_fft_dev(FftDev* f) { delete f; }
 
+void fft_stage_stats(const HostPlan& hp, int* launches, double* table_bytes) {
+    *launches = 0;
+    *table_bytes = 0;
+    if (!hp.fft) return;
+    const FftDev& D = *hp.fft;
+    const double csz = hp.dtype == CUHPX_F64 ? 16 : 8;
+    if (D.n_direct) ++*launches;
+    for (int l = MIN_LOG; l <= MAX_LOG; ++l) {
+        if (D.n_pow2[l]) ++*launches;
+        if (D.n_blue[l]) {
+            ++*launches;
+            *table_bytes += 0.5 * D.n_blue[l] * (double)(1 << l) * csz;  // one filter per ring size i, shared N/S
+        }
+    }
+    *table_bytes += D.tabs.twlen * csz;
+}
+
 // ------------------------------------------------------------------ launchers
 template <typename T, int LOG>
 static void launch_class_analysis(const DevPlan& P, const FftDev& D, const T* map, const double* w, int use_w, cudaStream_t st) {

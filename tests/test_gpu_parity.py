@@ -291,3 +291,104 @@ def test_fft_stages_every_size_class(nside, lmax, dtype):
         ref = oracle.ring_synth(nside, r, Gs[r])
         err = np.abs(out[start:start + n] - ref).max() / np.abs(ref).max()
         assert err < tol, f"synthesis FFT stage ring {r} (N={n}): {err:.3e}"
+
+
+# ----------------------------------------------------------------------------- BASELINE configs 4 and 5 (subset oracle)
+
+def _subset_lm(seed, lmax, mmax, n_m, per_m):
+    """Seeded (l, m) sample: mandated corner cases plus n_m random orders with per_m degrees each."""
+    u = synth.uniform(seed, 77, n_m * (per_m + 1))
+    sel = {(0, 0), (lmax, 0), (lmax, mmax), (lmax, mmax - 1), (mmax, mmax), (lmax - 1, 5), (lmax, 7), (17, 6)}
+    ms = sorted(set(int(x * (mmax + 1)) for x in u[:n_m]))
+    k = n_m
+    for m in ms:
+        for _ in range(per_m):
+            sel.add((m + int(u[k] * (lmax - m + 1)), m))
+            k += 1
+    sel = sorted(sel, key=lambda t: (t[1], t[0]))
+    return [s[0] for s in sel], [s[1] for s in sel]
+
+
+def _subset_rings(seed, nside, count):
+    u = synth.uniform(seed, 78, count)
+    rings = {1, 2, 3, nside - 1, nside, nside + 1, 2 * nside, 2 * nside + 1, 4 * nside - 1, 4 * nside - 5, 3 * nside + 7,
+             nside // 2 + 1, 3 * nside // 4 + 3, 97}
+    rings |= set(1 + int(x * (4 * nside - 1)) for x in u)
+    return sorted(r for r in rings if 1 <= r <= 4 * nside - 1)
+
+
+def _ring_slices(nside, rings):
+    return [slice(s, s + n) for n, s in (oracle.ring_geometry(nside, r)[:2] for r in rings)]
+
+
+@pytest.mark.slow
+def test_cfg4_nside1024_fp32_batch8():
+    """configs[3]: nside 1024, lmax = mmax = 2047, 8 channels fp32; alm -> alm2map + 0.01 noise -> map2alm; adjoints.
+    Oracle: seeded subset (256+ coefficients, 40+ rings) on channels 0 and 7 (full oracle = hours of x87 work)."""
+    nside, lmax, batch = 1024, 2047, 8
+    T = make_transform(nside, lmax, lmax, batch, "f32")
+    alm = synth.powerlaw_alm(404, lmax, lmax, batch)
+    rings = _subset_rings(404, nside, 32)
+    sl, sm = _subset_lm(404, lmax, lmax, 32, 8)
+    sl_idx = [oracle.alm_index(lmax, l, m) for l, m in zip(sl, sm)]
+    slices = _ring_slices(nside, rings)
+    gmap = T.alm2map(to_dev(alm, "f32", True))
+    got_map = gmap.cpu().numpy().astype(np.float64)
+    noisy = got_map + 0.01 * synth.gaussian_map(405, nside, batch)
+    noisy32 = noisy.astype(np.float32)
+    galm = T.map2alm(torch.from_numpy(noisy32).cuda()).cpu().numpy().astype(np.complex128)
+    gst = T.alm2map_adjoint(torch.from_numpy(noisy32).cuda()).cpu().numpy().astype(np.complex128)
+    cot = synth.white_alm(406, lmax, lmax, batch)
+    gat = T.map2alm_adjoint(to_dev(cot, "f32", True)).cpu().numpy().astype(np.float64)
+    for c in (0, 7):
+        a_in = rounded(alm[c], "f32", True)
+        ref = oracle.alm2map_rings(nside, lmax, lmax, a_in, rings)
+        got = np.concatenate([got_map[c][s] for s in slices])
+        assert err32(got, ref) <= TOL32
+        f_in = noisy32[c].astype(np.float64)
+        ref = oracle.map2alm_subset(nside, lmax, lmax, f_in, sl, sm)
+        assert err32(galm[c][sl_idx], ref) <= TOL32
+        # per coefficient: nothing hides in the norm (the largest coefficients dominate it)
+        assert np.abs(galm[c][sl_idx] - ref).max() <= 2e-5 * np.abs(galm[c]).max()
+        ref = oracle.alm2map_adjoint_subset(nside, lmax, lmax, f_in, sl, sm)
+        assert err32(gst[c][sl_idx], ref) <= TOL32
+        ref = oracle.map2alm_adjoint_rings(nside, lmax, lmax, rounded(cot[c], "f32", True), rings)
+        got = np.concatenate([gat[c][s] for s in slices])
+        assert err32(got, ref) <= TOL32
+
+
+@pytest.mark.slow
+def test_cfg5_nside4096_fp64():
+    """configs[4]: nside 4096, lmax = mmax = 8191, fp64: alm -> alm2map -> map2alm.  Oracle checked on a seeded
+    subset of 512+ (l, m) and 64+ rings; the analysis is checked on the GPU's own map so both
+    sides see identical input."""
+    nside, lmax = 4096, 8191
+    T = make_transform(nside, lmax, lmax, 1, "f64")
+    alm = synth.powerlaw_alm(505, lmax, lmax, 1)
+    rings = _subset_rings(505, nside, 50)
+    sl, sm = _subset_lm(505, lmax, lmax, 56, 9)
+    assert len(sl) >= 512 and len(rings) >= 64
+    sl_idx = [oracle.alm_index(lmax, l, m) for l, m in zip(sl, sm)]
+    slices = _ring_slices(nside, rings)
+    dmap = T.alm2map(to_dev(alm, "f64", True))
+    got_map = dmap.cpu().numpy()[0]
+    ref = oracle.alm2map_rings(nside, lmax, lmax, alm[0], rings)
+    got = np.concatenate([got_map[s] for s in slices])
+    e_syn = np.abs(got - ref).max() / np.abs(got_map).max()
+    assert e_syn <= TOL64, f"alm2map {e_syn:.3e}"
+    galm = T.map2alm(dmap).cpu().numpy()[0]
+    ref = oracle.map2alm_subset(nside, lmax, lmax, got_map, sl, sm)
+    e_ana = np.abs(galm[sl_idx] - ref).max() / np.abs(galm).max()
+    assert e_ana <= TOL64, f"map2alm {e_ana:.3e}"
+    assert np.all(galm[: lmax + 1].imag == 0.0)
+    # adjoints on the same subset
+    gst = T.alm2map_adjoint(dmap).cpu().numpy()[0]
+    ref = oracle.alm2map_adjoint_subset(nside, lmax, lmax, got_map, sl, sm)
+    e_st = np.abs(gst[sl_idx] - ref).max() / np.abs(gst).max()
+    assert e_st <= TOL64, f"alm2map_adjoint {e_st:.3e}"
+    gat = T.map2alm_adjoint(to_dev(alm, "f64", True)).cpu().numpy()[0]
+    ref = oracle.map2alm_adjoint_rings(nside, lmax, lmax, alm[0], rings)
+    got = np.concatenate([gat[s] for s in slices])
+    e_at = np.abs(got - ref).max() / np.abs(gat).max()
+    assert e_at <= TOL64, f"map2alm_adjoint {e_at:.3e}"
+    print("cfg5", e_syn, e_ana, e_st, e_at)
