@@ -348,7 +348,7 @@ def main():
         import oracle
 
         cores = oracle.num_threads()
-        nr = max(2, cores // 2) if nside >= 1024 else 4 * nside - 1
+        nr = max(8, (4 if nside >= 4096 else 16) * cores) if nside >= 1024 else 4 * nside - 1
         rings = oracle_sample_rings(nside, nr)
         frac = oracle_cost_fraction(nside, lmax, mmax, rings)
         a_in = alm_np[0] if dt == "f64" else alm_np[0].astype(np.complex64).astype(np.complex128)

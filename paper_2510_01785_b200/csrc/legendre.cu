@@ -109,14 +109,21 @@ __device__ __forceinline__ void warp_transpose_reduce(T (&v)[NV], int lane) {
 }
 
 // ------------------------------------------------------------------ analysis (row a3)
+// Per warp: every LT degrees the NV = LT*BT*2 per-thread partial sums are reduced over the 32 lanes by a
+// transposing butterfly (NV-1 adds per thread) and parked in shared memory; every GROUP_L degrees one
+// __syncthreads lets the first threads add the 8 warps' values and write a_lm.  Warps whose rings are all still
+// below the significance threshold skip the accumulation (recurrence only).
+constexpr int GROUP_L = 32;  // degrees per cross-warp reduction
+
 template <typename T, int BT, int R, int LT>
-__global__ void __launch_bounds__(LEG_THREADS) legendre_analysis_kernel(LegArgs a) {
+__global__ void __launch_bounds__(LEG_THREADS, 2) legendre_analysis_kernel(LegArgs a) {
     using T2 = typename Vec2<T>::type;
     constexpr int NV = LT * BT * 2;
     constexpr int Q = NV >= 32 ? NV / 32 : 1;
     constexpr int SH = NV >= 32 ? 0 : (NV == 16 ? 1 : NV == 8 ? 2 : NV == 4 ? 3 : 4);
-    static_assert(CHECK_EVERY % LT == 0 && CT % CHECK_EVERY == 0, "tile sizes");
-    static_assert(NV <= LEG_THREADS && NV >= 2, "reduction tile");
+    constexpr int TPG = GROUP_L / LT;  // tiles per group
+    static_assert(CHECK_EVERY % LT == 0 && CT % GROUP_L == 0 && GROUP_L % CHECK_EVERY == 0, "tile sizes");
+    static_assert(TPG * NV <= LEG_THREADS && NV >= 2, "reduction tile");
     const DevPlan& P = a.p;
     const int m = blockIdx.x;
     const int chunk = blockIdx.y;
@@ -126,7 +133,7 @@ __global__ void __launch_bounds__(LEG_THREADS) legendre_analysis_kernel(LegArgs 
     if (jbase >= P.npairs) return;
 
     __shared__ double sA[2][CT], sB[2][CT];
-    __shared__ T red[2][LEG_WARPS][NV];
+    __shared__ T red[2][TPG][LEG_WARPS][NV];
 
     const T2* spectra = reinterpret_cast<const T2*>(P.spectra);
     double cur[R], prev[R], y[R];
@@ -180,7 +187,7 @@ __global__ void __launch_bounds__(LEG_THREADS) legendre_analysis_kernel(LegArgs 
     if (a.to_partial) out += (size_t)chunk * P.batch * P.nalm * 2;
 
     const int nl = P.lmax - m + 1;  // l values of this m
-    bool block_active = false;
+    bool warp_active = __any_sync(0xffffffffu, nact > 0);
     int buf = 0;
     for (int t0 = 0; t0 < nl; t0 += CT) {
         // coefficients of degrees l = m + t0 + 1 + i (the step that produces lambda_{l}) for this tile
@@ -188,80 +195,84 @@ __global__ void __launch_bounds__(LEG_THREADS) legendre_analysis_kernel(LegArgs 
         if (tid < CT) recurrence_coeff(m + t0 + 1 + tid, m, sA[cb][tid], sB[cb][tid]);
         __syncthreads();
         const int tend = min(CT, nl - t0);
-        for (int s0 = 0; s0 < tend; s0 += LT) {
-            if ((s0 % CHECK_EVERY) == 0) {
-#pragma unroll
-                for (int r = 0; r < R; ++r) {
-                    if (sc[r] < 0 && fabs(cur[r]) > pow2c(ScaleCfg<T>::THR)) {
-                        cur[r] *= pow2c(-ScaleCfg<T>::K);
-                        prev[r] *= pow2c(-ScaleCfg<T>::K);
-                        if (++sc[r] == 0) {
-                            load_F(r);
-                            ++nact;
-                        }
-                    }
-                }
-                if (!block_active) block_active = __syncthreads_or(nact > 0);
-            }
-            T acc[NV];
-#pragma unroll
-            for (int i = 0; i < NV; ++i) acc[i] = 0;
-            if (block_active) {
-#pragma unroll
-                for (int i = 0; i < LT; ++i) {
-                    const double A = sA[cb][s0 + i], B = sB[cb][s0 + i];
+        for (int g0 = 0; g0 < tend; g0 += GROUP_L) {
+#pragma unroll 1
+            for (int ti = 0; ti < TPG; ++ti) {
+                const int s0 = g0 + ti * LT;
+                if ((s0 % CHECK_EVERY) == 0 && !__all_sync(0xffffffffu, nact == R)) {
 #pragma unroll
                     for (int r = 0; r < R; ++r) {
-                        const T lam = (T)cur[r];
-#pragma unroll
-                        for (int c = 0; c < BT; ++c) {
-                            // (t0 + s0 + i) = l - m; even -> symmetric combination
-                            if (((s0 + i) & 1) == 0) {
-                                acc[(i * BT + c) * 2 + 0] = fma(lam, fs[r][c][0], acc[(i * BT + c) * 2 + 0]);
-                                acc[(i * BT + c) * 2 + 1] = fma(lam, fs[r][c][1], acc[(i * BT + c) * 2 + 1]);
-                            } else {
-                                acc[(i * BT + c) * 2 + 0] = fma(lam, fa[r][c][0], acc[(i * BT + c) * 2 + 0]);
-                                acc[(i * BT + c) * 2 + 1] = fma(lam, fa[r][c][1], acc[(i * BT + c) * 2 + 1]);
+                        if (sc[r] < 0 && fabs(cur[r]) > pow2c(ScaleCfg<T>::THR)) {
+                            cur[r] *= pow2c(-ScaleCfg<T>::K);
+                            prev[r] *= pow2c(-ScaleCfg<T>::K);
+                            if (++sc[r] == 0) {
+                                load_F(r);
+                                ++nact;
                             }
                         }
-                        const double xl = fma(-y[r], cur[r], cur[r]);
-                        const double nx = fma(A, xl, B * prev[r]);
-                        prev[r] = cur[r];
-                        cur[r] = nx;
                     }
+                    warp_active = __any_sync(0xffffffffu, nact > 0);
                 }
-                warp_transpose_reduce<T, NV>(acc, lane);
-                if ((lane & ((1 << SH) - 1)) == 0) {
+                if (warp_active) {
+                    T acc[NV];
 #pragma unroll
-                    for (int q = 0; q < Q; ++q) red[buf][warp][Q * (lane >> SH) + q] = acc[q];
-                }
-            } else {
+                    for (int i = 0; i < NV; ++i) acc[i] = 0;
 #pragma unroll
-                for (int i = 0; i < LT; ++i) {
-                    const double A = sA[cb][s0 + i], B = sB[cb][s0 + i];
+                    for (int i = 0; i < LT; ++i) {
+                        const double A = sA[cb][s0 + i], B = sB[cb][s0 + i];
 #pragma unroll
-                    for (int r = 0; r < R; ++r) {
-                        const double xl = fma(-y[r], cur[r], cur[r]);
-                        const double nx = fma(A, xl, B * prev[r]);
-                        prev[r] = cur[r];
-                        cur[r] = nx;
+                        for (int r = 0; r < R; ++r) {
+                            const T lam = (T)cur[r];
+#pragma unroll
+                            for (int c = 0; c < BT; ++c) {
+                                // (t0 + s0 + i) = l - m; even -> symmetric combination
+                                if (((s0 + i) & 1) == 0) {
+                                    acc[(i * BT + c) * 2 + 0] = fma(lam, fs[r][c][0], acc[(i * BT + c) * 2 + 0]);
+                                    acc[(i * BT + c) * 2 + 1] = fma(lam, fs[r][c][1], acc[(i * BT + c) * 2 + 1]);
+                                } else {
+                                    acc[(i * BT + c) * 2 + 0] = fma(lam, fa[r][c][0], acc[(i * BT + c) * 2 + 0]);
+                                    acc[(i * BT + c) * 2 + 1] = fma(lam, fa[r][c][1], acc[(i * BT + c) * 2 + 1]);
+                                }
+                            }
+                            const double xl = fma(-y[r], cur[r], cur[r]);
+                            const double nx = fma(A, xl, B * prev[r]);
+                            prev[r] = cur[r];
+                            cur[r] = nx;
+                        }
                     }
+                    warp_transpose_reduce<T, NV>(acc, lane);
+                    if ((lane & ((1 << SH) - 1)) == 0) {
+#pragma unroll
+                        for (int q = 0; q < Q; ++q) red[buf][ti][warp][Q * (lane >> SH) + q] = acc[q];
+                    }
+                } else {
+#pragma unroll
+                    for (int i = 0; i < LT; ++i) {
+                        const double A = sA[cb][s0 + i], B = sB[cb][s0 + i];
+#pragma unroll
+                        for (int r = 0; r < R; ++r) {
+                            const double xl = fma(-y[r], cur[r], cur[r]);
+                            const double nx = fma(A, xl, B * prev[r]);
+                            prev[r] = cur[r];
+                            cur[r] = nx;
+                        }
+                    }
+                    for (int v = lane; v < NV; v += 32) red[buf][ti][warp][v] = 0;
                 }
             }
-            if (block_active) __syncthreads();
-            if (tid < NV) {
+            __syncthreads();
+            if (tid < TPG * NV) {
+                const int ti = tid / NV, v = tid % NV;
                 T sum = 0;
-                if (block_active) {
 #pragma unroll
-                    for (int w = 0; w < LEG_WARPS; ++w) sum += red[buf][w][tid];
-                }
-                const int i = tid / (BT * 2), c = (tid / 2) % BT, ri = tid & 1;
-                const int k = t0 + s0 + i;  // l - m
+                for (int w = 0; w < LEG_WARPS; ++w) sum += red[buf][ti][w][v];
+                const int i = v / (BT * 2), c = (v / 2) % BT, ri = v & 1;
+                const int k = t0 + g0 + ti * LT + i;  // l - m
                 const int ch = ch0 + c;
                 if (k < nl && ch < P.batch) {
-                    T v = (T)(outscale * (double)sum);
-                    if (m == 0 && ri == 1) v = 0;  // Im a_l0 is exactly zero
-                    out[((size_t)ch * P.nalm + abase + m + k) * 2 + ri] = v;
+                    T o = (T)(outscale * (double)sum);
+                    if (m == 0 && ri == 1) o = 0;  // Im a_l0 is exactly zero
+                    out[((size_t)ch * P.nalm + abase + m + k) * 2 + ri] = o;
                 }
             }
             buf ^= 1;

@@ -365,8 +365,8 @@ def test_cfg5_nside4096_fp64():
     nside, lmax = 4096, 8191
     T = make_transform(nside, lmax, lmax, 1, "f64")
     alm = synth.powerlaw_alm(505, lmax, lmax, 1)
-    rings = _subset_rings(505, nside, 50)
-    sl, sm = _subset_lm(505, lmax, lmax, 56, 9)
+    rings = _subset_rings(505, nside, 60)
+    sl, sm = _subset_lm(505, lmax, lmax, 60, 9)
     assert len(sl) >= 512 and len(rings) >= 64
     sl_idx = [oracle.alm_index(lmax, l, m) for l, m in zip(sl, sm)]
     slices = _ring_slices(nside, rings)
