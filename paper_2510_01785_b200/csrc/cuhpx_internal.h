@@ -32,6 +32,9 @@ struct DevPlan {
     const double* pref_hi;   // log2 |lambda_mm| prefactor, split hi + lo
     const double* pref_lo;
     const int* jmin;         // first ring pair processed for this m
+    // per (l, m) [nalm], packed like alm: rescaled recurrence coefficients (legendre.cu)
+    const double* coef_alpha;
+    const double* coef_scale;
     // scratch
     void* spectra;           // [batch][nrings][mstride] complex<T>
     void* partial;           // [nchunk_max][batch][nalm] complex<T> (analysis partial sums), or null
@@ -69,6 +72,7 @@ inline int ilog2_ceil(long long v) {
 inline bool is_pow2(long long v) { return v > 0 && (v & (v - 1)) == 0; }
 
 // ------------------------------------------------------------------ launchers (each returns a cudaError_t)
+cudaError_t launch_legendre_coeff(int lmax, int mmax, double* alpha, double* scale, cudaStream_t st);
 cudaError_t launch_legendre_analysis(const HostPlan& hp, void* d_alm, int adjoint, cudaStream_t st);
 cudaError_t launch_legendre_synthesis(const HostPlan& hp, const void* d_alm, int adjoint, cudaStream_t st);
 cudaError_t launch_fft_analysis(const HostPlan& hp, const void* d_map, const double* d_w, int use_w, cudaStream_t st);

@@ -65,14 +65,78 @@ __device__ __forceinline__ void lambda_seed(int m, double pref_hi, double pref_l
     if (m & 1) val = -val;
 }
 
-// recurrence coefficients for degree l (>= m + 1):  lambda_l = A x lambda_{l-1} + B lambda_{l-2}
-__device__ __forceinline__ void recurrence_coeff(int l, int m, double& A, double& B) {
-    const double dl = (double)l, dm = (double)m;
-    const double l2m2 = (dl - dm) * (dl + dm);  // exact: < 2^53
-    A = sqrt((4.0 * dl * dl - 1.0) / l2m2);
-    const double num = (2.0 * dl + 1.0) * ((dl - 1.0 - dm) * (dl - 1.0 + dm));
-    const double den = (2.0 * dl - 3.0) * l2m2;
-    B = (num == 0.0) ? 0.0 : -sqrt(num / den);
+// ------------------------------------------------------------------ recurrence coefficients (built once per plan)
+// Eq. 16 reads lambda_l = A_l x lambda_{l-1} + B_l lambda_{l-2}, A_l = sqrt((4l^2-1)/(l^2-m^2)),
+// B_l = -sqrt((2l+1)/(2l-3) ((l-1)^2-m^2)/(l^2-m^2)).  The kernels iterate the diagonally rescaled sequence
+// mu_l = lambda_l / s_l with s_m = s_{m+1} = 1, s_l = |B_l| s_{l-2}, for which
+//        mu_l = alpha_l x mu_{l-1} - mu_{l-2},   alpha_l = A_l s_{l-1} / s_l,
+// i.e. two FMAs per degree instead of mul + mul + FMA; s_l is applied once per coefficient (to a_lm before the
+// synthesis sum, to the reduced sum after the analysis).  alpha must be good to an ulp (near the poles the
+// recurrence amplifies coefficient errors by ~1/theta^2, R3), so the table is built in double-double.
+struct dd {
+    double hi, lo;
+};
+__device__ __forceinline__ dd dd_from(double a) { return dd{a, 0.0}; }
+__device__ __forceinline__ dd dd_two_prod(double a, double b) {
+    const double p = a * b;
+    return dd{p, fma(a, b, -p)};
+}
+__device__ __forceinline__ dd dd_norm(double hi, double lo) {
+    const double s = hi + lo;
+    return dd{s, lo - (s - hi)};
+}
+__device__ __forceinline__ dd dd_mul(dd a, dd b) {
+    dd p = dd_two_prod(a.hi, b.hi);
+    p.lo += a.hi * b.lo + a.lo * b.hi;
+    return dd_norm(p.hi, p.lo);
+}
+__device__ __forceinline__ dd dd_div(dd a, dd b) {
+    const double q1 = a.hi / b.hi;
+    // r = a - q1 * b
+    dd p = dd_mul(dd_from(q1), b);
+    const double r = (a.hi - p.hi) + (a.lo - p.lo);
+    const double q2 = r / b.hi;
+    return dd_norm(q1, q2);
+}
+__device__ __forceinline__ dd dd_sqrt(dd a) {
+    if (a.hi <= 0.0) return dd{0.0, 0.0};
+    const double x = sqrt(a.hi);
+    // one Newton step: x + (a - x^2) / (2x)
+    const dd x2 = dd_two_prod(x, x);
+    const double r = (a.hi - x2.hi) + (a.lo - x2.lo);
+    return dd_norm(x, r / (2.0 * x));
+}
+
+// one thread per m; alpha[idx(l,m)], scale[idx(l,m)] for l = m..lmax (alpha[idx(m,m)] = 0: no step produces lambda_mm)
+__global__ void legendre_coeff_kernel(int lmax, int mmax, double* __restrict__ alpha, double* __restrict__ scale) {
+    const int m = blockIdx.x * blockDim.x + threadIdx.x;
+    if (m > mmax) return;
+    const long long base = (long long)m * (2LL * lmax + 1 - m) / 2;
+    alpha[base + m] = 0.0;
+    scale[base + m] = 1.0;
+    dd s1 = dd_from(1.0), s2 = dd_from(1.0);  // s_{l-1}, s_{l-2}
+    const double dm = (double)m;
+    for (int l = m + 1; l <= lmax; ++l) {
+        const double dl = (double)l;
+        const double l2m2 = (dl - dm) * (dl + dm);  // exact integers below 2^53
+        const dd A = dd_sqrt(dd_div(dd_from(4.0 * dl * dl - 1.0), dd_from(l2m2)));
+        dd sl = dd_from(1.0);
+        if (l >= m + 2) {
+            const dd num = dd_two_prod(2.0 * dl + 1.0, (dl - 1.0 - dm) * (dl - 1.0 + dm));
+            const dd den = dd_two_prod(2.0 * dl - 3.0, l2m2);
+            sl = dd_mul(dd_sqrt(dd_div(num, den)), s2);  // |B_l| s_{l-2}
+        }
+        const dd al = dd_div(dd_mul(A, s1), sl);
+        alpha[base + l] = al.hi + al.lo;
+        scale[base + l] = sl.hi + sl.lo;
+        s2 = s1;
+        s1 = sl;
+    }
+}
+
+cudaError_t launch_legendre_coeff(int lmax, int mmax, double* alpha, double* scale, cudaStream_t st) {
+    legendre_coeff_kernel<<<(mmax + 1 + 63) / 64, 64, 0, st>>>(lmax, mmax, alpha, scale);
+    return cudaGetLastError();
 }
 
 struct LegArgs {
@@ -132,7 +196,7 @@ __global__ void __launch_bounds__(LEG_THREADS, 2) legendre_analysis_kernel(LegAr
     const int jbase = P.jmin[m] + chunk * (LEG_THREADS * R);
     if (jbase >= P.npairs) return;
 
-    __shared__ double sA[2][CT], sB[2][CT];
+    __shared__ double sA[2][CT];
     __shared__ T red[2][TPG][LEG_WARPS][NV];
 
     const T2* spectra = reinterpret_cast<const T2*>(P.spectra);
@@ -192,7 +256,7 @@ __global__ void __launch_bounds__(LEG_THREADS, 2) legendre_analysis_kernel(LegAr
     for (int t0 = 0; t0 < nl; t0 += CT) {
         // coefficients of degrees l = m + t0 + 1 + i (the step that produces lambda_{l}) for this tile
         const int cb = (t0 / CT) & 1;
-        if (tid < CT) recurrence_coeff(m + t0 + 1 + tid, m, sA[cb][tid], sB[cb][tid]);
+        if (tid < CT) sA[cb][tid] = (t0 + 1 + tid < nl) ? P.coef_alpha[abase + m + t0 + 1 + tid] : 0.0;
         __syncthreads();
         const int tend = min(CT, nl - t0);
         for (int g0 = 0; g0 < tend; g0 += GROUP_L) {
@@ -219,7 +283,7 @@ __global__ void __launch_bounds__(LEG_THREADS, 2) legendre_analysis_kernel(LegAr
                     for (int i = 0; i < NV; ++i) acc[i] = 0;
 #pragma unroll
                     for (int i = 0; i < LT; ++i) {
-                        const double A = sA[cb][s0 + i], B = sB[cb][s0 + i];
+                        const double A = sA[cb][s0 + i];
 #pragma unroll
                         for (int r = 0; r < R; ++r) {
                             const T lam = (T)cur[r];
@@ -235,7 +299,7 @@ __global__ void __launch_bounds__(LEG_THREADS, 2) legendre_analysis_kernel(LegAr
                                 }
                             }
                             const double xl = fma(-y[r], cur[r], cur[r]);
-                            const double nx = fma(A, xl, B * prev[r]);
+                            const double nx = fma(A, xl, -prev[r]);
                             prev[r] = cur[r];
                             cur[r] = nx;
                         }
@@ -248,11 +312,11 @@ __global__ void __launch_bounds__(LEG_THREADS, 2) legendre_analysis_kernel(LegAr
                 } else {
 #pragma unroll
                     for (int i = 0; i < LT; ++i) {
-                        const double A = sA[cb][s0 + i], B = sB[cb][s0 + i];
+                        const double A = sA[cb][s0 + i];
 #pragma unroll
                         for (int r = 0; r < R; ++r) {
                             const double xl = fma(-y[r], cur[r], cur[r]);
-                            const double nx = fma(A, xl, B * prev[r]);
+                            const double nx = fma(A, xl, -prev[r]);
                             prev[r] = cur[r];
                             cur[r] = nx;
                         }
@@ -270,7 +334,7 @@ __global__ void __launch_bounds__(LEG_THREADS, 2) legendre_analysis_kernel(LegAr
                 const int k = t0 + g0 + ti * LT + i;  // l - m
                 const int ch = ch0 + c;
                 if (k < nl && ch < P.batch) {
-                    T o = (T)(outscale * (double)sum);
+                    T o = (T)(outscale * P.coef_scale[abase + m + k] * (double)sum);  // lambda = s_l mu
                     if (m == 0 && ri == 1) o = 0;  // Im a_l0 is exactly zero
                     out[((size_t)ch * P.nalm + abase + m + k) * 2 + ri] = o;
                 }
@@ -308,7 +372,7 @@ __global__ void __launch_bounds__(LEG_THREADS) legendre_synthesis_kernel(LegArgs
     const int jbase = P.jmin[m] + chunk * (LEG_THREADS * R);
     if (jbase >= P.npairs) return;
 
-    __shared__ double sA[CT], sB[CT];
+    __shared__ double sA[CT];
     __shared__ T sAlm[CT][BT][2];
 
     double cur[R], prev[R], y[R];
@@ -338,13 +402,15 @@ __global__ void __launch_bounds__(LEG_THREADS) legendre_synthesis_kernel(LegArgs
 
     for (int t0 = 0; t0 < nl; t0 += CT) {
         __syncthreads();  // previous tile fully consumed
-        if (tid < CT) recurrence_coeff(m + t0 + 1 + tid, m, sA[tid], sB[tid]);
+        if (tid < CT) sA[tid] = (t0 + 1 + tid < nl) ? P.coef_alpha[abase + m + t0 + 1 + tid] : 0.0;
         for (int e = tid; e < CT * BT * 2; e += LEG_THREADS) {
             const int i = e / (BT * 2), c = (e / 2) % BT, ri = e & 1;
             const int k = t0 + i;
             const int ch = ch0 + c;
             T v = 0;
-            if (k < nl && ch < P.batch) v = inscale * alm[((size_t)ch * P.nalm + abase + m + k) * 2 + ri];
+            if (k < nl && ch < P.batch)  // a_lm s_l: the kernel sums mu_l = lambda_l / s_l
+                v = (T)((double)inscale * P.coef_scale[abase + m + k] *
+                        (double)alm[((size_t)ch * P.nalm + abase + m + k) * 2 + ri]);
             if (m == 0 && ri == 1) v = 0;  // Im a_l0 is ignored
             sAlm[i][c][ri] = v;
         }
@@ -370,7 +436,7 @@ __global__ void __launch_bounds__(LEG_THREADS) legendre_synthesis_kernel(LegArgs
             if (warp_active) {
 #pragma unroll
                 for (int i = 0; i < CHECK_EVERY; ++i) {
-                    const double A = sA[s0 + i], B = sB[s0 + i];
+                    const double A = sA[s0 + i];
 #pragma unroll
                     for (int r = 0; r < R; ++r) {
                         const T lam = (T)cur[r];
@@ -386,7 +452,7 @@ __global__ void __launch_bounds__(LEG_THREADS) legendre_synthesis_kernel(LegArgs
                             }
                         }
                         const double xl = fma(-y[r], cur[r], cur[r]);
-                        const double nx = fma(A, xl, B * prev[r]);
+                        const double nx = fma(A, xl, -prev[r]);
                         prev[r] = cur[r];
                         cur[r] = nx;
                     }
@@ -394,11 +460,11 @@ __global__ void __launch_bounds__(LEG_THREADS) legendre_synthesis_kernel(LegArgs
             } else {
 #pragma unroll
                 for (int i = 0; i < CHECK_EVERY; ++i) {
-                    const double A = sA[s0 + i], B = sB[s0 + i];
+                    const double A = sA[s0 + i];
 #pragma unroll
                     for (int r = 0; r < R; ++r) {
                         const double xl = fma(-y[r], cur[r], cur[r]);
-                        const double nx = fma(A, xl, B * prev[r]);
+                        const double nx = fma(A, xl, -prev[r]);
                         prev[r] = cur[r];
                         cur[r] = nx;
                     }

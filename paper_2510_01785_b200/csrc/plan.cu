@@ -97,7 +97,7 @@ bool pair_active(int lmax, int m, ld pref_m, ld lg2sin, double yj) {
 
 struct Layout {
     size_t off_y, off_lshi, off_lslo, off_ringN, off_start, off_shifted, off_mcut, off_prefhi, off_preflo, off_jmin;
-    size_t off_fft, fft_bytes, off_spectra, off_partial, total;
+    size_t off_fft, fft_bytes, off_alpha, off_scale, off_spectra, off_partial, total;
 };
 
 Layout make_layout(HostPlan& hp) {
@@ -123,6 +123,8 @@ Layout make_layout(HostPlan& hp) {
     cudaError_t err = cudaSuccess;
     L.fft_bytes = plan_fft_tables(hp, nullptr, false, nullptr, &err);
     o = align_up(o + L.fft_bytes);
+    L.off_alpha = take(sizeof(double) * (size_t)d.nalm);
+    L.off_scale = take(sizeof(double) * (size_t)d.nalm);
     const size_t csize = hp.dtype == CUHPX_F64 ? 16 : 8;
     L.off_spectra = take(csize * (size_t)d.batch * d.nrings * d.mstride);
     L.off_partial = o;
@@ -315,6 +317,10 @@ int cuhpx_workspace_init(int nside, int lmax, int mmax, int batch, cuhpx_dtype_t
     d.pref_hi = (const double*)(base + L.off_prefhi);
     d.pref_lo = (const double*)(base + L.off_preflo);
     d.jmin = (const int*)(base + L.off_jmin);
+    d.coef_alpha = (const double*)(base + L.off_alpha);
+    d.coef_scale = (const double*)(base + L.off_scale);
+    if (e == cudaSuccess)
+        e = launch_legendre_coeff(lmax, mmax, (double*)(base + L.off_alpha), (double*)(base + L.off_scale), st);
     d.spectra = base + L.off_spectra;
     d.partial = d.nchunk_max > 1 ? base + L.off_partial : nullptr;
 
