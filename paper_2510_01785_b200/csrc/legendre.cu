@@ -174,40 +174,74 @@ __device__ __forceinline__ void warp_transpose_reduce(T (&v)[NV], int lane) {
 
 // ------------------------------------------------------------------ analysis (row a3)
 // Per warp: every LT degrees the NV = LT*BT*2 per-thread partial sums are reduced over the 32 lanes by a
-// transposing butterfly (NV-1 adds per thread) and parked in shared memory; every GROUP_L degrees one
-// __syncthreads lets the first threads add the 8 warps' values and write a_lm.  Warps whose rings are all still
-// below the significance threshold skip the accumulation (recurrence only).
+// transposing butterfly and parked in shared memory; every GROUP_L degrees one __syncthreads lets the first
+// threads add the warps' values and write a_lm.  The first butterfly level splits (re, im): lanes 16..31 hold
+// their F with re and im swapped, so that every lane KEEPS component slot 0 and SENDS slot 1 -- no selects on the
+// widest level.  Warps whose rings are all still below the significance threshold skip the accumulation.
 constexpr int GROUP_L = 32;  // degrees per cross-warp reduction
 
-template <typename T, int BT, int R, int LT>
-__global__ void __launch_bounds__(LEG_THREADS, 2) legendre_analysis_kernel(LegArgs a) {
+// v[2*k + comp], k < NV/2.  After the call lane L holds in v[0 .. Q-1] the 32-lane totals of
+// (k = Q * ((L & 15) >> SH) + q, comp = L >> 4), Q = max(NV / 32, 1), SH = max(4 - log2(NV/2), 0).
+template <typename T, int NV>
+__device__ __forceinline__ void warp_reduce_split(T (&v)[NV], int lane) {
+    constexpr int H = NV / 2;
+#pragma unroll
+    for (int k = 0; k < H; ++k) v[k] = v[2 * k] + __shfl_xor_sync(0xffffffffu, v[2 * k + 1], 16);
+    int n = H;
+#pragma unroll
+    for (int mask = 8; mask >= 1; mask >>= 1) {
+        if (n > 1) {
+            const int h = n / 2;
+            const bool up = (lane & mask) != 0;
+#pragma unroll
+            for (int i = 0; i < H / 2; ++i) {
+                if (i < h) {
+                    const T send = up ? v[i] : v[i + h];
+                    const T keep = up ? v[i + h] : v[i];
+                    v[i] = keep + __shfl_xor_sync(0xffffffffu, send, mask);
+                }
+            }
+            n = h;
+        } else {
+            v[0] += __shfl_xor_sync(0xffffffffu, v[0], mask);
+        }
+    }
+}
+
+template <typename T, int BT, int R, int LT, int NT>
+__global__ void __launch_bounds__(NT, 512 / NT >= 3 ? 3 : 2) legendre_analysis_kernel(LegArgs a) {
     using T2 = typename Vec2<T>::type;
+    constexpr int NW = NT / 32;
     constexpr int NV = LT * BT * 2;
-    constexpr int Q = NV >= 32 ? NV / 32 : 1;
-    constexpr int SH = NV >= 32 ? 0 : (NV == 16 ? 1 : NV == 8 ? 2 : NV == 4 ? 3 : 4);
+    constexpr int HV = NV / 2;
+    constexpr int Q = HV >= 16 ? HV / 16 : 1;
+    constexpr int SH = HV >= 16 ? 0 : (HV == 8 ? 1 : HV == 4 ? 2 : HV == 2 ? 3 : 4);
     constexpr int TPG = GROUP_L / LT;  // tiles per group
     static_assert(CHECK_EVERY % LT == 0 && CT % GROUP_L == 0 && GROUP_L % CHECK_EVERY == 0, "tile sizes");
-    static_assert(TPG * NV <= LEG_THREADS && NV >= 2, "reduction tile");
+    static_assert(NV >= 4, "reduction tile");
     const DevPlan& P = a.p;
     const int m = blockIdx.x;
     const int chunk = blockIdx.y;
     const int ch0 = blockIdx.z * BT;
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-    const int jbase = P.jmin[m] + chunk * (LEG_THREADS * R);
+    const int jbase = P.jmin[m] + chunk * (NT * R);
     if (jbase >= P.npairs) return;
 
     __shared__ double sA[2][CT];
-    __shared__ T red[2][TPG][LEG_WARPS][NV];
+    __shared__ T red[2][TPG][NW][NV];
 
     const T2* spectra = reinterpret_cast<const T2*>(P.spectra);
     double cur[R], prev[R], y[R];
     int sc[R];
-    T fs[R][BT][2], fa[R][BT][2];  // F_N + F_S and F_N - F_S of the ACTIVE rings (zero while inactive)
+    // F_N + F_S and F_N - F_S of the ACTIVE rings (zero while inactive); [.][.][0] is the component this lane
+    // keeps in the first butterfly level (re for lanes 0-15, im for lanes 16-31), [.][.][1] the one it sends
+    T fs[R][BT][2], fa[R][BT][2];
     int nact = 0;
     const double pref_hi = P.pref_hi[m], pref_lo = P.pref_lo[m];
+    const bool swap_c = (lane & 16) != 0;
 
     auto load_F = [&](int r) {
-        const int j = jbase + tid + LEG_THREADS * r;
+        const int j = jbase + tid + NT * r;
         const int rn = j, rs = P.nrings - 1 - j;
 #pragma unroll
         for (int c = 0; c < BT; ++c) {
@@ -217,16 +251,17 @@ __global__ void __launch_bounds__(LEG_THREADS, 2) legendre_analysis_kernel(LegAr
             fsv.x = 0;
             fsv.y = 0;
             if (rs != rn) fsv = spectra[((size_t)ch * P.nrings + rs) * P.mstride + m];
-            fs[r][c][0] = fn.x + fsv.x;
-            fs[r][c][1] = fn.y + fsv.y;
-            fa[r][c][0] = fn.x - fsv.x;
-            fa[r][c][1] = fn.y - fsv.y;
+            const T sr = fn.x + fsv.x, si = fn.y + fsv.y, ar = fn.x - fsv.x, ai = fn.y - fsv.y;
+            fs[r][c][0] = swap_c ? si : sr;
+            fs[r][c][1] = swap_c ? sr : si;
+            fa[r][c][0] = swap_c ? ai : ar;
+            fa[r][c][1] = swap_c ? ar : ai;
         }
     };
 
 #pragma unroll
     for (int r = 0; r < R; ++r) {
-        const int j = jbase + tid + LEG_THREADS * r;
+        const int j = jbase + tid + NT * r;
 #pragma unroll
         for (int c = 0; c < BT; ++c) fs[r][c][0] = fs[r][c][1] = fa[r][c][0] = fa[r][c][1] = 0;
         if (j < P.npairs) {
@@ -254,7 +289,7 @@ __global__ void __launch_bounds__(LEG_THREADS, 2) legendre_analysis_kernel(LegAr
     bool warp_active = __any_sync(0xffffffffu, nact > 0);
     int buf = 0;
     for (int t0 = 0; t0 < nl; t0 += CT) {
-        // coefficients of degrees l = m + t0 + 1 + i (the step that produces lambda_{l}) for this tile
+        // alpha of the steps that produce degrees l = m + t0 + 1 + i
         const int cb = (t0 / CT) & 1;
         if (tid < CT) sA[cb][tid] = (t0 + 1 + tid < nl) ? P.coef_alpha[abase + m + t0 + 1 + tid] : 0.0;
         __syncthreads();
@@ -304,10 +339,11 @@ __global__ void __launch_bounds__(LEG_THREADS, 2) legendre_analysis_kernel(LegAr
                             cur[r] = nx;
                         }
                     }
-                    warp_transpose_reduce<T, NV>(acc, lane);
+                    warp_reduce_split<T, NV>(acc, lane);
                     if ((lane & ((1 << SH) - 1)) == 0) {
 #pragma unroll
-                        for (int q = 0; q < Q; ++q) red[buf][ti][warp][Q * (lane >> SH) + q] = acc[q];
+                        for (int q = 0; q < Q; ++q)
+                            red[buf][ti][warp][2 * (Q * ((lane & 15) >> SH) + q) + (lane >> 4)] = acc[q];
                     }
                 } else {
 #pragma unroll
@@ -325,11 +361,11 @@ __global__ void __launch_bounds__(LEG_THREADS, 2) legendre_analysis_kernel(LegAr
                 }
             }
             __syncthreads();
-            if (tid < TPG * NV) {
-                const int ti = tid / NV, v = tid % NV;
+            for (int e = tid; e < TPG * NV; e += NT) {
+                const int ti = e / NV, v = e % NV;
                 T sum = 0;
 #pragma unroll
-                for (int w = 0; w < LEG_WARPS; ++w) sum += red[buf][ti][w][v];
+                for (int w = 0; w < NW; ++w) sum += red[buf][ti][w][v];
                 const int i = v / (BT * 2), c = (v / 2) % BT, ri = v & 1;
                 const int k = t0 + g0 + ti * LT + i;  // l - m
                 const int ch = ch0 + c;
@@ -498,13 +534,14 @@ __global__ void __launch_bounds__(LEG_THREADS) legendre_synthesis_kernel(LegArgs
 // ------------------------------------------------------------------ launch configuration
 // R (ring pairs per thread) and LT (l values per reduction tile) per instantiation.
 template <typename T, int BT> struct LegCfg;
-template <> struct LegCfg<double, 1> { static constexpr int R = 4, LT = 8, RS = 4; };
-template <> struct LegCfg<float, 1> { static constexpr int R = 4, LT = 8, RS = 4; };
-template <> struct LegCfg<float, 4> { static constexpr int R = 2, LT = 4, RS = 2; };
+// analysis: NT threads x R ring pairs = one chunk; synthesis: LEG_THREADS x RS
+template <> struct LegCfg<double, 1> { static constexpr int NT = 128, R = 8, LT = 8, RS = 4; };
+template <> struct LegCfg<float, 1> { static constexpr int NT = 128, R = 8, LT = 8, RS = 4; };
+template <> struct LegCfg<float, 4> { static constexpr int NT = 256, R = 2, LT = 4, RS = 2; };
 
 int legendre_chunk_pairs(cuhpx_dtype_t dt, int batch) {
-    if (dt == CUHPX_F64) return LEG_THREADS * LegCfg<double, 1>::R;
-    return batch >= 4 ? LEG_THREADS * LegCfg<float, 4>::R : LEG_THREADS * LegCfg<float, 1>::R;
+    if (dt == CUHPX_F64) return LegCfg<double, 1>::NT * LegCfg<double, 1>::R;
+    return batch >= 4 ? LegCfg<float, 4>::NT * LegCfg<float, 4>::R : LegCfg<float, 1>::NT * LegCfg<float, 1>::R;
 }
 
 template <typename T, int BT>
@@ -518,7 +555,7 @@ static cudaError_t run_analysis(const HostPlan& hp, void* d_alm, int adjoint, cu
     a.to_partial = P.nchunk_max > 1;
     a.out = a.to_partial ? P.partial : d_alm;
     dim3 grid(P.mmax + 1, P.nchunk_max, (P.batch + BT - 1) / BT);
-    legendre_analysis_kernel<T, BT, C::R, C::LT><<<grid, LEG_THREADS, 0, st>>>(a);
+    legendre_analysis_kernel<T, BT, C::R, C::LT, C::NT><<<grid, C::NT, 0, st>>>(a);
     cudaError_t e = cudaGetLastError();
     if (e != cudaSuccess) return e;
     if (a.to_partial) {
