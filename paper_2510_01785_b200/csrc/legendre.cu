@@ -537,7 +537,7 @@ template <typename T, int BT> struct LegCfg;
 // analysis: NT threads x R ring pairs = one chunk; synthesis: LEG_THREADS x RS
 template <> struct LegCfg<double, 1> { static constexpr int NT = 128, R = 8, LT = 8, RS = 4; };
 template <> struct LegCfg<float, 1> { static constexpr int NT = 128, R = 8, LT = 8, RS = 4; };
-template <> struct LegCfg<float, 4> { static constexpr int NT = 256, R = 2, LT = 4, RS = 2; };
+template <> struct LegCfg<float, 4> { static constexpr int NT = 128, R = 4, LT = 4, RS = 2; };
 
 int legendre_chunk_pairs(cuhpx_dtype_t dt, int batch) {
     if (dt == CUHPX_F64) return LegCfg<double, 1>::NT * LegCfg<double, 1>::R;

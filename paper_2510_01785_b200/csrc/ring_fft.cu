@@ -333,7 +333,7 @@ __global__ void __launch_bounds__(FftPlan<LOGN>::NT) ring_pow2_synthesis_kernel(
 // ------------------------------------------------------------------ Bluestein rings (N = 4 i, i not a power of two)
 // chirp c[u] = exp(-i pi u^2 / i) from the exact integer u^2 mod 2i  (Eq. 19 P:222 with N -> i)
 template <typename T> __device__ __forceinline__ void chirp(int u, int i, T& c, T& s) {
-    cispi_ratio((long long)((u * u) % (2 * i)), i, (T)-1, c, s);
+    cispi_ratio((long long)(((unsigned)u * (unsigned)u) % (unsigned)(2 * i)), i, (T)-1, c, s);
 }
 
 // One length-i chirp-z transform of the sequence already multiplied by the chirp and zero-padded in registers
@@ -355,7 +355,7 @@ __device__ __forceinline__ void chirp_convolve(T (&re)[BlockFFT<T, LOGM>::E], T 
 }
 
 template <typename T, int LOGM>
-__global__ void __launch_bounds__(FftPlan<LOGM>::NT) ring_blue_analysis_kernel(DevPlan P, const int* __restrict__ rings,
+__global__ void __launch_bounds__(FftPlan<LOGM>::NT, 512 / FftPlan<LOGM>::NT) ring_blue_analysis_kernel(DevPlan P, const int* __restrict__ rings,
                                                                                const T* __restrict__ map,
                                                                                const double* __restrict__ w, int use_w,
                                                                                FftTables tabs) {
@@ -410,32 +410,50 @@ __global__ void __launch_bounds__(FftPlan<LOGM>::NT) ring_blue_analysis_kernel(D
         }
     }
     __syncthreads();
-    // Z[q] = Ze[q mod i] + W_n^q Zo[q mod i], q < n = 2 i
+    // Z[q] = Ze[q mod i] + W_n^q Zo[q mod i], q < n = 2 i.  Every phase factor is a power of
+    // omega = exp(-i pi / (4 i)): twist = omega^m, W_N^kk = omega^(2 kk), W_n^q = omega^(4 q); without aliasing
+    // (m <= n, the common case) kk = m and one sincospi per output suffices.
     const Cis<T, false> cis{tw, tabs.twlen};
-    auto Zq = [&](int q, T& zr, T& zi) {
-        const int qi = q >= i ? q - i : q;
-        T c, s;
-        cis.template get<-1>(q, n, c, s);
-        const T2 ze = Ze[qi];
-        const T orr = sre[padi<T>(qi)], oi = sim[padi<T>(qi)];
-        zr = ze.x + (orr * c - oi * s);
-        zi = ze.y + (orr * s + oi * c);
-    };
     T2* dst = reinterpret_cast<T2*>(P.spectra) + ((size_t)ch * P.nrings + r) * P.mstride;
     const T wt = (T)R.weight;
     for (int m = tid; m <= R.mcut; m += NT) {
         const int k = m % N;
         const bool cj = k > n;
         const int kk = cj ? N - k : k;
-        T z1r, z1i, z2r, z2i;
-        Zq(kk == n ? 0 : kk, z1r, z1i);
-        Zq(kk == 0 ? 0 : n - kk, z2r, z2i);
-        dst[m] = analysis_unpack<T, false>(z1r, z1i, z2r, z2i, m, kk, cj, N, R.shifted, wt, cis);
+        T pc, ps;  // omega^kk
+        cis.template get<-1>(kk, 2 * N, pc, ps);
+        const T w2c = pc * pc - ps * ps, w2s = 2 * pc * ps;      // W_N^kk
+        const T w4c = w2c * w2c - w2s * w2s, w4s = 2 * w2c * w2s;  // W_n^kk
+        const int q1 = kk == n ? 0 : kk, q2 = kk == 0 ? 0 : n - kk;
+        const int a1 = q1 >= i ? q1 - i : q1, a2 = q2 >= i ? q2 - i : q2;
+        // W_n^(n - kk) = conj(W_n^kk); W_n^0 = 1
+        const T c1 = (kk == n) ? (T)1 : w4c, s1 = (kk == n) ? (T)0 : w4s;
+        const T c2 = (kk == 0) ? (T)1 : w4c, s2 = (kk == 0) ? (T)0 : -w4s;
+        const T2 ze1 = Ze[a1], ze2 = Ze[a2];
+        const T o1r = sre[padi<T>(a1)], o1i = sim[padi<T>(a1)], o2r = sre[padi<T>(a2)], o2i = sim[padi<T>(a2)];
+        const T z1r = ze1.x + (o1r * c1 - o1i * s1), z1i = ze1.y + (o1r * s1 + o1i * c1);
+        const T z2r = ze2.x + (o2r * c2 - o2i * s2), z2i = ze2.y + (o2r * s2 + o2i * c2);
+        const T er = (T)0.5 * (z1r + z2r), ei = (T)0.5 * (z1i - z2i);
+        const T dr = (T)0.5 * (z1r - z2r), di = (T)0.5 * (z1i + z2i);
+        T xr = er + (w2c * di + w2s * dr);
+        T xi = ei + (w2s * di - w2c * dr);
+        if (cj) xi = -xi;
+        if (R.shifted) {
+            T tc = pc, ts = ps;
+            if (k != m || cj) cis.template get<-1>(m % (2 * N), 2 * N, tc, ts);  // aliased: twist != omega^kk
+            const T tr = xr * tc - xi * ts, ti = xr * ts + xi * tc;
+            xr = tr;
+            xi = ti;
+        }
+        T2 o;
+        o.x = wt * xr;
+        o.y = wt * xi;
+        dst[m] = o;
     }
 }
 
 template <typename T, int LOGM>
-__global__ void __launch_bounds__(FftPlan<LOGM>::NT) ring_blue_synthesis_kernel(DevPlan P, const int* __restrict__ rings,
+__global__ void __launch_bounds__(FftPlan<LOGM>::NT, 512 / FftPlan<LOGM>::NT) ring_blue_synthesis_kernel(DevPlan P, const int* __restrict__ rings,
                                                                                 T* __restrict__ map,
                                                                                 const double* __restrict__ w, int use_w,
                                                                                 FftTables tabs) {
