@@ -216,15 +216,37 @@ __device__ __forceinline__ void folded_H(const typename V2<T>::type* __restrict_
 template <typename T, bool POW2>
 __device__ __forceinline__ void synth_packed_input(const typename V2<T>::type* __restrict__ G, int k, int N, int mcut,
                                                    int shifted, const Cis<T, POW2>& cis, T& yr, T& yi) {
+    using T2 = typename V2<T>::type;
     const int n = N >> 1;
-    T ar, ai, br, bi;
-    folded_H<T, POW2>(G, k, N, mcut, shifted, cis, ar, ai);
-    folded_H<T, POW2>(G, n - k, N, mcut, shifted, cis, br, bi);
+    T ar, ai, br, bi, c, s;
+    if (mcut < n) {
+        // no order reaches the Nyquist bin: H[k] = G_k e^{i k phi0} for k <= mcut, else 0.  With p = e^{i pi k / N}:
+        // twist of bin k is p, of bin n - k is i conj(p), and e^{2 pi i k / N} = p^2: one sincos per element.
+        T pc, ps;
+        cis.template get<+1>(k, 2 * N, pc, ps);
+        T2 a, b;
+        a.x = a.y = b.x = b.y = 0;
+        if (k <= mcut) a = G[k];
+        if (n - k <= mcut) b = G[n - k];
+        if (k == 0) a.y = 0;  // Im G_0 is ignored
+        if (shifted) {
+            ar = a.x * pc - a.y * ps;
+            ai = a.x * ps + a.y * pc;
+            br = b.x * ps - b.y * pc;  // b * (ps + i pc)
+            bi = b.x * pc + b.y * ps;
+        } else {
+            ar = a.x; ai = a.y; br = b.x; bi = b.y;
+        }
+        c = pc * pc - ps * ps;
+        s = 2 * pc * ps;
+    } else {
+        folded_H<T, POW2>(G, k, N, mcut, shifted, cis, ar, ai);
+        folded_H<T, POW2>(G, n - k, N, mcut, shifted, cis, br, bi);
+        cis.template get<+1>(k, N, c, s);
+    }
     bi = -bi;  // conj H[n-k]
     const T er = ar + br, ei = ai + bi;
     const T dr = ar - br, di = ai - bi;
-    T c, s;
-    cis.template get<+1>(k, N, c, s);
     const T orr = dr * c - di * s, oi = dr * s + di * c;
     // Zs = E' + i O' = (er - oi) + i (ei + orr);  Y = conj
     yr = er - oi;
