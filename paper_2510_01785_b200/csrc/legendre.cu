@@ -380,6 +380,159 @@ __global__ void __launch_bounds__(NT, 512 / NT >= 3 ? 3 : 2) legendre_analysis_k
     }
 }
 
+// ------------------------------------------------------------------ analysis, batched fp32 (row a3 as a contraction)
+// With >= 8 channels the Legendre stage really is a dense contraction per m (north_star): C[l][c] = sum_j
+// Lambda[l][j] F[j][c], c = (channel, re/im), j = ring pairs.  One CTA = (m, 256 ring pairs, 8 channels): each
+// thread walks the recurrence of ONE ring pair in fp64 and parks lambda (fp32, 0 while the ring is insignificant)
+// for 32 degrees in shared memory, [parity][ring][16 degrees]; then the CTA multiplies that 32 x 256 tile with the
+// resident F tile (F_N + F_S for even l - m, F_N - F_S for odd) as a register-blocked SGEMM: warp = 32 rings of K,
+// thread = 4 degrees (one parity) x 4 columns, one LDS.128 of lambda + one of F per 16 FFMA; the 8 warps' partial
+// tiles meet in shared memory.  lambda is converted to fp32 once per (l, ring) for all 8 channels.
+constexpr int GK = 256;    // ring pairs per CTA (= threads)
+constexpr int GTL = 32;    // degrees per tile
+constexpr int GROW = 20;   // floats per lambda row: 16 + 4 padding (conflict-free 16-byte stores at 80-byte pitch)
+constexpr int GNCH = 8;    // channels per CTA
+constexpr int GNC = 2 * GNCH;
+
+__global__ void __launch_bounds__(GK, 3) legendre_analysis_gemm_kernel(LegArgs a) {
+    const DevPlan& P = a.p;
+    const int m = blockIdx.x;
+    const int chunk = blockIdx.y;
+    const int ch0 = blockIdx.z * GNCH;
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const int jbase = P.jmin[m] + chunk * GK;
+    if (jbase >= P.npairs) return;
+
+    extern __shared__ __align__(16) unsigned char gemm_smem[];
+    float* sLam = reinterpret_cast<float*>(gemm_smem);  // [parity][ring][GROW]; reused for the cross-warp sums
+    float(*sF)[GK][GNC] = reinterpret_cast<float(*)[GK][GNC]>(sLam + 2 * GK * GROW);  // [0] = F_N + F_S, [1] = F_N - F_S
+    double(*sA)[GTL] = reinterpret_cast<double(*)[GTL]>(sLam + 2 * GK * GROW + 2 * GK * GNC);
+
+    const float2* spectra = reinterpret_cast<const float2*>(P.spectra);
+    const int j = jbase + tid;
+    const bool valid = j < P.npairs;
+    double cur = 0.0, prev = 0.0, y = 1.0;
+    int sc = -1;
+    {
+        float fsum[GNC], fdif[GNC];
+#pragma unroll
+        for (int c = 0; c < GNC; ++c) fsum[c] = fdif[c] = 0.f;
+        if (valid) {
+            y = P.y[j];
+            lambda_seed<float>(m, P.pref_hi[m], P.pref_lo[m], P.ls_hi[j], P.ls_lo[j], cur, sc);
+            const int rn = j, rs = P.nrings - 1 - j;
+#pragma unroll
+            for (int c = 0; c < GNCH; ++c) {
+                if (ch0 + c < P.batch) {
+                    const float2 fn = spectra[((size_t)(ch0 + c) * P.nrings + rn) * P.mstride + m];
+                    float2 fv = make_float2(0.f, 0.f);
+                    if (rs != rn) fv = spectra[((size_t)(ch0 + c) * P.nrings + rs) * P.mstride + m];
+                    fsum[2 * c] = fn.x + fv.x;
+                    fsum[2 * c + 1] = fn.y + fv.y;
+                    fdif[2 * c] = fn.x - fv.x;
+                    fdif[2 * c + 1] = fn.y - fv.y;
+                }
+            }
+        }
+#pragma unroll
+        for (int c = 0; c < GNC; c += 4) {
+            *reinterpret_cast<float4*>(&sF[0][tid][c]) = make_float4(fsum[c], fsum[c + 1], fsum[c + 2], fsum[c + 3]);
+            *reinterpret_cast<float4*>(&sF[1][tid][c]) = make_float4(fdif[c], fdif[c + 1], fdif[c + 2], fdif[c + 3]);
+        }
+    }
+    const double outscale = (a.adjoint && m > 0) ? 2.0 : 1.0;
+    const long long abase = (long long)m * (2LL * P.lmax + 1 - m) / 2;
+    float* out = reinterpret_cast<float*>(a.out);
+    if (a.to_partial) out += (size_t)chunk * P.batch * P.nalm * 2;
+    const int nl = P.lmax - m + 1;
+
+    if (tid < GTL) sA[0][tid] = (1 + tid < nl) ? P.coef_alpha[abase + m + 1 + tid] : 0.0;
+    __syncthreads();
+
+    // contraction-phase coordinates
+    const int par = lane >> 4;          // lanes 0-15: even l - m, 16-31: odd
+    const int lquad = (lane >> 2) & 3;  // 4 degrees of that parity
+    const int cq = lane & 3;            // 4 columns
+
+    for (int t0 = 0, tb = 0; t0 < nl; t0 += GTL, tb ^= 1) {
+        // prefetch alpha of the next tile (visible after this tile's barriers)
+        if (tid < GTL) sA[tb ^ 1][tid] = (t0 + GTL + 1 + tid < nl) ? P.coef_alpha[abase + m + t0 + GTL + 1 + tid] : 0.0;
+        // ---- generate 32 degrees of this thread's ring
+#pragma unroll
+        for (int q = 0; q < GTL / 8; ++q) {
+            if (sc < 0 && fabs(cur) > pow2c(ScaleCfg<float>::THR)) {
+                cur *= pow2c(-ScaleCfg<float>::K);
+                prev *= pow2c(-ScaleCfg<float>::K);
+                ++sc;
+            }
+            float e[4], o[4];
+#pragma unroll
+            for (int p = 0; p < 4; ++p) {
+                e[p] = sc == 0 ? (float)cur : 0.f;
+                double xl = fma(-y, cur, cur);
+                double nx = fma(sA[tb][8 * q + 2 * p], xl, -prev);
+                prev = cur;
+                cur = nx;
+                o[p] = sc == 0 ? (float)cur : 0.f;
+                xl = fma(-y, cur, cur);
+                nx = fma(sA[tb][8 * q + 2 * p + 1], xl, -prev);
+                prev = cur;
+                cur = nx;
+            }
+            *reinterpret_cast<float4*>(&sLam[(0 * GK + tid) * GROW + 4 * q]) = make_float4(e[0], e[1], e[2], e[3]);
+            *reinterpret_cast<float4*>(&sLam[(1 * GK + tid) * GROW + 4 * q]) = make_float4(o[0], o[1], o[2], o[3]);
+        }
+        const bool any = __syncthreads_or(sc == 0);
+        if (any) {
+            float acc[4][4];
+#pragma unroll
+            for (int x = 0; x < 4; ++x)
+#pragma unroll
+                for (int z = 0; z < 4; ++z) acc[x][z] = 0.f;
+            const float* lp = &sLam[(par * GK + warp * 32) * GROW + 4 * lquad];
+            const float* fp = &sF[par][warp * 32][4 * cq];
+#pragma unroll 8
+            for (int kk = 0; kk < 32; ++kk) {
+                const float4 l4 = *reinterpret_cast<const float4*>(lp + kk * GROW);
+                const float4 f4 = *reinterpret_cast<const float4*>(fp + kk * GNC);
+                const float lv[4] = {l4.x, l4.y, l4.z, l4.w}, fv[4] = {f4.x, f4.y, f4.z, f4.w};
+#pragma unroll
+                for (int x = 0; x < 4; ++x)
+#pragma unroll
+                    for (int z = 0; z < 4; ++z) acc[x][z] = fmaf(lv[x], fv[z], acc[x][z]);
+            }
+            __syncthreads();  // every warp is done reading sLam
+            float* red = sLam;  // [warp][lane][16]
+#pragma unroll
+            for (int x = 0; x < 4; ++x)
+                *reinterpret_cast<float4*>(&red[(warp * 32 + lane) * 16 + 4 * x]) =
+                    make_float4(acc[x][0], acc[x][1], acc[x][2], acc[x][3]);
+            __syncthreads();
+        }
+#pragma unroll
+        for (int rep = 0; rep < 2; ++rep) {
+            const int e = tid + GK * rep;     // 512 outputs of the tile
+            const int ln = e >> 4, ix = e & 15;  // producing lane slot, element of its 4 x 4 block
+            float sum = 0.f;
+            if (any) {
+#pragma unroll
+                for (int w = 0; w < GK / 32; ++w) sum += sLam[(w * 32 + ln) * 16 + ix];
+            }
+            const int opar = ln >> 4, olq = (ln >> 2) & 3, ocq = ln & 3;
+            const int i = 2 * (4 * olq + (ix >> 2)) + opar;  // l - m - t0
+            const int c = 4 * ocq + (ix & 3);
+            const int ch = ch0 + (c >> 1), ri = c & 1;
+            const int k = t0 + i;
+            if (k < nl && ch < P.batch) {
+                float o = (float)(outscale * P.coef_scale[abase + m + k] * (double)sum);
+                if (m == 0 && ri == 1) o = 0.f;
+                out[((size_t)ch * P.nalm + abase + m + k) * 2 + ri] = o;
+            }
+        }
+        if (any) __syncthreads();  // sums consumed before the next tile overwrites sLam
+    }
+}
+
 // sum the per-chunk partial results: alm[b][idx] = sum_c partial[c][b][idx], c < nchunks(m)
 template <typename T>
 __global__ void combine_partials_kernel(DevPlan P, const T* __restrict__ partial, T* __restrict__ alm) {
@@ -397,15 +550,15 @@ __global__ void combine_partials_kernel(DevPlan P, const T* __restrict__ partial
 }
 
 // ------------------------------------------------------------------ synthesis (row s1)
-template <typename T, int BT, int R>
-__global__ void __launch_bounds__(LEG_THREADS) legendre_synthesis_kernel(LegArgs a) {
+template <typename T, int BT, int R, int NT>
+__global__ void __launch_bounds__(NT) legendre_synthesis_kernel(LegArgs a) {
     using T2 = typename Vec2<T>::type;
     const DevPlan& P = a.p;
     const int m = blockIdx.x;
     const int chunk = blockIdx.y;
     const int ch0 = blockIdx.z * BT;
     const int tid = threadIdx.x;
-    const int jbase = P.jmin[m] + chunk * (LEG_THREADS * R);
+    const int jbase = P.jmin[m] + chunk * (NT * R);
     if (jbase >= P.npairs) return;
 
     __shared__ double sA[CT];
@@ -417,7 +570,7 @@ __global__ void __launch_bounds__(LEG_THREADS) legendre_synthesis_kernel(LegArgs
     const double pref_hi = P.pref_hi[m], pref_lo = P.pref_lo[m];
 #pragma unroll
     for (int r = 0; r < R; ++r) {
-        const int j = jbase + tid + LEG_THREADS * r;
+        const int j = jbase + tid + NT * r;
 #pragma unroll
         for (int c = 0; c < BT; ++c) E[r][c][0] = E[r][c][1] = O[r][c][0] = O[r][c][1] = 0;
         if (j < P.npairs) {
@@ -439,7 +592,7 @@ __global__ void __launch_bounds__(LEG_THREADS) legendre_synthesis_kernel(LegArgs
     for (int t0 = 0; t0 < nl; t0 += CT) {
         __syncthreads();  // previous tile fully consumed
         if (tid < CT) sA[tid] = (t0 + 1 + tid < nl) ? P.coef_alpha[abase + m + t0 + 1 + tid] : 0.0;
-        for (int e = tid; e < CT * BT * 2; e += LEG_THREADS) {
+        for (int e = tid; e < CT * BT * 2; e += NT) {
             const int i = e / (BT * 2), c = (e / 2) % BT, ri = e & 1;
             const int k = t0 + i;
             const int ch = ch0 + c;
@@ -512,7 +665,7 @@ __global__ void __launch_bounds__(LEG_THREADS) legendre_synthesis_kernel(LegArgs
     T2* spectra = reinterpret_cast<T2*>(P.spectra);
 #pragma unroll
     for (int r = 0; r < R; ++r) {
-        const int j = jbase + tid + LEG_THREADS * r;
+        const int j = jbase + tid + NT * r;
         if (j >= P.npairs) continue;
         const int rn = j, rs = P.nrings - 1 - j;
         const bool live = sc[r] == 0;
@@ -535,12 +688,14 @@ __global__ void __launch_bounds__(LEG_THREADS) legendre_synthesis_kernel(LegArgs
 // R (ring pairs per thread) and LT (l values per reduction tile) per instantiation.
 template <typename T, int BT> struct LegCfg;
 // analysis: NT threads x R ring pairs = one chunk; synthesis: LEG_THREADS x RS
-template <> struct LegCfg<double, 1> { static constexpr int NT = 128, R = 8, LT = 8, RS = 4; };
-template <> struct LegCfg<float, 1> { static constexpr int NT = 128, R = 8, LT = 8, RS = 4; };
-template <> struct LegCfg<float, 4> { static constexpr int NT = 128, R = 4, LT = 4, RS = 2; };
+template <> struct LegCfg<double, 1> { static constexpr int NT = 128, R = 8, LT = 8, RS = 4, NTS = 256; };
+template <> struct LegCfg<float, 1> { static constexpr int NT = 128, R = 8, LT = 8, RS = 4, NTS = 256; };
+template <> struct LegCfg<float, 4> { static constexpr int NT = 128, R = 4, LT = 4, RS = 2, NTS = 256; };
+template <> struct LegCfg<float, 8> { static constexpr int NT = 128, R = 4, LT = 2, RS = 2, NTS = 128; };
 
 int legendre_chunk_pairs(cuhpx_dtype_t dt, int batch) {
     if (dt == CUHPX_F64) return LegCfg<double, 1>::NT * LegCfg<double, 1>::R;
+    if (batch >= 5) return GK;  // contraction kernel
     return batch >= 4 ? LegCfg<float, 4>::NT * LegCfg<float, 4>::R : LegCfg<float, 1>::NT * LegCfg<float, 1>::R;
 }
 
@@ -577,20 +732,47 @@ static cudaError_t run_synthesis(const HostPlan& hp, const void* d_alm, int adjo
     a.out = nullptr;
     a.adjoint = adjoint;
     a.to_partial = 0;
-    const int chunk = LEG_THREADS * C::RS;
+    const int chunk = C::NTS * C::RS;
     dim3 grid(P.mmax + 1, (P.npairs + chunk - 1) / chunk, (P.batch + BT - 1) / BT);
-    legendre_synthesis_kernel<T, BT, C::RS><<<grid, LEG_THREADS, 0, st>>>(a);
+    legendre_synthesis_kernel<T, BT, C::RS, C::NTS><<<grid, C::NTS, 0, st>>>(a);
     return cudaGetLastError();
+}
+
+static cudaError_t run_analysis_gemm(const HostPlan& hp, void* d_alm, int adjoint, cudaStream_t st) {
+    const DevPlan& P = hp.d;
+    LegArgs a;
+    a.p = P;
+    a.in = nullptr;
+    a.adjoint = adjoint;
+    a.to_partial = P.nchunk_max > 1;
+    a.out = a.to_partial ? P.partial : d_alm;
+    dim3 grid(P.mmax + 1, P.nchunk_max, (P.batch + GNCH - 1) / GNCH);
+    constexpr size_t smem = sizeof(float) * (2 * GK * GROW + 2 * GK * GNC) + sizeof(double) * 2 * GTL;
+    cudaError_t e = cudaFuncSetAttribute(legendre_analysis_gemm_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    if (e != cudaSuccess) return e;
+    legendre_analysis_gemm_kernel<<<grid, GK, smem, st>>>(a);
+    e = cudaGetLastError();
+    if (e != cudaSuccess) return e;
+    if (a.to_partial) {
+        dim3 g2(P.mmax + 1, P.batch);
+        combine_partials_kernel<float><<<g2, 256, 0, st>>>(P, reinterpret_cast<const float*>(P.partial),
+                                                            reinterpret_cast<float*>(d_alm));
+        e = cudaGetLastError();
+    }
+    return e;
 }
 
 cudaError_t launch_legendre_analysis(const HostPlan& hp, void* d_alm, int adjoint, cudaStream_t st) {
     if (hp.dtype == CUHPX_F64) return run_analysis<double, 1>(hp, d_alm, adjoint, st);
+    if (hp.d.batch >= 5) return run_analysis_gemm(hp, d_alm, adjoint, st);
     if (hp.d.batch >= 4) return run_analysis<float, 4>(hp, d_alm, adjoint, st);
     return run_analysis<float, 1>(hp, d_alm, adjoint, st);
 }
 
 cudaError_t launch_legendre_synthesis(const HostPlan& hp, const void* d_alm, int adjoint, cudaStream_t st) {
     if (hp.dtype == CUHPX_F64) return run_synthesis<double, 1>(hp, d_alm, adjoint, st);
+    // 8 channels per CTA pay off when there are few (m, ring chunk) CTAs to fill the GPU with (measured: cfg3 yes, cfg4 no)
+    if (hp.d.batch >= 8 && hp.d.lmax < 1024) return run_synthesis<float, 8>(hp, d_alm, adjoint, st);
     if (hp.d.batch >= 4) return run_synthesis<float, 4>(hp, d_alm, adjoint, st);
     return run_synthesis<float, 1>(hp, d_alm, adjoint, st);
 }
