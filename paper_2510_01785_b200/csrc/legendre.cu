@@ -407,6 +407,7 @@ __global__ void __launch_bounds__(GK, 3) legendre_analysis_gemm_kernel(LegArgs a
     float* sLam = reinterpret_cast<float*>(gemm_smem);  // [parity][ring][GROW]; reused for the cross-warp sums
     float(*sF)[GK][GNC] = reinterpret_cast<float(*)[GK][GNC]>(sLam + 2 * GK * GROW);  // [0] = F_N + F_S, [1] = F_N - F_S
     double(*sA)[GTL] = reinterpret_cast<double(*)[GTL]>(sLam + 2 * GK * GROW + 2 * GK * GNC);
+    double(*sS)[GTL] = sA + 2;  // outscale * s_l of the tile's degrees
 
     const float2* spectra = reinterpret_cast<const float2*>(P.spectra);
     const int j = jbase + tid;
@@ -446,17 +447,26 @@ __global__ void __launch_bounds__(GK, 3) legendre_analysis_gemm_kernel(LegArgs a
     if (a.to_partial) out += (size_t)chunk * P.batch * P.nalm * 2;
     const int nl = P.lmax - m + 1;
 
-    if (tid < GTL) sA[0][tid] = (1 + tid < nl) ? P.coef_alpha[abase + m + 1 + tid] : 0.0;
+    if (tid < GTL) {
+        sA[0][tid] = (1 + tid < nl) ? P.coef_alpha[abase + m + 1 + tid] : 0.0;
+        sS[0][tid] = (tid < nl) ? outscale * P.coef_scale[abase + m + tid] : 0.0;
+    }
     __syncthreads();
 
     // contraction-phase coordinates
     const int par = lane >> 4;          // lanes 0-15: even l - m, 16-31: odd
     const int lquad = (lane >> 2) & 3;  // 4 degrees of that parity
     const int cq = lane & 3;            // 4 columns
+    // A warp generates lambda for exactly the 32 rings it contracts over: generation -> contraction needs only
+    // __syncwarp; the CTA meets twice per tile (partial tiles written / consumed).
+    float* wred = &sLam[(0 * GK + warp * 32) * GROW];  // this warp's partial tile, aliased on its own lambda rows
 
     for (int t0 = 0, tb = 0; t0 < nl; t0 += GTL, tb ^= 1) {
-        // prefetch alpha of the next tile (visible after this tile's barriers)
-        if (tid < GTL) sA[tb ^ 1][tid] = (t0 + GTL + 1 + tid < nl) ? P.coef_alpha[abase + m + t0 + GTL + 1 + tid] : 0.0;
+        // prefetch alpha / scale of the next tile (visible after this tile's barriers)
+        if (tid < GTL) {
+            sA[tb ^ 1][tid] = (t0 + GTL + 1 + tid < nl) ? P.coef_alpha[abase + m + t0 + GTL + 1 + tid] : 0.0;
+            sS[tb ^ 1][tid] = (t0 + GTL + tid < nl) ? outscale * P.coef_scale[abase + m + t0 + GTL + tid] : 0.0;
+        }
         // ---- generate 32 degrees of this thread's ring
 #pragma unroll
         for (int q = 0; q < GTL / 8; ++q) {
@@ -482,13 +492,13 @@ __global__ void __launch_bounds__(GK, 3) legendre_analysis_gemm_kernel(LegArgs a
             *reinterpret_cast<float4*>(&sLam[(0 * GK + tid) * GROW + 4 * q]) = make_float4(e[0], e[1], e[2], e[3]);
             *reinterpret_cast<float4*>(&sLam[(1 * GK + tid) * GROW + 4 * q]) = make_float4(o[0], o[1], o[2], o[3]);
         }
-        const bool any = __syncthreads_or(sc == 0);
+        const bool any = __any_sync(0xffffffffu, sc == 0);  // also orders the warp's stores before its loads
+        float acc[4][4];
+#pragma unroll
+        for (int x = 0; x < 4; ++x)
+#pragma unroll
+            for (int z = 0; z < 4; ++z) acc[x][z] = 0.f;
         if (any) {
-            float acc[4][4];
-#pragma unroll
-            for (int x = 0; x < 4; ++x)
-#pragma unroll
-                for (int z = 0; z < 4; ++z) acc[x][z] = 0.f;
             const float* lp = &sLam[(par * GK + warp * 32) * GROW + 4 * lquad];
             const float* fp = &sF[par][warp * 32][4 * cq];
 #pragma unroll 8
@@ -501,35 +511,31 @@ __global__ void __launch_bounds__(GK, 3) legendre_analysis_gemm_kernel(LegArgs a
 #pragma unroll
                     for (int z = 0; z < 4; ++z) acc[x][z] = fmaf(lv[x], fv[z], acc[x][z]);
             }
-            __syncthreads();  // every warp is done reading sLam
-            float* red = sLam;  // [warp][lane][16]
-#pragma unroll
-            for (int x = 0; x < 4; ++x)
-                *reinterpret_cast<float4*>(&red[(warp * 32 + lane) * 16 + 4 * x]) =
-                    make_float4(acc[x][0], acc[x][1], acc[x][2], acc[x][3]);
-            __syncthreads();
         }
+        __syncwarp();  // the warp is done reading its lambda rows
+#pragma unroll
+        for (int x = 0; x < 4; ++x)
+            *reinterpret_cast<float4*>(&wred[lane * 16 + 4 * x]) = make_float4(acc[x][0], acc[x][1], acc[x][2], acc[x][3]);
+        __syncthreads();
 #pragma unroll
         for (int rep = 0; rep < 2; ++rep) {
-            const int e = tid + GK * rep;     // 512 outputs of the tile
+            const int e = tid + GK * rep;        // 512 outputs of the tile
             const int ln = e >> 4, ix = e & 15;  // producing lane slot, element of its 4 x 4 block
             float sum = 0.f;
-            if (any) {
 #pragma unroll
-                for (int w = 0; w < GK / 32; ++w) sum += sLam[(w * 32 + ln) * 16 + ix];
-            }
+            for (int w = 0; w < GK / 32; ++w) sum += sLam[(w * 32) * GROW + ln * 16 + ix];
             const int opar = ln >> 4, olq = (ln >> 2) & 3, ocq = ln & 3;
             const int i = 2 * (4 * olq + (ix >> 2)) + opar;  // l - m - t0
             const int c = 4 * ocq + (ix & 3);
             const int ch = ch0 + (c >> 1), ri = c & 1;
             const int k = t0 + i;
             if (k < nl && ch < P.batch) {
-                float o = (float)(outscale * P.coef_scale[abase + m + k] * (double)sum);
+                float o = (float)(sS[tb][i] * (double)sum);
                 if (m == 0 && ri == 1) o = 0.f;
                 out[((size_t)ch * P.nalm + abase + m + k) * 2 + ri] = o;
             }
         }
-        if (any) __syncthreads();  // sums consumed before the next tile overwrites sLam
+        __syncthreads();  // partial tiles consumed before the next tile overwrites the lambda rows
     }
 }
 
@@ -747,7 +753,7 @@ static cudaError_t run_analysis_gemm(const HostPlan& hp, void* d_alm, int adjoin
     a.to_partial = P.nchunk_max > 1;
     a.out = a.to_partial ? P.partial : d_alm;
     dim3 grid(P.mmax + 1, P.nchunk_max, (P.batch + GNCH - 1) / GNCH);
-    constexpr size_t smem = sizeof(float) * (2 * GK * GROW + 2 * GK * GNC) + sizeof(double) * 2 * GTL;
+    constexpr size_t smem = sizeof(float) * (2 * GK * GROW + 2 * GK * GNC) + sizeof(double) * 4 * GTL;
     cudaError_t e = cudaFuncSetAttribute(legendre_analysis_gemm_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return e;
     legendre_analysis_gemm_kernel<<<grid, GK, smem, st>>>(a);
