@@ -26,7 +26,7 @@ if ROOT not in sys.path:
 
 import numpy as np  # noqa: E402
 
-from paper_2510_01785_b200 import synth  # noqa: E402
+from paper_2510_01785_b200 import replicas, synth  # noqa: E402
 
 METRIC = "map2alm/alm2map transforms/s at Nside 1024-4096; % of FP64/HBM roofline"
 UNIT = "transforms/s"
@@ -193,7 +193,7 @@ def main():
     # ---- inputs (synthetic, seeded): alm ~ (l+1)^-2 power law; the map inputs of the
     # analysis-type calls are the synthesised map (+ sigma = 0.01 pixel noise for cfg4), resident in HBM.
     t_setup = time.perf_counter()
-    alm_np = synth.powerlaw_alm(cfg["seed"] + 1000 * rank, lmax, mmax, batch)
+    alm_np = synth.powerlaw_alm(replicas.rank_seed(cfg["seed"], rank), lmax, mmax, batch)
     h_alm = torch.from_numpy(alm_np).to(cdt).pin_memory()
     T = B.Transform(nside, lmax, mmax, batch, rdt, dev)
     stats = B.cuhpx_workspace_stats(T.workspace)
@@ -260,13 +260,10 @@ def main():
     e1.record()
     barrier()
     clocks = sampler.stop()
-    ms = e0.elapsed_time(e1)
-    if world > 1:
-        t = torch.tensor([ms], device=dev)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        ms = float(t.item())
     transforms_per_step = 4 * batch
-    value = world * transforms_per_step * args.steps / (ms * 1e-3)
+    # whole job: every rank's transforms over the slowest rank's device time (no data-path collective)
+    ms, units = replicas.reduce_timing(e0.elapsed_time(e1), transforms_per_step * args.steps, dev)
+    value = units / (ms * 1e-3)
 
     stage_ms = {s: [] for s in stages}
     for name, a, b in ev:
@@ -298,12 +295,8 @@ def main():
         e2e_step()
     b.record()
     barrier()
-    ms_e2e = a.elapsed_time(b)
-    if world > 1:
-        t = torch.tensor([ms_e2e], device=dev)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        ms_e2e = float(t.item())
-    e2e_value = world * transforms_per_step * k_e2e / (ms_e2e * 1e-3)
+    ms_e2e, units_e2e = replicas.reduce_timing(a.elapsed_time(b), transforms_per_step * k_e2e, dev)
+    e2e_value = units_e2e / (ms_e2e * 1e-3)
     map_bytes, alm_bytes = batch * npix * rbytes, batch * nalm * 2 * rbytes
     h2d = 2 * map_bytes + 2 * alm_bytes
     d2h = 2 * map_bytes + 2 * alm_bytes
