@@ -12,10 +12,11 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libcuhpx.so")
 SOURCES = ["plan.cu", "legendre.cu", "ring_fft.cu"]
-HEADERS = [os.path.join(CSRC, "cuhpx_internal.h"), os.path.join(HERE, "..", "include", "cuhpx.h")]
+HEADERS = [os.path.join(CSRC, "cuhpx_internal.h"), os.path.join(CSRC, "block_fft.cuh"),
+           os.path.join(HERE, "..", "include", "cuhpx.h")]
 NVCC_FLAGS = [
     "-O3", "-std=c++17", "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo",
-    "-Xcompiler", "-fPIC", "-shared", "-Xptxas", "-v",
+    "-Xcompiler", "-fPIC", "-Xptxas", "-v",
 ]
 
 
@@ -27,15 +28,39 @@ def needs_build() -> bool:
     return any(os.path.getmtime(d) > t for d in deps)
 
 
+def _compile_one(args):
+    nvcc, src, obj = args
+    cmd = [nvcc] + NVCC_FLAGS + ["-c", "-o", obj, src]
+    res = subprocess.run(cmd, capture_output=True, text=True)
+    return res.returncode, res.stdout + res.stderr
+
+
 def build(force: bool = False, verbose: bool = False) -> str:
-    if force or needs_build():
-        nvcc = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
-        cmd = [nvcc] + NVCC_FLAGS + ["-o", LIB] + [os.path.join(CSRC, s) for s in SOURCES]
-        res = subprocess.run(cmd, capture_output=True, text=True)
-        if verbose or res.returncode != 0:
-            sys.stderr.write(res.stdout + res.stderr)
-        if res.returncode != 0:
-            raise RuntimeError("nvcc failed building libcuhpx.so")
+    """Compile every csrc/*.cu to an object file (in parallel, only the stale ones) and link libcuhpx.so."""
+    if not (force or needs_build()):
+        return LIB
+    from concurrent.futures import ThreadPoolExecutor
+
+    nvcc = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
+    objdir = os.path.join(HERE, "build")
+    os.makedirs(objdir, exist_ok=True)
+    hdr_t = max(os.path.getmtime(h) for h in HEADERS)
+    jobs, objs = [], []
+    for s in SOURCES:
+        src, obj = os.path.join(CSRC, s), os.path.join(objdir, s.replace(".cu", ".o"))
+        objs.append(obj)
+        if force or not os.path.exists(obj) or os.path.getmtime(obj) < max(os.path.getmtime(src), hdr_t):
+            jobs.append((nvcc, src, obj))
+    with ThreadPoolExecutor(max_workers=len(SOURCES)) as ex:
+        for rc, out in ex.map(_compile_one, jobs):
+            if verbose or rc != 0:
+                sys.stderr.write(out)
+            if rc != 0:
+                raise RuntimeError("nvcc failed building libcuhpx.so")
+    res = subprocess.run([nvcc, "-shared", "-o", LIB] + objs, capture_output=True, text=True)
+    if res.returncode != 0:
+        sys.stderr.write(res.stdout + res.stderr)
+        raise RuntimeError("nvcc failed linking libcuhpx.so")
     return LIB
 
 

@@ -2,12 +2,14 @@
 //
 // n = 2^LOGN points are held ENTIRELY in registers (E = n / NT per thread); shared memory is only the exchange
 // buffer between passes.  Each pass is a set of radix-R (R = 2..16) butterflies done in registers with
-// compile-time twiddles; the inter-pass twiddles W_L^(j q) come from a global table (L1/L2 resident).
+// compile-time twiddles; the inter-pass twiddles W_L^(j q) are products of two entries of small shared-memory
+// root tables (Roots: exp(-2 pi i t / Q) = hi[t >> 7] * lo[t & 127]) -- no global-memory latency inside a pass.
 // Decimation in frequency, in place: after the last pass the element at position p is X[bitrev(p)].
 // The inverse runs the same passes backwards (conjugated, decimation in time), so a forward+inverse pair
 // (the Bluestein convolution, Eq. 22) never needs a bit-reversal permutation.
-// Bank conflicts: positions are padded p -> p + (p >> 4) (8-byte) / p + (p >> 5) (4-byte); with the plans
-// below every pass is <= 2 wavefronts per request (measured by brute force).
+// Exchange buffer (Xchg): 8-byte slots at padded positions p -> p + (p >> 4) -- fp64 as split re / im arrays,
+// fp32 as one interleaved float2 array (one 64-bit access per element); with the plans below every pass is
+// <= 2 wavefronts per request (measured by brute force).
 #pragma once
 #include <cuda_runtime.h>
 
@@ -17,8 +19,78 @@ template <typename T> struct V2;
 template <> struct V2<float> { using type = float2; };
 template <> struct V2<double> { using type = double2; };
 
-template <typename T> __device__ __forceinline__ int padi(int p) { return p + (p >> (sizeof(T) == 8 ? 4 : 5)); }
-template <typename T> __host__ __device__ constexpr int padded_len(int n) { return n + (n >> (sizeof(T) == 8 ? 4 : 5)) + 1; }
+__device__ __forceinline__ int padi(int p) { return p + (p >> 4); }
+__host__ __device__ constexpr int padded_len(int n) { return n + (n >> 4) + 1; }
+
+// Exchange buffer of n complex values in shared memory.
+template <typename T> struct Xchg;
+template <> struct Xchg<double> {
+    double* re;
+    double* im;
+    static __host__ __device__ constexpr size_t bytes(int n) { return 2 * (size_t)padded_len(n) * sizeof(double); }
+    __device__ __forceinline__ Xchg(void* base, int n) : re(reinterpret_cast<double*>(base)), im(re + padded_len(n)) {}
+    __device__ __forceinline__ void st(int p, double a, double b) const {
+        const int q = padi(p);
+        re[q] = a;
+        im[q] = b;
+    }
+    __device__ __forceinline__ void ld(int p, double& a, double& b) const {
+        const int q = padi(p);
+        a = re[q];
+        b = im[q];
+    }
+};
+template <> struct Xchg<float> {
+    float2* z;
+    static __host__ __device__ constexpr size_t bytes(int n) { return (size_t)padded_len(n) * sizeof(float2); }
+    __device__ __forceinline__ Xchg(void* base, int) : z(reinterpret_cast<float2*>(base)) {}
+    __device__ __forceinline__ void st(int p, float a, float b) const { z[padi(p)] = make_float2(a, b); }
+    __device__ __forceinline__ void ld(int p, float& a, float& b) const {
+        const float2 v = z[padi(p)];
+        a = v.x;
+        b = v.y;
+    }
+};
+
+// Roots of unity exp(-2 pi i t / Q), 0 <= t < Q, from two shared-memory tables:
+//   lo[k] = exp(-2 pi i k / Q), k < 128;  hi[k] = exp(-2 pi i 128 k / Q), k < ceil(Q / 128).
+constexpr int ROOT_LO = 128;
+__host__ __device__ constexpr int roots_len(int Q) { return ROOT_LO + (Q + ROOT_LO - 1) / ROOT_LO; }
+template <typename T> struct Roots {
+    using T2 = typename V2<T>::type;
+    const T2* lo;
+    const T2* hi;
+    __device__ __forceinline__ Roots(const T2* base) : lo(base), hi(base + ROOT_LO) {}
+    // exp(SIGN * 2 pi i t / Q)
+    template <int SIGN> __device__ __forceinline__ void get(int t, T& c, T& s) const {
+        const T2 a = hi[t >> 7], b = lo[t & (ROOT_LO - 1)];
+        c = a.x * b.x - a.y * b.y;
+        const T v = a.x * b.y + a.y * b.x;
+        s = SIGN > 0 ? -v : v;
+    }
+};
+// fill a root table of power-of-two order Q from the global table tw[k] = exp(-2 pi i k / twlen), Q | twlen
+template <typename T>
+__device__ __forceinline__ void fill_roots_pow2(typename V2<T>::type* base, int Q, const typename V2<T>::type* __restrict__ tw,
+                                                int twlen, int tid, int nt) {
+    const int nhi = Q / ROOT_LO, step = twlen / Q;
+    for (int k = tid; k < ROOT_LO + nhi; k += nt) base[k] = __ldg(tw + (size_t)(k < ROOT_LO ? k : (k - ROOT_LO) * ROOT_LO) * step);
+}
+// fill a root table of arbitrary order Q (sincospi of the exact rational 2 t / Q)
+template <typename T>
+__device__ __forceinline__ void fill_roots_any(typename V2<T>::type* base, int Q, int tid, int nt) {
+    const int nhi = (Q + ROOT_LO - 1) / ROOT_LO;
+    const double inv = 2.0 / (double)Q;
+    for (int k = tid; k < ROOT_LO + nhi; k += nt) {
+        const int t = k < ROOT_LO ? k : (k - ROOT_LO) * ROOT_LO;
+        double sn, cs;
+        sincospi(-(double)t * inv, &sn, &cs);
+        typename V2<T>::type v;
+        v.x = (T)cs;
+        v.y = (T)sn;
+        base[k] = v;
+    }
+}
 
 // radix plans: passes in DIF order
 template <int LOGN> struct FftPlan;
@@ -118,17 +190,16 @@ template <int R> __device__ __forceinline__ constexpr int brev_r(int x) {
     return r;
 }
 
-// Multiply register r (holding butterfly output q = bitrev_R(r)) by w^q, w = tw[idx] (conjugated if CONJ).
-// w^(2^k) are loaded from the table, the other powers are running products (<= 3 multiplies from a table value).
+// Multiply register r (holding butterfly output q = bitrev_R(r)) by w^q, w = exp(-2 pi i t / Q) (conjugated if
+// CONJ).  w^(2^k) come from the root table, the other powers are running products (<= 3 multiplies from a table
+// value).  q t < Q for every q < R.
 template <int R, bool CONJ, typename T>
-__device__ __forceinline__ void apply_twiddles(const typename V2<T>::type* __restrict__ tw, int idx, T* re, T* im) {
+__device__ __forceinline__ void apply_twiddles(const Roots<T>& rt, int t, T* re, T* im) {
     T w1r = 0, w1i = 0, cr = 1, ci = 0;
 #pragma unroll
     for (int q = 1; q < R; ++q) {
-        if ((q & (q - 1)) == 0) {  // power of two: exact table value
-            const typename V2<T>::type w = __ldg(tw + q * idx);
-            cr = w.x;
-            ci = CONJ ? -w.y : w.y;
+        if ((q & (q - 1)) == 0) {  // power of two: table value
+            rt.template get<(CONJ ? +1 : -1)>(q * t, cr, ci);
             if (q == 1) {
                 w1r = cr;
                 w1i = ci;
@@ -145,13 +216,14 @@ __device__ __forceinline__ void apply_twiddles(const typename V2<T>::type* __res
     }
 }
 
-template <typename T, int LOGN> struct BlockFFT {
+// LOGQ: log2 of the order of the root table handed to forward / inverse (LOGQ >= LOGN)
+template <typename T, int LOGN, int LOGQ = LOGN> struct BlockFFT {
     using P = FftPlan<LOGN>;
     using T2 = typename V2<T>::type;
     static constexpr int N = 1 << LOGN, NT = P::NT, E = N / NT, NP = P::NP;
     static constexpr int RLAST = PassRadix<LOGN, NP - 1>::value;
     static constexpr int R0 = P::R0;
-    static constexpr size_t SMEM_BYTES = 2 * (size_t)padded_len<T>(N) * sizeof(T);
+    static constexpr size_t SMEM_BYTES = Xchg<T>::bytes(N);
 
     // position of register e = c R + rho in pass S
     template <int S> static __device__ __forceinline__ int pos(int tid, int c, int rho) {
@@ -168,91 +240,77 @@ template <typename T, int LOGN> struct BlockFFT {
         return (int)(__brev((unsigned)p) >> (32 - LOGN));
     }
 
-    template <int S> static __device__ __forceinline__ void load(T (&re)[E], T (&im)[E], const T* sre, const T* sim, int tid) {
+    template <int S> static __device__ __forceinline__ void load(T (&re)[E], T (&im)[E], const Xchg<T>& x, int tid) {
         constexpr int R = PassRadix<LOGN, S>::value;
 #pragma unroll
         for (int c = 0; c < E / R; ++c)
 #pragma unroll
-            for (int r = 0; r < R; ++r) {
-                const int p = padi<T>(pos<S>(tid, c, r));
-                re[c * R + r] = sre[p];
-                im[c * R + r] = sim[p];
-            }
+            for (int r = 0; r < R; ++r) x.ld(pos<S>(tid, c, r), re[c * R + r], im[c * R + r]);
     }
-    template <int S> static __device__ __forceinline__ void store(const T (&re)[E], const T (&im)[E], T* sre, T* sim, int tid) {
+    template <int S> static __device__ __forceinline__ void store(const T (&re)[E], const T (&im)[E], const Xchg<T>& x, int tid) {
         constexpr int R = PassRadix<LOGN, S>::value;
 #pragma unroll
         for (int c = 0; c < E / R; ++c)
 #pragma unroll
-            for (int r = 0; r < R; ++r) {
-                const int p = padi<T>(pos<S>(tid, c, r));
-                sre[p] = re[c * R + r];
-                sim[p] = im[c * R + r];
-            }
+            for (int r = 0; r < R; ++r) x.st(pos<S>(tid, c, r), re[c * R + r], im[c * R + r]);
     }
 
-    template <int S> static __device__ __forceinline__ void fwd_pass(T (&re)[E], T (&im)[E], T* sre, T* sim,
-                                                                  const T2* __restrict__ tw, int twlen, int tid) {
+    template <int S> static __device__ __forceinline__ void fwd_pass(T (&re)[E], T (&im)[E], const Xchg<T>& x,
+                                                                  const Roots<T>& rt, int tid) {
         if constexpr (S < NP) {
             constexpr int R = PassRadix<LOGN, S>::value, L = PassLen<LOGN, S>::value, LR = L / R;
             if constexpr (S > 0) {
                 __syncthreads();
-                load<S>(re, im, sre, sim, tid);
+                load<S>(re, im, x, tid);
             }
 #pragma unroll
             for (int c = 0; c < E / R; ++c) {
                 RegDif<R, -1, T>::run(re + c * R, im + c * R);
                 if constexpr (LR > 1) {
                     const int j = (tid + NT * c) % LR;
-                    apply_twiddles<R, false, T>(tw, j * (twlen / L), re + c * R, im + c * R);
+                    apply_twiddles<R, false, T>(rt, j * ((1 << LOGQ) / L), re + c * R, im + c * R);
                 }
             }
-            if constexpr (S < NP - 1) store<S>(re, im, sre, sim, tid);
-            fwd_pass<S + 1>(re, im, sre, sim, tw, twlen, tid);
+            if constexpr (S < NP - 1) store<S>(re, im, x, tid);
+            fwd_pass<S + 1>(re, im, x, rt, tid);
         }
     }
 
-    template <int S> static __device__ __forceinline__ void inv_pass(T (&re)[E], T (&im)[E], T* sre, T* sim,
-                                                                  const T2* __restrict__ tw, int twlen, int tid) {
+    template <int S> static __device__ __forceinline__ void inv_pass(T (&re)[E], T (&im)[E], const Xchg<T>& x,
+                                                                  const Roots<T>& rt, int tid) {
         if constexpr (S >= 0) {
             constexpr int R = PassRadix<LOGN, S>::value, L = PassLen<LOGN, S>::value, LR = L / R;
             if constexpr (S < NP - 1) {
                 __syncthreads();
-                load<S>(re, im, sre, sim, tid);
+                load<S>(re, im, x, tid);
             }
 #pragma unroll
             for (int c = 0; c < E / R; ++c) {
                 if constexpr (LR > 1) {
                     const int j = (tid + NT * c) % LR;
-                    apply_twiddles<R, true, T>(tw, j * (twlen / L), re + c * R, im + c * R);
+                    apply_twiddles<R, true, T>(rt, j * ((1 << LOGQ) / L), re + c * R, im + c * R);
                 }
                 RegDit<R, +1, T>::run(re + c * R, im + c * R);
             }
-            if constexpr (S > 0) store<S>(re, im, sre, sim, tid);
-            inv_pass<S - 1>(re, im, sre, sim, tw, twlen, tid);
+            if constexpr (S > 0) store<S>(re, im, x, tid);
+            inv_pass<S - 1>(re, im, x, rt, tid);
         }
     }
 
     // forward DFT (exp(-i...)): registers in pass-0 layout -> registers in last-pass layout (freq_index)
-    static __device__ __forceinline__ void forward(T (&re)[E], T (&im)[E], T* sre, T* sim, const T2* __restrict__ tw,
-                                                   int twlen, int tid) {
-        fwd_pass<0>(re, im, sre, sim, tw, twlen, tid);
+    static __device__ __forceinline__ void forward(T (&re)[E], T (&im)[E], const Xchg<T>& x, const Roots<T>& rt, int tid) {
+        fwd_pass<0>(re, im, x, rt, tid);
     }
     // unnormalised inverse (exp(+i...), factor n): last-pass layout -> pass-0 layout
-    static __device__ __forceinline__ void inverse(T (&re)[E], T (&im)[E], T* sre, T* sim, const T2* __restrict__ tw,
-                                                   int twlen, int tid) {
-        inv_pass<NP - 1>(re, im, sre, sim, tw, twlen, tid);
+    static __device__ __forceinline__ void inverse(T (&re)[E], T (&im)[E], const Xchg<T>& x, const Roots<T>& rt, int tid) {
+        inv_pass<NP - 1>(re, im, x, rt, tid);
     }
     // write the forward result to shared memory in natural frequency order (call after forward; syncs first,
     // because other threads may still be reading the exchange buffer; caller syncs before reading)
-    static __device__ __forceinline__ void store_natural(const T (&re)[E], const T (&im)[E], T* sre, T* sim, int tid) {
+    static __device__ __forceinline__ void store_natural(const T (&re)[E], const T (&im)[E], const Xchg<T>& x, int tid) {
         __syncthreads();
 #pragma unroll
-        for (int e = 0; e < E; ++e) {
-            const int p = padi<T>(freq_index(tid, e));
-            sre[p] = re[e];
-            sim[p] = im[e];
-        }
+        for (int e = 0; e < E; ++e) x.st(freq_index(tid, e), re[e], im[e]);
     }
 };
 

@@ -288,13 +288,27 @@ __global__ void __launch_bounds__(NT, 512 / NT >= 3 ? 3 : 2) legendre_analysis_k
     const int nl = P.lmax - m + 1;  // l values of this m
     bool warp_active = __any_sync(0xffffffffu, nact > 0);
     int buf = 0;
+    // alpha of the steps that produce degrees l = m + t0 + 1 + i; the next tile is fetched into a register while
+    // the current one is consumed, so no global-load latency sits between two tiles
+    double nextA = (tid < CT && 1 + tid < nl) ? P.coef_alpha[abase + m + 1 + tid] : 0.0;
+    constexpr int NOUT = (TPG * NV + NT - 1) / NT;  // output elements per thread and group (cross-warp sums)
     for (int t0 = 0; t0 < nl; t0 += CT) {
-        // alpha of the steps that produce degrees l = m + t0 + 1 + i
         const int cb = (t0 / CT) & 1;
-        if (tid < CT) sA[cb][tid] = (t0 + 1 + tid < nl) ? P.coef_alpha[abase + m + t0 + 1 + tid] : 0.0;
+        if (tid < CT) {
+            sA[cb][tid] = nextA;
+            nextA = (t0 + CT + 1 + tid < nl) ? P.coef_alpha[abase + m + t0 + CT + 1 + tid] : 0.0;
+        }
         __syncthreads();
         const int tend = min(CT, nl - t0);
         for (int g0 = 0; g0 < tend; g0 += GROUP_L) {
+            // s_l of this thread's output element, requested before the group's arithmetic
+            double oscl[NOUT];
+#pragma unroll
+            for (int q = 0; q < NOUT; ++q) {
+                const int e = tid + NT * q;
+                const int k = t0 + g0 + (e / NV) * LT + (e % NV) / (BT * 2);
+                oscl[q] = (e < TPG * NV && k < nl) ? outscale * P.coef_scale[abase + m + k] : 0.0;
+            }
 #pragma unroll 1
             for (int ti = 0; ti < TPG; ++ti) {
                 const int s0 = g0 + ti * LT;
@@ -361,7 +375,10 @@ __global__ void __launch_bounds__(NT, 512 / NT >= 3 ? 3 : 2) legendre_analysis_k
                 }
             }
             __syncthreads();
-            for (int e = tid; e < TPG * NV; e += NT) {
+#pragma unroll
+            for (int q = 0; q < NOUT; ++q) {
+                const int e = tid + NT * q;
+                if (e >= TPG * NV) break;
                 const int ti = e / NV, v = e % NV;
                 T sum = 0;
 #pragma unroll
@@ -370,7 +387,7 @@ __global__ void __launch_bounds__(NT, 512 / NT >= 3 ? 3 : 2) legendre_analysis_k
                 const int k = t0 + g0 + ti * LT + i;  // l - m
                 const int ch = ch0 + c;
                 if (k < nl && ch < P.batch) {
-                    T o = (T)(outscale * P.coef_scale[abase + m + k] * (double)sum);  // lambda = s_l mu
+                    T o = (T)(oscl[q] * (double)sum);  // lambda = s_l mu
                     if (m == 0 && ri == 1) o = 0;  // Im a_l0 is exactly zero
                     out[((size_t)ch * P.nalm + abase + m + k) * 2 + ri] = o;
                 }
@@ -595,21 +612,39 @@ __global__ void __launch_bounds__(NT) legendre_synthesis_kernel(LegArgs a) {
     const T* alm = reinterpret_cast<const T*>(a.in);
     const int nl = P.lmax - m + 1;
 
+    // Tile t0 + CT is fetched into registers while tile t0 is consumed (no global-load latency between tiles).
+    constexpr int NP = (CT * BT * 2 + NT - 1) / NT;
+    double nA = 0.0, nScl[NP];
+    T nAlm[NP];
+    auto fetch = [&](int tn) {
+        nA = (tid < CT && tn + 1 + tid < nl) ? P.coef_alpha[abase + m + tn + 1 + tid] : 0.0;
+#pragma unroll
+        for (int q = 0; q < NP; ++q) {
+            const int e = tid + NT * q;
+            const int i = e / (BT * 2), c = (e / 2) % BT, ri = e & 1;
+            const int k = tn + i, ch = ch0 + c;
+            const bool ok = e < CT * BT * 2 && k < nl && ch < P.batch;
+            nScl[q] = ok ? P.coef_scale[abase + m + k] : 0.0;
+            nAlm[q] = ok ? alm[((size_t)ch * P.nalm + abase + m + k) * 2 + ri] : (T)0;
+        }
+    };
+    fetch(0);
     for (int t0 = 0; t0 < nl; t0 += CT) {
         __syncthreads();  // previous tile fully consumed
-        if (tid < CT) sA[tid] = (t0 + 1 + tid < nl) ? P.coef_alpha[abase + m + t0 + 1 + tid] : 0.0;
-        for (int e = tid; e < CT * BT * 2; e += NT) {
-            const int i = e / (BT * 2), c = (e / 2) % BT, ri = e & 1;
-            const int k = t0 + i;
-            const int ch = ch0 + c;
-            T v = 0;
-            if (k < nl && ch < P.batch)  // a_lm s_l: the kernel sums mu_l = lambda_l / s_l
-                v = (T)((double)inscale * P.coef_scale[abase + m + k] *
-                        (double)alm[((size_t)ch * P.nalm + abase + m + k) * 2 + ri]);
-            if (m == 0 && ri == 1) v = 0;  // Im a_l0 is ignored
-            sAlm[i][c][ri] = v;
+        if (tid < CT) sA[tid] = nA;
+#pragma unroll
+        for (int q = 0; q < NP; ++q) {
+            const int e = tid + NT * q;
+            if (e < CT * BT * 2) {
+                const int i = e / (BT * 2), c = (e / 2) % BT, ri = e & 1;
+                // a_lm s_l: the kernel sums mu_l = lambda_l / s_l
+                T v = (T)((double)inscale * nScl[q] * (double)nAlm[q]);
+                if (m == 0 && ri == 1) v = 0;  // Im a_l0 is ignored
+                sAlm[i][c][ri] = v;
+            }
         }
         __syncthreads();
+        fetch(t0 + CT);
         const int tend = min(CT, nl - t0);
         for (int s0 = 0; s0 < tend; s0 += CHECK_EVERY) {
             bool any = false;

@@ -14,6 +14,7 @@
 // One CTA per (ring, channel); rings are read and spectra written exactly once, coalesced.
 #include <cuda_runtime.h>
 #include <math.h>
+#include <string.h>
 
 #include <algorithm>
 
@@ -26,32 +27,54 @@ constexpr int DIRECT_MAX_N = 256;
 constexpr int FFT_THREADS = 256;  // direct kernels
 constexpr int MIN_LOG = 8, MAX_LOG = 13;
 
-// exp(sign * i * pi * num / den) from exact integers (num already reduced mod 2 den)
+// exp(sign * i * pi * num / den) from exact integers (num already reduced mod 2 den); direct kernels only
 __device__ __forceinline__ void cispi_ratio(long long num, long long den, double sign, double& c, double& s) {
     sincospi((double)num / (double)den, &s, &c);
     s *= sign;
 }
 __device__ __forceinline__ void cispi_ratio(long long num, long long den, float sign, float& c, float& s) {
-    sincospif((float)((double)num / (double)den), &s, &c);
+    sincospif((float)num / (float)den, &s, &c);  // num < 2 den <= 512: exact integers, one rounding
     s *= sign;
 }
 
-struct RingRef {
-    int N, mcut, shifted;
-    long long start;
-    double weight;
+// One work item of an FFT-stage launch: everything a CTA needs to know about its ring, in one 32-byte record
+// (built per plan on the host; replaces four dependent table look-ups).
+struct __align__(16) RingInfo {
+    long long start;  // RING index of the ring's first pixel
+    int N;            // pixels in the ring
+    int mcut;         // largest order kept on this ring
+    int shifted;      // 1: phi0 = pi / N, 0: phi0 = 0
+    int r;            // 0-based ring number, north to south
+    int pad0, pad1;
 };
+static_assert(sizeof(RingInfo) == 32, "RingInfo layout");
 
-__device__ __forceinline__ RingRef ring_ref(const DevPlan& P, int r, const double* w, int use_w) {
-    RingRef R;
-    const int j = min(r, P.nrings - 1 - r);
-    R.N = P.ringN[j];
-    R.mcut = P.mcut[j];
-    R.shifted = P.shifted[j];
-    R.start = (r > j) ? P.npix - R.N - P.start[j] : P.start[j];
-    R.weight = 1.0;
-    if (use_w) R.weight = w ? w[r] : 4.0 * 3.14159265358979323846 / (double)P.npix;
+__device__ __forceinline__ RingInfo load_info(const RingInfo* __restrict__ info, int idx) {
+    const int4 a = __ldg(reinterpret_cast<const int4*>(info + idx));
+    const int4 b = __ldg(reinterpret_cast<const int4*>(info + idx) + 1);
+    RingInfo R;
+    R.start = (long long)(((unsigned long long)(unsigned)a.y << 32) | (unsigned)a.x);
+    R.N = a.z;
+    R.mcut = a.w;
+    R.shifted = b.x;
+    R.r = b.y;
     return R;
+}
+
+__device__ __forceinline__ double ring_weight(const DevPlan& P, const RingInfo& R, const double* __restrict__ w, int use_w) {
+    if (!use_w) return 1.0;
+    return w ? __ldg(w + R.r) : 4.0 * 3.14159265358979323846 / (double)P.npix;
+}
+
+// Ask the memory system to bring `bytes` at `ptr` into L2 (no register or shared-memory destination): issued
+// for the work item the SM will run next, so its HBM traffic overlaps the current item's arithmetic.
+__device__ __forceinline__ void prefetch_l2(const void* ptr, unsigned bytes) {
+    constexpr unsigned CHUNK = 16384;
+    const char* p = reinterpret_cast<const char*>(ptr);
+    for (unsigned o = (threadIdx.x & 31) * CHUNK; o < bytes; o += 32 * CHUNK) {
+        const unsigned n = min(CHUNK, bytes - o) & ~15u;
+        if (n) asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" ::"l"(p + o), "r"(n) : "memory");
+    }
 }
 
 struct FftTables {
@@ -59,18 +82,40 @@ struct FftTables {
     int twlen;
     const void* filt;             // Bluestein filter spectra, register order, concatenated
     const long long* filt_offset; // [nside] offset (complex units) for cap ring i, -1 if none
+    int pf;                       // prefetch distance in work items (CTAs resident on the GPU at once)
 };
+
+// work item of this CTA and L2 prefetch of the item `pf` launches ahead (grid = (items, channels), x fastest)
+template <typename T, bool ANALYSIS>
+__device__ __forceinline__ RingInfo begin_item(const DevPlan& P, const RingInfo* __restrict__ info, const T* map, int pf) {
+    const RingInfo R = load_info(info, blockIdx.x);
+    if (threadIdx.x < 32 && pf > 0) {
+        const long long lin = (long long)blockIdx.y * gridDim.x + blockIdx.x + pf;
+        if (lin < (long long)gridDim.x * gridDim.y) {
+            const int nx = (int)(lin % gridDim.x), nch = (int)(lin / gridDim.x);
+            const RingInfo Rn = load_info(info, nx);
+            if (ANALYSIS) {
+                prefetch_l2(map + (size_t)nch * P.npix + Rn.start, (unsigned)(Rn.N * sizeof(T)));
+            } else {
+                using T2 = typename V2<T>::type;
+                const T2* row = reinterpret_cast<const T2*>(P.spectra) + ((size_t)nch * P.nrings + Rn.r) * P.mstride;
+                prefetch_l2(row, (unsigned)(((Rn.mcut + 1) * sizeof(T2) + 15) & ~15u));
+            }
+        }
+    }
+    return R;
+}
 
 // ------------------------------------------------------------------ direct kernels (short rings)
 template <typename T>
-__global__ void __launch_bounds__(FFT_THREADS) ring_direct_analysis_kernel(DevPlan P, const int* __restrict__ rings,
+__global__ void __launch_bounds__(FFT_THREADS) ring_direct_analysis_kernel(DevPlan P, const RingInfo* __restrict__ info,
                                                                           const T* __restrict__ map,
                                                                           const double* __restrict__ w, int use_w) {
     using T2 = typename V2<T>::type;
     extern __shared__ __align__(16) unsigned char smem_raw[];
-    const int r = rings[blockIdx.x], ch = blockIdx.y;
-    const RingRef R = ring_ref(P, r, w, use_w);
-    const int N = R.N;
+    const int ch = blockIdx.y;
+    const RingInfo R = load_info(info, blockIdx.x);
+    const int N = R.N, r = R.r;
     T2* tw = reinterpret_cast<T2*>(smem_raw);
     T* p = reinterpret_cast<T*>(tw + N);
     const T* src = map + (size_t)ch * P.npix + R.start;
@@ -83,6 +128,7 @@ __global__ void __launch_bounds__(FFT_THREADS) ring_direct_analysis_kernel(DevPl
     }
     __syncthreads();
     T2* dst = reinterpret_cast<T2*>(P.spectra) + ((size_t)ch * P.nrings + r) * P.mstride;
+    const T wt = (T)ring_weight(P, R, w, use_w);
     for (int m = threadIdx.x; m <= R.mcut; m += blockDim.x) {
         const int step = m % N;
         int idx = 0;
@@ -95,7 +141,6 @@ __global__ void __launch_bounds__(FFT_THREADS) ring_direct_analysis_kernel(DevPl
         }
         T c = 1, s = 0;
         if (R.shifted) cispi_ratio((long long)(m % (2 * N)), N, (T)-1, c, s);
-        const T wt = (T)R.weight;
         T2 o;
         o.x = wt * (ar * c - ai * s);
         o.y = wt * (ar * s + ai * c);
@@ -104,14 +149,14 @@ __global__ void __launch_bounds__(FFT_THREADS) ring_direct_analysis_kernel(DevPl
 }
 
 template <typename T>
-__global__ void __launch_bounds__(FFT_THREADS) ring_direct_synthesis_kernel(DevPlan P, const int* __restrict__ rings,
+__global__ void __launch_bounds__(FFT_THREADS) ring_direct_synthesis_kernel(DevPlan P, const RingInfo* __restrict__ info,
                                                                            T* __restrict__ map,
                                                                            const double* __restrict__ w, int use_w) {
     using T2 = typename V2<T>::type;
     extern __shared__ __align__(16) unsigned char smem_raw[];
-    const int r = rings[blockIdx.x], ch = blockIdx.y;
-    const RingRef R = ring_ref(P, r, w, use_w);
-    const int N = R.N;
+    const int ch = blockIdx.y;
+    const RingInfo R = load_info(info, blockIdx.x);
+    const int N = R.N, r = R.r;
     T2* tw = reinterpret_cast<T2*>(smem_raw);
     T2* G = tw + N;
     const T2* src = reinterpret_cast<const T2*>(P.spectra) + ((size_t)ch * P.nrings + r) * P.mstride;
@@ -134,6 +179,7 @@ __global__ void __launch_bounds__(FFT_THREADS) ring_direct_synthesis_kernel(DevP
     }
     __syncthreads();
     T* dst = map + (size_t)ch * P.npix + R.start;
+    const T wt = (T)ring_weight(P, R, w, use_w);
     for (int x = threadIdx.x; x < N; x += blockDim.x) {
         T acc = 0;
         int idx = 0;
@@ -143,36 +189,22 @@ __global__ void __launch_bounds__(FFT_THREADS) ring_direct_synthesis_kernel(DevP
             acc = fma(G[m].x, tw[idx].x, acc);
             acc = fma(-G[m].y, tw[idx].y, acc);
         }
-        dst[x] = (T)R.weight * (G[0].x + 2 * acc);
+        dst[x] = wt * (G[0].x + 2 * acc);
     }
 }
 
 // ------------------------------------------------------------------ shared pieces of the FFT kernels
-
-// exp(-+ i pi num / den) for the FFT kernels: POW2 rings read the twiddle table (den | twlen/2... exact integer
-// index), other rings evaluate sincospi of the exact rational.
-template <typename T, bool POW2> struct Cis {
-    using T2 = typename V2<T>::type;
-    const T2* tw;
-    int twlen;
-    // exp(SIGN * 2 pi i * num / den), 0 <= num < den
-    template <int SIGN> __device__ __forceinline__ void get(int num, int den, T& c, T& s) const {
-        if (POW2) {
-            const T2 w = __ldg(tw + (size_t)num * (twlen / den));
-            c = w.x;
-            s = SIGN > 0 ? -w.y : w.y;
-        } else {
-            cispi_ratio(2LL * num, den, (T)SIGN, c, s);
-        }
-    }
-};
+// Every phase factor of a ring of N pixels is a power of omega = exp(-2 pi i / Q), Q = 2 N:
+//   twist exp(-i m phi0) = omega^m (phi0 = pi / N),  W_N^k = omega^(2 k),  W_{N/2}^k = omega^(4 k).
+// `rt` is the shared-memory root table of order Q (block_fft.cuh).
+template <bool POW2> __device__ __forceinline__ int mod_q(int m, int Q) { return POW2 ? (m & (Q - 1)) : (m % Q); }
 
 // Folded half spectrum H[k], k = 0..n (n = N/2), of the synthesis input:
 //   c_m = G_m exp(+i m phi0);  0 < k < n: H[k] = sum_{m = k (N)} c_m + sum_{m = -k (N)} conj(c_m);
 //   k in {0, n}: H[k] = sum_{m = k (N)} (m == 0 ? Re c_0 : 2 Re c_m)
 template <typename T, bool POW2>
 __device__ __forceinline__ void folded_H(const typename V2<T>::type* __restrict__ G, int k, int N, int mcut, int shifted,
-                                         const Cis<T, POW2>& cis, T& hr, T& hi) {
+                                         const Roots<T>& rt, T& hr, T& hi) {
     using T2 = typename V2<T>::type;
     const int n = N >> 1;
     hr = 0;
@@ -181,7 +213,7 @@ __device__ __forceinline__ void folded_H(const typename V2<T>::type* __restrict_
         const T2 g = G[m];
         if (shifted) {
             T c, s;
-            cis.template get<+1>(m % (2 * N), 2 * N, c, s);
+            rt.template get<+1>(mod_q<POW2>(m, 2 * N), c, s);
             cr = g.x * c - g.y * s;
             ci = g.x * s + g.y * c;
         } else {
@@ -215,15 +247,15 @@ __device__ __forceinline__ void folded_H(const typename V2<T>::type* __restrict_
 // O' = (H[k] - conj H[n-k]) exp(+2 pi i k / N); the ring is then x[2t] = Re D[t], x[2t+1] = -Im D[t], D = DFT_n(Y).
 template <typename T, bool POW2>
 __device__ __forceinline__ void synth_packed_input(const typename V2<T>::type* __restrict__ G, int k, int N, int mcut,
-                                                   int shifted, const Cis<T, POW2>& cis, T& yr, T& yi) {
+                                                   int shifted, const Roots<T>& rt, T& yr, T& yi) {
     using T2 = typename V2<T>::type;
     const int n = N >> 1;
     T ar, ai, br, bi, c, s;
     if (mcut < n) {
         // no order reaches the Nyquist bin: H[k] = G_k e^{i k phi0} for k <= mcut, else 0.  With p = e^{i pi k / N}:
-        // twist of bin k is p, of bin n - k is i conj(p), and e^{2 pi i k / N} = p^2: one sincos per element.
+        // twist of bin k is p, of bin n - k is i conj(p), and e^{2 pi i k / N} = p^2: one root per element.
         T pc, ps;
-        cis.template get<+1>(k, 2 * N, pc, ps);
+        rt.template get<+1>(k, pc, ps);
         T2 a, b;
         a.x = a.y = b.x = b.y = 0;
         if (k <= mcut) a = G[k];
@@ -240,9 +272,9 @@ __device__ __forceinline__ void synth_packed_input(const typename V2<T>::type* _
         c = pc * pc - ps * ps;
         s = 2 * pc * ps;
     } else {
-        folded_H<T, POW2>(G, k, N, mcut, shifted, cis, ar, ai);
-        folded_H<T, POW2>(G, n - k, N, mcut, shifted, cis, br, bi);
-        cis.template get<+1>(k, N, c, s);
+        folded_H<T, POW2>(G, k, N, mcut, shifted, rt, ar, ai);
+        folded_H<T, POW2>(G, n - k, N, mcut, shifted, rt, br, bi);
+        rt.template get<+1>(2 * k, c, s);
     }
     bi = -bi;  // conj H[n-k]
     const T er = ar + br, ei = ai + bi;
@@ -254,21 +286,26 @@ __device__ __forceinline__ void synth_packed_input(const typename V2<T>::type* _
 }
 
 // Hermitian unpack of the packed analysis FFT + twist: given Z[kk mod n] and Z[(n-kk) mod n] returns
-// F_m = weight * exp(-i m phi0) * X~[m mod N]
+// F_m = weight * exp(-i m phi0) * X~[m mod N]  (k = m mod N, kk = min(k, N - k), cj = k > n)
 template <typename T, bool POW2>
 __device__ __forceinline__ typename V2<T>::type analysis_unpack(T z1r, T z1i, T z2r, T z2i, int m, int kk, bool cj, int N,
-                                                                 int shifted, T wt, const Cis<T, POW2>& cis) {
+                                                                 int shifted, T wt, const Roots<T>& rt) {
     const T er = (T)0.5 * (z1r + z2r), ei = (T)0.5 * (z1i - z2i);
     const T dr = (T)0.5 * (z1r - z2r), di = (T)0.5 * (z1i + z2i);
-    // O = -i D = (di, -dr);  X = E + W_N^kk O
-    T c, s;
-    cis.template get<-1>(kk, N, c, s);
+    // O = -i D = (di, -dr);  X = E + W_N^kk O.  Unaliased (kk == m): W_N^kk = omega^(2 m) is the square of the twist.
+    T pc, ps, c, s;
+    const bool plain = (kk == m);
+    rt.template get<-1>(plain ? m : mod_q<POW2>(m, 2 * N), pc, ps);  // twist omega^m
+    if (plain) {
+        c = pc * pc - ps * ps;
+        s = 2 * pc * ps;
+    } else {
+        rt.template get<-1>(2 * kk, c, s);
+    }
     T xr = er + (c * di + s * dr);
     T xi = ei + (s * di - c * dr);
     if (cj) xi = -xi;
     if (shifted) {
-        T pc, ps;
-        cis.template get<-1>(m % (2 * N), 2 * N, pc, ps);
         const T tr = xr * pc - xi * ps, ti = xr * ps + xi * pc;
         xr = tr;
         xi = ti;
@@ -280,22 +317,22 @@ __device__ __forceinline__ typename V2<T>::type analysis_unpack(T z1r, T z1i, T 
 }
 
 // ------------------------------------------------------------------ power-of-two rings
+// shared memory: [exchange buffer of n complex][root table of order Q = 2 N = 4 n]
 template <typename T, int LOGN>
-__global__ void __launch_bounds__(FftPlan<LOGN>::NT) ring_pow2_analysis_kernel(DevPlan P, const int* __restrict__ rings,
+__global__ void __launch_bounds__(FftPlan<LOGN>::NT) ring_pow2_analysis_kernel(DevPlan P, const RingInfo* __restrict__ info,
                                                                                const T* __restrict__ map,
                                                                                const double* __restrict__ w, int use_w,
                                                                                FftTables tabs) {
-    using F = BlockFFT<T, LOGN>;
+    using F = BlockFFT<T, LOGN, LOGN + 2>;
     using T2 = typename V2<T>::type;
-    constexpr int n = F::N, N = 2 * n, E = F::E, NT = F::NT;
+    constexpr int n = F::N, N = 2 * n, Q = 2 * N, E = F::E, NT = F::NT;
     extern __shared__ __align__(16) unsigned char smem_raw[];
-    T* sre = reinterpret_cast<T*>(smem_raw);
-    T* sim = sre + padded_len<T>(n);
+    const Xchg<T> xs(smem_raw, n);
+    T2* rbase = reinterpret_cast<T2*>(smem_raw + Xchg<T>::bytes(n));
     const int tid = threadIdx.x;
-    const int r = rings[blockIdx.x], ch = blockIdx.y;
-    const RingRef R = ring_ref(P, r, w, use_w);
+    const int ch = blockIdx.y;
+    const RingInfo R = begin_item<T, true>(P, info, map, tabs.pf);
     const T2* src = reinterpret_cast<const T2*>(map + (size_t)ch * P.npix + R.start);
-    const T2* tw = reinterpret_cast<const T2*>(tabs.tw);
     T re[E], im[E];
 #pragma unroll
     for (int e = 0; e < E; ++e) {
@@ -303,69 +340,81 @@ __global__ void __launch_bounds__(FftPlan<LOGN>::NT) ring_pow2_analysis_kernel(D
         re[e] = z.x;
         im[e] = z.y;
     }
-    F::forward(re, im, sre, sim, tw, tabs.twlen, tid);
-    F::store_natural(re, im, sre, sim, tid);
+    fill_roots_pow2<T>(rbase, Q, reinterpret_cast<const T2*>(tabs.tw), tabs.twlen, tid, NT);
+    const T wt = (T)ring_weight(P, R, w, use_w);
     __syncthreads();
-    const Cis<T, true> cis{tw, tabs.twlen};
-    T2* dst = reinterpret_cast<T2*>(P.spectra) + ((size_t)ch * P.nrings + r) * P.mstride;
-    const T wt = (T)R.weight;
+    const Roots<T> rt(rbase);
+    F::forward(re, im, xs, rt, tid);
+    F::store_natural(re, im, xs, tid);
+    __syncthreads();
+    T2* dst = reinterpret_cast<T2*>(P.spectra) + ((size_t)ch * P.nrings + R.r) * P.mstride;
     for (int m = tid; m <= R.mcut; m += NT) {
         const int k = m & (N - 1);
         const bool cj = k > n;
         const int kk = cj ? N - k : k;
-        const int i1 = padi<T>(kk & (n - 1)), i2 = padi<T>((n - kk) & (n - 1));
-        dst[m] = analysis_unpack<T, true>(sre[i1], sim[i1], sre[i2], sim[i2], m, kk, cj, N, R.shifted, wt, cis);
+        T z1r, z1i, z2r, z2i;
+        xs.ld(kk & (n - 1), z1r, z1i);
+        xs.ld((n - kk) & (n - 1), z2r, z2i);
+        dst[m] = analysis_unpack<T, true>(z1r, z1i, z2r, z2i, m, kk, cj, N, R.shifted, wt, rt);
     }
 }
 
 template <typename T, int LOGN>
-__global__ void __launch_bounds__(FftPlan<LOGN>::NT) ring_pow2_synthesis_kernel(DevPlan P, const int* __restrict__ rings,
+__global__ void __launch_bounds__(FftPlan<LOGN>::NT) ring_pow2_synthesis_kernel(DevPlan P, const RingInfo* __restrict__ info,
                                                                                 T* __restrict__ map,
                                                                                 const double* __restrict__ w, int use_w,
                                                                                 FftTables tabs) {
-    using F = BlockFFT<T, LOGN>;
+    using F = BlockFFT<T, LOGN, LOGN + 2>;
     using T2 = typename V2<T>::type;
-    constexpr int n = F::N, N = 2 * n, E = F::E, NT = F::NT;
+    constexpr int n = F::N, N = 2 * n, Q = 2 * N, E = F::E, NT = F::NT;
     extern __shared__ __align__(16) unsigned char smem_raw[];
-    T* sre = reinterpret_cast<T*>(smem_raw);
-    T* sim = sre + padded_len<T>(n);
+    const Xchg<T> xs(smem_raw, n);
+    T2* rbase = reinterpret_cast<T2*>(smem_raw + Xchg<T>::bytes(n));
     const int tid = threadIdx.x;
-    const int r = rings[blockIdx.x], ch = blockIdx.y;
-    const RingRef R = ring_ref(P, r, w, use_w);
-    const T2* tw = reinterpret_cast<const T2*>(tabs.tw);
-    const Cis<T, true> cis{tw, tabs.twlen};
-    const T2* G = reinterpret_cast<const T2*>(P.spectra) + ((size_t)ch * P.nrings + r) * P.mstride;
+    const int ch = blockIdx.y;
+    const RingInfo R = begin_item<T, false>(P, info, map, tabs.pf);
+    fill_roots_pow2<T>(rbase, Q, reinterpret_cast<const T2*>(tabs.tw), tabs.twlen, tid, NT);
+    const T wt = (T)ring_weight(P, R, w, use_w);
+    __syncthreads();
+    const Roots<T> rt(rbase);
+    const T2* G = reinterpret_cast<const T2*>(P.spectra) + ((size_t)ch * P.nrings + R.r) * P.mstride;
     T re[E], im[E];
 #pragma unroll
     for (int e = 0; e < E; ++e)
-        synth_packed_input<T, true>(G, F::index0(tid, e), N, R.mcut, R.shifted, cis, re[e], im[e]);
-    F::forward(re, im, sre, sim, tw, tabs.twlen, tid);
-    F::store_natural(re, im, sre, sim, tid);
+        synth_packed_input<T, true>(G, F::index0(tid, e), N, R.mcut, R.shifted, rt, re[e], im[e]);
+    F::forward(re, im, xs, rt, tid);
+    F::store_natural(re, im, xs, tid);
     __syncthreads();
     T2* dst = reinterpret_cast<T2*>(map + (size_t)ch * P.npix + R.start);
-    const T wt = (T)R.weight;
     for (int t = tid; t < n; t += NT) {
+        T a, b;
+        xs.ld(t, a, b);
         T2 o;
-        o.x = wt * sre[padi<T>(t)];
-        o.y = -wt * sim[padi<T>(t)];
+        o.x = wt * a;
+        o.y = -wt * b;
         dst[t] = o;
     }
 }
 
 // ------------------------------------------------------------------ Bluestein rings (N = 4 i, i not a power of two)
-// chirp c[u] = exp(-i pi u^2 / i) from the exact integer u^2 mod 2i  (Eq. 19 P:222 with N -> i)
-template <typename T> __device__ __forceinline__ void chirp(int u, int i, T& c, T& s) {
-    cispi_ratio((long long)(((unsigned)u * (unsigned)u) % (unsigned)(2 * i)), i, (T)-1, c, s);
+// shared memory: [exchange buffer of M complex][Ze / De: M/2 + 2 complex][roots of order Q = 8 i][roots of order M]
+// chirp c[u] = exp(-i pi u^2 / i) = omega^(4 (u^2 mod 2 i)), omega = exp(-2 pi i / 8 i)   (Eq. 19 P:222 with N -> i)
+__device__ __forceinline__ int chirp_index(int u, int twoi, float inv_twoi) {
+    const unsigned t = (unsigned)u * (unsigned)u;  // < 2^24: exact in fp32
+    const int q = (int)((float)t * inv_twoi);      // floor(t / 2i) +- 1
+    int r = (int)t - q * twoi;
+    if (r < 0) r += twoi;
+    if (r >= twoi) r -= twoi;
+    return 4 * r;
 }
 
 // One length-i chirp-z transform of the sequence already multiplied by the chirp and zero-padded in registers
 // (pass-0 layout): FFT_M -> times filter spectrum -> IFFT_M (Eq. 22).  Result: conv[idx] in registers.
 template <typename T, int LOGM>
-__device__ __forceinline__ void chirp_convolve(T (&re)[BlockFFT<T, LOGM>::E], T (&im)[BlockFFT<T, LOGM>::E], T* sre, T* sim,
-                                               const typename V2<T>::type* __restrict__ tw, int twlen,
-                                               const typename V2<T>::type* __restrict__ filt, int tid) {
+__device__ __forceinline__ void chirp_convolve(T (&re)[BlockFFT<T, LOGM>::E], T (&im)[BlockFFT<T, LOGM>::E], const Xchg<T>& xs,
+                                               const Roots<T>& rtM, const typename V2<T>::type* __restrict__ filt, int tid) {
     using F = BlockFFT<T, LOGM>;
-    F::forward(re, im, sre, sim, tw, twlen, tid);
+    F::forward(re, im, xs, rtM, tid);
 #pragma unroll
     for (int e = 0; e < F::E; ++e) {
         const typename V2<T>::type f = __ldg(filt + e * F::NT + tid);
@@ -373,28 +422,43 @@ __device__ __forceinline__ void chirp_convolve(T (&re)[BlockFFT<T, LOGM>::E], T 
         re[e] = a * f.x - b * f.y;
         im[e] = a * f.y + b * f.x;
     }
-    F::inverse(re, im, sre, sim, tw, twlen, tid);
+    F::inverse(re, im, xs, rtM, tid);
 }
 
+template <typename T, int LOGM> struct BlueSmem {
+    static constexpr int M = 1 << LOGM;
+    static constexpr size_t off_z = Xchg<T>::bytes(M);
+    static constexpr size_t off_rq = off_z + sizeof(T) * 2 * ((size_t)M / 2 + 2);
+    static constexpr size_t off_rm = off_rq + sizeof(T) * 2 * (size_t)roots_len(4 * M + 8);  // Q = 8 i <= 4 M + 8
+    static constexpr size_t total = off_rm + sizeof(T) * 2 * (size_t)roots_len(M);
+};
+
 template <typename T, int LOGM>
-__global__ void __launch_bounds__(FftPlan<LOGM>::NT, 512 / FftPlan<LOGM>::NT) ring_blue_analysis_kernel(DevPlan P, const int* __restrict__ rings,
+__global__ void __launch_bounds__(FftPlan<LOGM>::NT, 512 / FftPlan<LOGM>::NT) ring_blue_analysis_kernel(DevPlan P, const RingInfo* __restrict__ info,
                                                                                const T* __restrict__ map,
                                                                                const double* __restrict__ w, int use_w,
                                                                                FftTables tabs) {
     using F = BlockFFT<T, LOGM>;
     using T2 = typename V2<T>::type;
+    using SM = BlueSmem<T, LOGM>;
     constexpr int M = F::N, E = F::E, NT = F::NT;
     extern __shared__ __align__(16) unsigned char smem_raw[];
-    T* sre = reinterpret_cast<T*>(smem_raw);
-    T* sim = sre + padded_len<T>(M);
-    T2* Ze = reinterpret_cast<T2*>(sim + padded_len<T>(M));
+    const Xchg<T> xs(smem_raw, M);
+    T2* Ze = reinterpret_cast<T2*>(smem_raw + SM::off_z);
+    T2* rq = reinterpret_cast<T2*>(smem_raw + SM::off_rq);
+    T2* rm = reinterpret_cast<T2*>(smem_raw + SM::off_rm);
     const int tid = threadIdx.x;
-    const int r = rings[blockIdx.x], ch = blockIdx.y;
-    const RingRef R = ring_ref(P, r, w, use_w);
-    const int N = R.N, i = N >> 2, n = N >> 1;
+    const int ch = blockIdx.y;
+    const RingInfo R = begin_item<T, true>(P, info, map, tabs.pf);
+    const int N = R.N, i = N >> 2, n = N >> 1, Q = 2 * N;
     const T2* src = reinterpret_cast<const T2*>(map + (size_t)ch * P.npix + R.start);
-    const T2* tw = reinterpret_cast<const T2*>(tabs.tw);
-    const T2* filt = reinterpret_cast<const T2*>(tabs.filt) + tabs.filt_offset[i];
+    const T2* filt = reinterpret_cast<const T2*>(tabs.filt) + __ldg(tabs.filt_offset + i);
+    fill_roots_any<T>(rq, Q, tid, NT);
+    fill_roots_pow2<T>(rm, M, reinterpret_cast<const T2*>(tabs.tw), tabs.twlen, tid, NT);
+    const T wt = (T)ring_weight(P, R, w, use_w);
+    const float inv_twoi = 1.0f / (float)(2 * i);
+    __syncthreads();
+    const Roots<T> rt(rq), rtM(rm);
     T re[E], im[E];
 #pragma unroll 1
     for (int sub = 0; sub < 2; ++sub) {
@@ -406,18 +470,18 @@ __global__ void __launch_bounds__(FftPlan<LOGM>::NT, 512 / FftPlan<LOGM>::NT) ri
             if (u < i) {
                 const T2 z = src[2 * u + sub];
                 T c, s;
-                chirp<T>(u, i, c, s);
+                rt.template get<-1>(chirp_index(u, 2 * i, inv_twoi), c, s);
                 re[e] = z.x * c - z.y * s;
                 im[e] = z.x * s + z.y * c;
             }
         }
-        chirp_convolve<T, LOGM>(re, im, sre, sim, tw, tabs.twlen, filt, tid);
+        chirp_convolve<T, LOGM>(re, im, xs, rtM, filt, tid);
 #pragma unroll
         for (int e = 0; e < E; ++e) {
             const int u = F::index0(tid, e);
             if (u < i) {
                 T c, s;
-                chirp<T>(u, i, c, s);
+                rt.template get<-1>(chirp_index(u, 2 * i, inv_twoi), c, s);
                 const T vr = re[e] * c - im[e] * s, vi = re[e] * s + im[e] * c;
                 if (sub == 0) {
                     T2 v;
@@ -425,25 +489,21 @@ __global__ void __launch_bounds__(FftPlan<LOGM>::NT, 512 / FftPlan<LOGM>::NT) ri
                     v.y = vi;
                     Ze[u] = v;
                 } else {  // own pass-0 slot of the exchange buffer: no other thread touches it
-                    sre[padi<T>(u)] = vr;
-                    sim[padi<T>(u)] = vi;
+                    xs.st(u, vr, vi);
                 }
             }
         }
     }
     __syncthreads();
-    // Z[q] = Ze[q mod i] + W_n^q Zo[q mod i], q < n = 2 i.  Every phase factor is a power of
-    // omega = exp(-i pi / (4 i)): twist = omega^m, W_N^kk = omega^(2 kk), W_n^q = omega^(4 q); without aliasing
-    // (m <= n, the common case) kk = m and one sincospi per output suffices.
-    const Cis<T, false> cis{tw, tabs.twlen};
-    T2* dst = reinterpret_cast<T2*>(P.spectra) + ((size_t)ch * P.nrings + r) * P.mstride;
-    const T wt = (T)R.weight;
+    // Z[q] = Ze[q mod i] + W_n^q Zo[q mod i], q < n = 2 i.  twist = omega^m, W_N^kk = omega^(2 kk),
+    // W_n^q = omega^(4 q); without aliasing (m <= n, the common case) kk = m and one root per output suffices.
+    T2* dst = reinterpret_cast<T2*>(P.spectra) + ((size_t)ch * P.nrings + R.r) * P.mstride;
     for (int m = tid; m <= R.mcut; m += NT) {
-        const int k = m % N;
+        const int k = m < N ? m : m % N;
         const bool cj = k > n;
         const int kk = cj ? N - k : k;
         T pc, ps;  // omega^kk
-        cis.template get<-1>(kk, 2 * N, pc, ps);
+        rt.template get<-1>(kk, pc, ps);
         const T w2c = pc * pc - ps * ps, w2s = 2 * pc * ps;      // W_N^kk
         const T w4c = w2c * w2c - w2s * w2s, w4s = 2 * w2c * w2s;  // W_n^kk
         const int q1 = kk == n ? 0 : kk, q2 = kk == 0 ? 0 : n - kk;
@@ -452,7 +512,9 @@ __global__ void __launch_bounds__(FftPlan<LOGM>::NT, 512 / FftPlan<LOGM>::NT) ri
         const T c1 = (kk == n) ? (T)1 : w4c, s1 = (kk == n) ? (T)0 : w4s;
         const T c2 = (kk == 0) ? (T)1 : w4c, s2 = (kk == 0) ? (T)0 : -w4s;
         const T2 ze1 = Ze[a1], ze2 = Ze[a2];
-        const T o1r = sre[padi<T>(a1)], o1i = sim[padi<T>(a1)], o2r = sre[padi<T>(a2)], o2i = sim[padi<T>(a2)];
+        T o1r, o1i, o2r, o2i;
+        xs.ld(a1, o1r, o1i);
+        xs.ld(a2, o2r, o2i);
         const T z1r = ze1.x + (o1r * c1 - o1i * s1), z1i = ze1.y + (o1r * s1 + o1i * c1);
         const T z2r = ze2.x + (o2r * c2 - o2i * s2), z2i = ze2.y + (o2r * s2 + o2i * c2);
         const T er = (T)0.5 * (z1r + z2r), ei = (T)0.5 * (z1i - z2i);
@@ -462,7 +524,7 @@ __global__ void __launch_bounds__(FftPlan<LOGM>::NT, 512 / FftPlan<LOGM>::NT) ri
         if (cj) xi = -xi;
         if (R.shifted) {
             T tc = pc, ts = ps;
-            if (k != m || cj) cis.template get<-1>(m % (2 * N), 2 * N, tc, ts);  // aliased: twist != omega^kk
+            if (k != m || cj) rt.template get<-1>(m % Q, tc, ts);  // aliased: twist != omega^kk
             const T tr = xr * tc - xi * ts, ti = xr * ts + xi * tc;
             xr = tr;
             xi = ti;
@@ -475,25 +537,31 @@ __global__ void __launch_bounds__(FftPlan<LOGM>::NT, 512 / FftPlan<LOGM>::NT) ri
 }
 
 template <typename T, int LOGM>
-__global__ void __launch_bounds__(FftPlan<LOGM>::NT, 512 / FftPlan<LOGM>::NT) ring_blue_synthesis_kernel(DevPlan P, const int* __restrict__ rings,
+__global__ void __launch_bounds__(FftPlan<LOGM>::NT, 512 / FftPlan<LOGM>::NT) ring_blue_synthesis_kernel(DevPlan P, const RingInfo* __restrict__ info,
                                                                                 T* __restrict__ map,
                                                                                 const double* __restrict__ w, int use_w,
                                                                                 FftTables tabs) {
     using F = BlockFFT<T, LOGM>;
     using T2 = typename V2<T>::type;
+    using SM = BlueSmem<T, LOGM>;
     constexpr int M = F::N, E = F::E, NT = F::NT;
     extern __shared__ __align__(16) unsigned char smem_raw[];
-    T* sre = reinterpret_cast<T*>(smem_raw);
-    T* sim = sre + padded_len<T>(M);
-    T2* De = reinterpret_cast<T2*>(sim + padded_len<T>(M));
+    const Xchg<T> xs(smem_raw, M);
+    T2* De = reinterpret_cast<T2*>(smem_raw + SM::off_z);
+    T2* rq = reinterpret_cast<T2*>(smem_raw + SM::off_rq);
+    T2* rm = reinterpret_cast<T2*>(smem_raw + SM::off_rm);
     const int tid = threadIdx.x;
-    const int r = rings[blockIdx.x], ch = blockIdx.y;
-    const RingRef R = ring_ref(P, r, w, use_w);
-    const int N = R.N, i = N >> 2, n = N >> 1;
-    const T2* tw = reinterpret_cast<const T2*>(tabs.tw);
-    const T2* filt = reinterpret_cast<const T2*>(tabs.filt) + tabs.filt_offset[i];
-    const Cis<T, false> cis{tw, tabs.twlen};
-    const T2* G = reinterpret_cast<const T2*>(P.spectra) + ((size_t)ch * P.nrings + r) * P.mstride;
+    const int ch = blockIdx.y;
+    const RingInfo R = begin_item<T, false>(P, info, map, tabs.pf);
+    const int N = R.N, i = N >> 2, n = N >> 1, Q = 2 * N;
+    const T2* filt = reinterpret_cast<const T2*>(tabs.filt) + __ldg(tabs.filt_offset + i);
+    fill_roots_any<T>(rq, Q, tid, NT);
+    fill_roots_pow2<T>(rm, M, reinterpret_cast<const T2*>(tabs.tw), tabs.twlen, tid, NT);
+    const T wt = (T)ring_weight(P, R, w, use_w);
+    const float inv_twoi = 1.0f / (float)(2 * i);
+    __syncthreads();
+    const Roots<T> rt(rq), rtM(rm);
+    const T2* G = reinterpret_cast<const T2*>(P.spectra) + ((size_t)ch * P.nrings + R.r) * P.mstride;
     T re[E], im[E];
 #pragma unroll 1
     for (int sub = 0; sub < 2; ++sub) {
@@ -504,20 +572,20 @@ __global__ void __launch_bounds__(FftPlan<LOGM>::NT, 512 / FftPlan<LOGM>::NT) ri
             im[e] = 0;
             if (u < i) {
                 T yr, yi;
-                synth_packed_input<T, false>(G, 2 * u + sub, N, R.mcut, R.shifted, cis, yr, yi);
+                synth_packed_input<T, false>(G, 2 * u + sub, N, R.mcut, R.shifted, rt, yr, yi);
                 T c, s;
-                chirp<T>(u, i, c, s);
+                rt.template get<-1>(chirp_index(u, 2 * i, inv_twoi), c, s);
                 re[e] = yr * c - yi * s;
                 im[e] = yr * s + yi * c;
             }
         }
-        chirp_convolve<T, LOGM>(re, im, sre, sim, tw, tabs.twlen, filt, tid);
+        chirp_convolve<T, LOGM>(re, im, xs, rtM, filt, tid);
 #pragma unroll
         for (int e = 0; e < E; ++e) {
             const int u = F::index0(tid, e);
             if (u < i) {
                 T c, s;
-                chirp<T>(u, i, c, s);
+                rt.template get<-1>(chirp_index(u, 2 * i, inv_twoi), c, s);
                 const T vr = re[e] * c - im[e] * s, vi = re[e] * s + im[e] * c;
                 if (sub == 0) {
                     T2 v;
@@ -525,8 +593,7 @@ __global__ void __launch_bounds__(FftPlan<LOGM>::NT, 512 / FftPlan<LOGM>::NT) ri
                     v.y = vi;
                     De[u] = v;
                 } else {
-                    sre[padi<T>(u)] = vr;
-                    sim[padi<T>(u)] = vi;
+                    xs.st(u, vr, vi);
                 }
             }
         }
@@ -534,13 +601,13 @@ __global__ void __launch_bounds__(FftPlan<LOGM>::NT, 512 / FftPlan<LOGM>::NT) ri
     __syncthreads();
     // D[t] = De[t mod i] + W_n^t Do[t mod i];  x[2t] = Re D[t], x[2t+1] = -Im D[t]
     T2* dst = reinterpret_cast<T2*>(map + (size_t)ch * P.npix + R.start);
-    const T wt = (T)R.weight;
     for (int t = tid; t < n; t += NT) {
         const int ti = t >= i ? t - i : t;
         T c, s;
-        cis.template get<-1>(t, n, c, s);
+        rt.template get<-1>(4 * t, c, s);
         const T2 de = De[ti];
-        const T orr = sre[padi<T>(ti)], oi = sim[padi<T>(ti)];
+        T orr, oi;
+        xs.ld(ti, orr, oi);
         T2 o;
         o.x = wt * (de.x + (orr * c - oi * s));
         o.y = -wt * (de.y + (orr * s + oi * c));
@@ -558,10 +625,13 @@ __global__ void __launch_bounds__(FftPlan<LOGM>::NT) blue_filter_kernel(const in
     using F = BlockFFT<double, LOGM>;
     constexpr int M = F::N, E = F::E, NT = F::NT;
     extern __shared__ __align__(16) unsigned char smem_raw[];
-    double* sre = reinterpret_cast<double*>(smem_raw);
-    double* sim = sre + padded_len<double>(M);
+    const Xchg<double> xs(smem_raw, M);
+    double2* rm = reinterpret_cast<double2*>(smem_raw + Xchg<double>::bytes(M));
     const int tid = threadIdx.x;
     const int i = ivals[blockIdx.x];
+    fill_roots_pow2<double>(rm, M, tw64, twlen, tid, NT);
+    __syncthreads();
+    const Roots<double> rtM(rm);
     double re[E], im[E];
 #pragma unroll
     for (int e = 0; e < E; ++e) {
@@ -578,7 +648,7 @@ __global__ void __launch_bounds__(FftPlan<LOGM>::NT) blue_filter_kernel(const in
             im[e] = s;
         }
     }
-    F::forward(re, im, sre, sim, tw64, twlen, tid);
+    F::forward(re, im, xs, rtM, tid);
     typename V2<T>::type* dst = out + offsets[i];
 #pragma unroll
     for (int e = 0; e < E; ++e) {
@@ -607,20 +677,22 @@ static int blue_logm(int i) {  // M = 2^LOGM >= 2 i - 1, at least 2^MIN_LOG
 }
 
 template <typename T, int LOG> static size_t fft_smem_bytes(bool blue) {
-    size_t b = 2 * (size_t)padded_len<T>(1 << LOG) * sizeof(T);
-    if (blue) b += sizeof(T) * 2 * ((size_t)(1 << LOG) / 2 + 2) + 16;  // Ze: i <= (M + 1) / 2 complex
-    return b;
+    if (blue) return BlueSmem<T, LOG>::total;
+    return Xchg<T>::bytes(1 << LOG) + sizeof(T) * 2 * (size_t)roots_len(4 << LOG);
+}
+template <int LOG> static size_t filter_smem_bytes() {
+    return Xchg<double>::bytes(1 << LOG) + sizeof(double2) * (size_t)roots_len(1 << LOG);
 }
 
 bool fft_supported(int nside, cuhpx_dtype_t dt) {
     (void)dt;
-    return nside <= 4096;  // belt: n = 2 nside <= 2^13; caps: M <= 2^13 (fp64 needs 205 KB of the SM's 227 KB)
+    return nside <= 4096;  // belt: n = 2 nside <= 2^13; caps: M <= 2^13 (fp64 needs 209 KB of the SM's 227 KB)
 }
 
 struct RingFftLists {
-    std::vector<int> direct;
-    std::vector<int> pow2[MAX_LOG + 1];
-    std::vector<int> blue[MAX_LOG + 1];
+    std::vector<RingInfo> direct;
+    std::vector<RingInfo> pow2[MAX_LOG + 1];
+    std::vector<RingInfo> blue[MAX_LOG + 1];
     std::vector<int> blue_i[MAX_LOG + 1];  // distinct i per LOGM
 };
 
@@ -628,19 +700,29 @@ static void classify(const HostPlan& hp, RingFftLists& L) {
     const DevPlan& d = hp.d;
     for (int r = 0; r < d.nrings; ++r) {
         const int j = std::min(r, d.nrings - 1 - r);
-        const int N = hp.h_ringN[j];
-        if (N <= DIRECT_MAX_N) L.direct.push_back(r);
-        else if (is_pow2(N)) L.pow2[ilog2_ceil(N) - 1].push_back(r);
+        RingInfo R;
+        R.N = hp.h_ringN[j];
+        R.start = (r > j) ? d.npix - R.N - hp.h_start[j] : hp.h_start[j];
+        R.mcut = hp.h_mcut.empty() ? 0 : hp.h_mcut[j];  // sizing pass: cut-offs not computed yet
+        R.shifted = hp.h_shifted[j];
+        R.r = r;
+        R.pad0 = R.pad1 = 0;
+        const int N = R.N;
+        if (N <= DIRECT_MAX_N) L.direct.push_back(R);
+        else if (is_pow2(N)) L.pow2[ilog2_ceil(N) - 1].push_back(R);
         else {
             const int i = N / 4, lm = blue_logm(i);
-            L.blue[lm].push_back(r);
+            L.blue[lm].push_back(R);
             if (r == j) L.blue_i[lm].push_back(i);
         }
     }
+    // longest rings first inside a class: the tail of a launch is then made of its cheapest items
+    for (int l = MIN_LOG; l <= MAX_LOG; ++l)
+        std::stable_sort(L.blue[l].begin(), L.blue[l].end(), [](const RingInfo& a, const RingInfo& b) { return a.N > b.N; });
 }
 
 // Device layout of the FFT tables inside the workspace (all offsets relative to `base`):
-//   [ring lists: direct | pow2[8..13] | blue[8..13] | blue_i[8..13]] [filt_offset: nside x i64]
+//   [work items: direct | pow2[8..13] | blue[8..13]] [blue_i[8..13]] [filt_offset: nside x i64]
 //   [twiddle T2[twlen]] [twiddle double2[twlen] (set-up only, kept)] [filters]
 struct FftLayout {
     size_t off_direct, off_pow2[MAX_LOG + 1], off_blue[MAX_LOG + 1], off_blue_i[MAX_LOG + 1];
@@ -658,10 +740,10 @@ static FftLayout fft_layout(const HostPlan& hp, const RingFftLists& L, std::vect
         o = (o + bytes + 255) / 256 * 256;
         return r;
     };
-    Y.off_direct = take(sizeof(int) * L.direct.size());
+    Y.off_direct = take(sizeof(RingInfo) * L.direct.size());
     for (int l = MIN_LOG; l <= MAX_LOG; ++l) {
-        Y.off_pow2[l] = take(sizeof(int) * L.pow2[l].size());
-        Y.off_blue[l] = take(sizeof(int) * L.blue[l].size());
+        Y.off_pow2[l] = take(sizeof(RingInfo) * L.pow2[l].size());
+        Y.off_blue[l] = take(sizeof(RingInfo) * L.blue[l].size());
         Y.off_blue_i[l] = take(sizeof(int) * L.blue_i[l].size());
     }
     Y.off_filt_offset = take(sizeof(long long) * d.nside);
@@ -682,15 +764,17 @@ static FftLayout fft_layout(const HostPlan& hp, const RingFftLists& L, std::vect
 }
 
 struct FftDev {  // device pointers resolved from the layout (kept per plan in a side table)
-    const int* direct;
-    const int* pow2[MAX_LOG + 1];
-    const int* blue[MAX_LOG + 1];
+    const RingInfo* direct;
+    const RingInfo* pow2[MAX_LOG + 1];
+    const RingInfo* blue[MAX_LOG + 1];
     int n_direct, n_pow2[MAX_LOG + 1], n_blue[MAX_LOG + 1];
+    // prefetch distance per launch: CTAs resident on the whole GPU, [analysis 0 / synthesis 1][pow2 0 / blue 1][LOG]
+    int pf[2][2][MAX_LOG + 1];
     int max_mcut_direct;
     FftTables tabs;
 };
 
-template <typename T, int LOG> static cudaError_t set_smem_attrs() {
+template <typename T, int LOG> static cudaError_t set_smem_attrs(FftDev& D, int sms) {
     cudaError_t e;
     const size_t sp = fft_smem_bytes<T, LOG>(false), sb = fft_smem_bytes<T, LOG>(true);
     if ((e = cudaFuncSetAttribute(ring_pow2_analysis_kernel<T, LOG>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sp))) return e;
@@ -698,7 +782,17 @@ template <typename T, int LOG> static cudaError_t set_smem_attrs() {
     if ((e = cudaFuncSetAttribute(ring_blue_analysis_kernel<T, LOG>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sb))) return e;
     if ((e = cudaFuncSetAttribute(ring_blue_synthesis_kernel<T, LOG>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sb))) return e;
     if ((e = cudaFuncSetAttribute(blue_filter_kernel<T, LOG>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                  (int)fft_smem_bytes<double, LOG>(false)))) return e;
+                                  (int)filter_smem_bytes<LOG>()))) return e;
+    int occ = 0;
+    constexpr int NT = FftPlan<LOG>::NT;
+    if ((e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, ring_pow2_analysis_kernel<T, LOG>, NT, sp))) return e;
+    D.pf[0][0][LOG] = occ * sms;
+    if ((e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, ring_pow2_synthesis_kernel<T, LOG>, NT, sp))) return e;
+    D.pf[1][0][LOG] = occ * sms;
+    if ((e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, ring_blue_analysis_kernel<T, LOG>, NT, sb))) return e;
+    D.pf[0][1][LOG] = occ * sms;
+    if ((e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, ring_blue_synthesis_kernel<T, LOG>, NT, sb))) return e;
+    D.pf[1][1][LOG] = occ * sms;
     return cudaSuccess;
 }
 
@@ -706,17 +800,20 @@ template <typename T, int LOG>
 static cudaError_t build_filters(const RingFftLists& L, const FftLayout& Y, char* base, cudaStream_t st, int twlen) {
     if (L.blue_i[LOG].empty()) return cudaSuccess;
     using T2 = typename V2<T>::type;
-    blue_filter_kernel<T, LOG><<<(unsigned)L.blue_i[LOG].size(), FftPlan<LOG>::NT, fft_smem_bytes<double, LOG>(false), st>>>(
+    blue_filter_kernel<T, LOG><<<(unsigned)L.blue_i[LOG].size(), FftPlan<LOG>::NT, filter_smem_bytes<LOG>(), st>>>(
         (const int*)(base + Y.off_blue_i[LOG]), (const long long*)(base + Y.off_filt_offset), (T2*)(base + Y.off_filt),
         (const double2*)(base + Y.off_tw64), twlen);
     return cudaGetLastError();
 }
 
-template <typename T> static cudaError_t build_tables_t(HostPlan& hp, const RingFftLists& L, const FftLayout& Y, char* base,
+template <typename T> static cudaError_t build_tables_t(FftDev& D, const RingFftLists& L, const FftLayout& Y, char* base,
                                                         cudaStream_t st, int twlen) {
     using T2 = typename V2<T>::type;
     cudaError_t e;
-#define CUHPX_ATTR(LOG) if ((e = set_smem_attrs<T, LOG>()) != cudaSuccess) return e;
+    int dev = 0, sms = 0;
+    if ((e = cudaGetDevice(&dev)) != cudaSuccess) return e;
+    if ((e = cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev)) != cudaSuccess) return e;
+#define CUHPX_ATTR(LOG) if ((e = set_smem_attrs<T, LOG>(D, sms)) != cudaSuccess) return e;
     CUHPX_ATTR(8) CUHPX_ATTR(9) CUHPX_ATTR(10) CUHPX_ATTR(11) CUHPX_ATTR(12) CUHPX_ATTR(13)
 #undef CUHPX_ATTR
     twiddle_table_kernel<T><<<(twlen + 255) / 256, 256, 0, st>>>((T2*)(base + Y.off_tw), twlen);
@@ -725,7 +822,6 @@ template <typename T> static cudaError_t build_tables_t(HostPlan& hp, const Ring
 #define CUHPX_FILT(LOG) if ((e = build_filters<T, LOG>(L, Y, base, st, twlen)) != cudaSuccess) return e;
     CUHPX_FILT(8) CUHPX_FILT(9) CUHPX_FILT(10) CUHPX_FILT(11) CUHPX_FILT(12) CUHPX_FILT(13)
 #undef CUHPX_FILT
-    (void)hp;
     return cudaSuccess;
 }
 
@@ -741,23 +837,24 @@ size_t plan_fft_tables(HostPlan& hp, char* base, bool build, cudaStream_t st, cu
     auto up = [&](size_t off, const void* src, size_t bytes) {
         if (e == cudaSuccess && bytes) e = cudaMemcpyAsync(base + off, src, bytes, cudaMemcpyHostToDevice, st);
     };
-    up(Y.off_direct, L.direct.data(), sizeof(int) * L.direct.size());
+    up(Y.off_direct, L.direct.data(), sizeof(RingInfo) * L.direct.size());
     for (int l = MIN_LOG; l <= MAX_LOG; ++l) {
-        up(Y.off_pow2[l], L.pow2[l].data(), sizeof(int) * L.pow2[l].size());
-        up(Y.off_blue[l], L.blue[l].data(), sizeof(int) * L.blue[l].size());
+        up(Y.off_pow2[l], L.pow2[l].data(), sizeof(RingInfo) * L.pow2[l].size());
+        up(Y.off_blue[l], L.blue[l].data(), sizeof(RingInfo) * L.blue[l].size());
         up(Y.off_blue_i[l], L.blue_i[l].data(), sizeof(int) * L.blue_i[l].size());
     }
     up(Y.off_filt_offset, filt_off.data(), sizeof(long long) * d.nside);
     if (e == cudaSuccess) e = cudaStreamSynchronize(st);  // pageable sources
-    if (e == cudaSuccess)
-        e = hp.dtype == CUHPX_F64 ? build_tables_t<double>(hp, L, Y, base, st, twlen)
-                                  : build_tables_t<float>(hp, L, Y, base, st, twlen);
     FftDev D;
-    D.direct = (const int*)(base + Y.off_direct);
+    memset(&D, 0, sizeof(D));
+    if (e == cudaSuccess)
+        e = hp.dtype == CUHPX_F64 ? build_tables_t<double>(D, L, Y, base, st, twlen)
+                                  : build_tables_t<float>(D, L, Y, base, st, twlen);
+    D.direct = (const RingInfo*)(base + Y.off_direct);
     D.n_direct = (int)L.direct.size();
     for (int l = 0; l <= MAX_LOG; ++l) {
-        D.pow2[l] = l >= MIN_LOG ? (const int*)(base + Y.off_pow2[l]) : nullptr;
-        D.blue[l] = l >= MIN_LOG ? (const int*)(base + Y.off_blue[l]) : nullptr;
+        D.pow2[l] = l >= MIN_LOG ? (const RingInfo*)(base + Y.off_pow2[l]) : nullptr;
+        D.blue[l] = l >= MIN_LOG ? (const RingInfo*)(base + Y.off_blue[l]) : nullptr;
         D.n_pow2[l] = l >= MIN_LOG ? (int)L.pow2[l].size() : 0;
         D.n_blue[l] = l >= MIN_LOG ? (int)L.blue[l].size() : 0;
     }
@@ -765,8 +862,9 @@ size_t plan_fft_tables(HostPlan& hp, char* base, bool build, cudaStream_t st, cu
     D.tabs.twlen = twlen;
     D.tabs.filt = base + Y.off_filt;
     D.tabs.filt_offset = (const long long*)(base + Y.off_filt_offset);
+    D.tabs.pf = 0;
     D.max_mcut_direct = 0;
-    for (int r : L.direct) D.max_mcut_direct = std::max(D.max_mcut_direct, hp.h_mcut[std::min(r, d.nrings - 1 - r)]);
+    for (const RingInfo& R : L.direct) D.max_mcut_direct = std::max(D.max_mcut_direct, R.mcut);
     const size_t csz = hp.dtype == CUHPX_F64 ? 16 : 8;
     if (e == cudaSuccess && (DIRECT_MAX_N + D.max_mcut_direct + 1) * csz > 200 * 1024) e = cudaErrorInvalidConfiguration;
     if (e == cudaSuccess) {
@@ -777,7 +875,8 @@ size_t plan_fft_tables(HostPlan& hp, char* base, bool build, cudaStream_t st, cu
     }
     delete hp.fft;
     hp.fft = new FftDev(D);
-    hp.rings_direct = L.direct;
+    hp.rings_direct.clear();
+    for (const RingInfo& R : L.direct) hp.rings_direct.push_back(R.r);
     *err = e;
     return Y.total;
 }
@@ -804,22 +903,32 @@ void fft_stage_stats(const HostPlan& hp, int* launches, double* table_bytes) {
 // ------------------------------------------------------------------ launchers
 template <typename T, int LOG>
 static void launch_class_analysis(const DevPlan& P, const FftDev& D, const T* map, const double* w, int use_w, cudaStream_t st) {
-    if (D.n_pow2[LOG])
+    FftTables tabs = D.tabs;
+    if (D.n_pow2[LOG]) {
+        tabs.pf = D.pf[0][0][LOG];
         ring_pow2_analysis_kernel<T, LOG><<<dim3(D.n_pow2[LOG], P.batch), FftPlan<LOG>::NT, fft_smem_bytes<T, LOG>(false), st>>>(
-            P, D.pow2[LOG], map, w, use_w, D.tabs);
-    if (D.n_blue[LOG])
+            P, D.pow2[LOG], map, w, use_w, tabs);
+    }
+    if (D.n_blue[LOG]) {
+        tabs.pf = D.pf[0][1][LOG];
         ring_blue_analysis_kernel<T, LOG><<<dim3(D.n_blue[LOG], P.batch), FftPlan<LOG>::NT, fft_smem_bytes<T, LOG>(true), st>>>(
-            P, D.blue[LOG], map, w, use_w, D.tabs);
+            P, D.blue[LOG], map, w, use_w, tabs);
+    }
 }
 
 template <typename T, int LOG>
 static void launch_class_synthesis(const DevPlan& P, const FftDev& D, T* map, const double* w, int use_w, cudaStream_t st) {
-    if (D.n_pow2[LOG])
+    FftTables tabs = D.tabs;
+    if (D.n_pow2[LOG]) {
+        tabs.pf = D.pf[1][0][LOG];
         ring_pow2_synthesis_kernel<T, LOG><<<dim3(D.n_pow2[LOG], P.batch), FftPlan<LOG>::NT, fft_smem_bytes<T, LOG>(false), st>>>(
-            P, D.pow2[LOG], map, w, use_w, D.tabs);
-    if (D.n_blue[LOG])
+            P, D.pow2[LOG], map, w, use_w, tabs);
+    }
+    if (D.n_blue[LOG]) {
+        tabs.pf = D.pf[1][1][LOG];
         ring_blue_synthesis_kernel<T, LOG><<<dim3(D.n_blue[LOG], P.batch), FftPlan<LOG>::NT, fft_smem_bytes<T, LOG>(true), st>>>(
-            P, D.blue[LOG], map, w, use_w, D.tabs);
+            P, D.blue[LOG], map, w, use_w, tabs);
+    }
 }
 
 template <typename T>
