@@ -316,10 +316,18 @@ __device__ __forceinline__ typename V2<T>::type analysis_unpack(T z1r, T z1i, T 
     return o;
 }
 
+// Resident CTAs per SM the register allocation aims for: 16 points per thread are 64 (fp64) / 32 (fp32) data
+// registers, so fp64 kernels get 128 registers per thread and fp32 pow2 kernels 64.
+template <typename T, int LOG> struct MinBlocks {
+    static constexpr int NT = FftPlan<LOG>::NT;
+    static constexpr int value = (sizeof(T) == 4 ? 1024 : 512) / NT > 16 ? 16 : (sizeof(T) == 4 ? 1024 : 512) / NT;
+    static constexpr int blue = 512 / NT;
+};
+
 // ------------------------------------------------------------------ power-of-two rings
 // shared memory: [exchange buffer of n complex][root table of order Q = 2 N = 4 n]
 template <typename T, int LOGN>
-__global__ void __launch_bounds__(FftPlan<LOGN>::NT) ring_pow2_analysis_kernel(DevPlan P, const RingInfo* __restrict__ info,
+__global__ void __launch_bounds__(FftPlan<LOGN>::NT, MinBlocks<T, LOGN>::value) ring_pow2_analysis_kernel(DevPlan P, const RingInfo* __restrict__ info,
                                                                                const T* __restrict__ map,
                                                                                const double* __restrict__ w, int use_w,
                                                                                FftTables tabs) {
@@ -348,6 +356,7 @@ __global__ void __launch_bounds__(FftPlan<LOGN>::NT) ring_pow2_analysis_kernel(D
     F::store_natural(re, im, xs, tid);
     __syncthreads();
     T2* dst = reinterpret_cast<T2*>(P.spectra) + ((size_t)ch * P.nrings + R.r) * P.mstride;
+#pragma unroll 4
     for (int m = tid; m <= R.mcut; m += NT) {
         const int k = m & (N - 1);
         const bool cj = k > n;
@@ -360,7 +369,7 @@ __global__ void __launch_bounds__(FftPlan<LOGN>::NT) ring_pow2_analysis_kernel(D
 }
 
 template <typename T, int LOGN>
-__global__ void __launch_bounds__(FftPlan<LOGN>::NT) ring_pow2_synthesis_kernel(DevPlan P, const RingInfo* __restrict__ info,
+__global__ void __launch_bounds__(FftPlan<LOGN>::NT, MinBlocks<T, LOGN>::value) ring_pow2_synthesis_kernel(DevPlan P, const RingInfo* __restrict__ info,
                                                                                 T* __restrict__ map,
                                                                                 const double* __restrict__ w, int use_w,
                                                                                 FftTables tabs) {
@@ -386,6 +395,7 @@ __global__ void __launch_bounds__(FftPlan<LOGN>::NT) ring_pow2_synthesis_kernel(
     F::store_natural(re, im, xs, tid);
     __syncthreads();
     T2* dst = reinterpret_cast<T2*>(map + (size_t)ch * P.npix + R.start);
+#pragma unroll
     for (int t = tid; t < n; t += NT) {
         T a, b;
         xs.ld(t, a, b);
@@ -434,7 +444,7 @@ template <typename T, int LOGM> struct BlueSmem {
 };
 
 template <typename T, int LOGM>
-__global__ void __launch_bounds__(FftPlan<LOGM>::NT, 512 / FftPlan<LOGM>::NT) ring_blue_analysis_kernel(DevPlan P, const RingInfo* __restrict__ info,
+__global__ void __launch_bounds__(FftPlan<LOGM>::NT, MinBlocks<T, LOGM>::blue) ring_blue_analysis_kernel(DevPlan P, const RingInfo* __restrict__ info,
                                                                                const T* __restrict__ map,
                                                                                const double* __restrict__ w, int use_w,
                                                                                FftTables tabs) {
@@ -498,6 +508,7 @@ __global__ void __launch_bounds__(FftPlan<LOGM>::NT, 512 / FftPlan<LOGM>::NT) ri
     // Z[q] = Ze[q mod i] + W_n^q Zo[q mod i], q < n = 2 i.  twist = omega^m, W_N^kk = omega^(2 kk),
     // W_n^q = omega^(4 q); without aliasing (m <= n, the common case) kk = m and one root per output suffices.
     T2* dst = reinterpret_cast<T2*>(P.spectra) + ((size_t)ch * P.nrings + R.r) * P.mstride;
+#pragma unroll 2
     for (int m = tid; m <= R.mcut; m += NT) {
         const int k = m < N ? m : m % N;
         const bool cj = k > n;
@@ -537,7 +548,7 @@ __global__ void __launch_bounds__(FftPlan<LOGM>::NT, 512 / FftPlan<LOGM>::NT) ri
 }
 
 template <typename T, int LOGM>
-__global__ void __launch_bounds__(FftPlan<LOGM>::NT, 512 / FftPlan<LOGM>::NT) ring_blue_synthesis_kernel(DevPlan P, const RingInfo* __restrict__ info,
+__global__ void __launch_bounds__(FftPlan<LOGM>::NT, MinBlocks<T, LOGM>::blue) ring_blue_synthesis_kernel(DevPlan P, const RingInfo* __restrict__ info,
                                                                                 T* __restrict__ map,
                                                                                 const double* __restrict__ w, int use_w,
                                                                                 FftTables tabs) {
@@ -601,6 +612,7 @@ __global__ void __launch_bounds__(FftPlan<LOGM>::NT, 512 / FftPlan<LOGM>::NT) ri
     __syncthreads();
     // D[t] = De[t mod i] + W_n^t Do[t mod i];  x[2t] = Re D[t], x[2t+1] = -Im D[t]
     T2* dst = reinterpret_cast<T2*>(map + (size_t)ch * P.npix + R.start);
+#pragma unroll 4
     for (int t = tid; t < n; t += NT) {
         const int ti = t >= i ? t - i : t;
         T c, s;
@@ -709,8 +721,8 @@ static void classify(const HostPlan& hp, RingFftLists& L) {
         R.pad0 = R.pad1 = 0;
         const int N = R.N;
         if (N <= DIRECT_MAX_N) L.direct.push_back(R);
-        else if (is_pow2(N)) L.pow2[ilog2_ceil(N) - 1].push_back(R);
-        else {
+        else if (N == 4 * d.nside) L.pow2[ilog2_ceil(N) - 1].push_back(R);  // belt rings (N = 4 nside = 2^k)
+        else {  // cap rings, chirp-z for every i (the few i = 2^k among them are not worth launches of their own)
             const int i = N / 4, lm = blue_logm(i);
             L.blue[lm].push_back(R);
             if (r == j) L.blue_i[lm].push_back(i);
@@ -772,6 +784,11 @@ struct FftDev {  // device pointers resolved from the layout (kept per plan in a
     int pf[2][2][MAX_LOG + 1];
     int max_mcut_direct;
     FftTables tabs;
+    // The short-ring classes run on a side stream beside the long-ring kernels (fork / join with events), so
+    // their launch latencies and partial waves hide under the kernels that carry the bytes.
+    cudaStream_t side;
+    cudaEvent_t ev_fork, ev_join;
+    int side_from;  // Bluestein classes with LOG <= side_from go to the side stream (with the direct kernel)
 };
 
 template <typename T, int LOG> static cudaError_t set_smem_attrs(FftDev& D, int sms) {
@@ -873,7 +890,17 @@ size_t plan_fft_tables(HostPlan& hp, char* base, bool build, cudaStream_t st, cu
                 ? cudaFuncSetAttribute(ring_direct_synthesis_kernel<double>, cudaFuncAttributeMaxDynamicSharedMemorySize, std::max(want, 48 * 1024))
                 : cudaFuncSetAttribute(ring_direct_synthesis_kernel<float>, cudaFuncAttributeMaxDynamicSharedMemorySize, std::max(want, 48 * 1024));
     }
-    delete hp.fft;
+    D.side_from = -1;
+    {
+        int lmax_blue = -1;
+        for (int l = MIN_LOG; l <= MAX_LOG; ++l)
+            if (D.n_blue[l]) lmax_blue = l;
+        D.side_from = lmax_blue - 2;
+    }
+    if (e == cudaSuccess) e = cudaStreamCreateWithFlags(&D.side, cudaStreamNonBlocking);
+    if (e == cudaSuccess) e = cudaEventCreateWithFlags(&D.ev_fork, cudaEventDisableTiming);
+    if (e == cudaSuccess) e = cudaEventCreateWithFlags(&D.ev_join, cudaEventDisableTiming);
+    free_fft_dev(hp.fft);
     hp.fft = new FftDev(D);
     hp.rings_direct.clear();
     for (const RingInfo& R : L.direct) hp.rings_direct.push_back(R.r);
@@ -881,7 +908,13 @@ size_t plan_fft_tables(HostPlan& hp, char* base, bool build, cudaStream_t st, cu
     return Y.total;
 }
 
-void free_fft_dev(FftDev* f) { delete f; }
+void free_fft_dev(FftDev* f) {
+    if (!f) return;
+    if (f->ev_fork) cudaEventDestroy(f->ev_fork);
+    if (f->ev_join) cudaEventDestroy(f->ev_join);
+    if (f->side) cudaStreamDestroy(f->side);
+    delete f;
+}
 
 void fft_stage_stats(const HostPlan& hp, int* launches, double* table_bytes) {
     *launches = 0;
@@ -901,81 +934,82 @@ void fft_stage_stats(const HostPlan& hp, int* launches, double* table_bytes) {
 }
 
 // ------------------------------------------------------------------ launchers
-template <typename T, int LOG>
-static void launch_class_analysis(const DevPlan& P, const FftDev& D, const T* map, const double* w, int use_w, cudaStream_t st) {
+// Bluestein classes LOG <= side_from and the direct kernel go to the side stream
+template <typename T, bool ANALYSIS, int LOG>
+static void launch_class(const DevPlan& P, const FftDev& D, T* map, const double* w, int use_w, cudaStream_t main_st,
+                         cudaStream_t side_st) {
     FftTables tabs = D.tabs;
+    constexpr int A = ANALYSIS ? 0 : 1;
     if (D.n_pow2[LOG]) {
-        tabs.pf = D.pf[0][0][LOG];
-        ring_pow2_analysis_kernel<T, LOG><<<dim3(D.n_pow2[LOG], P.batch), FftPlan<LOG>::NT, fft_smem_bytes<T, LOG>(false), st>>>(
-            P, D.pow2[LOG], map, w, use_w, tabs);
+        tabs.pf = D.pf[A][0][LOG];
+        if (ANALYSIS)
+            ring_pow2_analysis_kernel<T, LOG><<<dim3(D.n_pow2[LOG], P.batch), FftPlan<LOG>::NT, fft_smem_bytes<T, LOG>(false), main_st>>>(
+                P, D.pow2[LOG], map, w, use_w, tabs);
+        else
+            ring_pow2_synthesis_kernel<T, LOG><<<dim3(D.n_pow2[LOG], P.batch), FftPlan<LOG>::NT, fft_smem_bytes<T, LOG>(false), main_st>>>(
+                P, D.pow2[LOG], map, w, use_w, tabs);
     }
     if (D.n_blue[LOG]) {
-        tabs.pf = D.pf[0][1][LOG];
-        ring_blue_analysis_kernel<T, LOG><<<dim3(D.n_blue[LOG], P.batch), FftPlan<LOG>::NT, fft_smem_bytes<T, LOG>(true), st>>>(
-            P, D.blue[LOG], map, w, use_w, tabs);
+        tabs.pf = D.pf[A][1][LOG];
+        cudaStream_t st = LOG <= D.side_from ? side_st : main_st;
+        if (ANALYSIS)
+            ring_blue_analysis_kernel<T, LOG><<<dim3(D.n_blue[LOG], P.batch), FftPlan<LOG>::NT, fft_smem_bytes<T, LOG>(true), st>>>(
+                P, D.blue[LOG], map, w, use_w, tabs);
+        else
+            ring_blue_synthesis_kernel<T, LOG><<<dim3(D.n_blue[LOG], P.batch), FftPlan<LOG>::NT, fft_smem_bytes<T, LOG>(true), st>>>(
+                P, D.blue[LOG], map, w, use_w, tabs);
     }
 }
 
-template <typename T, int LOG>
-static void launch_class_synthesis(const DevPlan& P, const FftDev& D, T* map, const double* w, int use_w, cudaStream_t st) {
-    FftTables tabs = D.tabs;
-    if (D.n_pow2[LOG]) {
-        tabs.pf = D.pf[1][0][LOG];
-        ring_pow2_synthesis_kernel<T, LOG><<<dim3(D.n_pow2[LOG], P.batch), FftPlan<LOG>::NT, fft_smem_bytes<T, LOG>(false), st>>>(
-            P, D.pow2[LOG], map, w, use_w, tabs);
-    }
-    if (D.n_blue[LOG]) {
-        tabs.pf = D.pf[1][1][LOG];
-        ring_blue_synthesis_kernel<T, LOG><<<dim3(D.n_blue[LOG], P.batch), FftPlan<LOG>::NT, fft_smem_bytes<T, LOG>(true), st>>>(
-            P, D.blue[LOG], map, w, use_w, tabs);
-    }
-}
-
-template <typename T>
-static cudaError_t run_fft_analysis(const HostPlan& hp, const void* d_map, const double* d_w, int use_w, cudaStream_t st) {
+template <typename T, bool ANALYSIS>
+static cudaError_t run_fft_stage(const HostPlan& hp, T* map, const double* d_w, int use_w, cudaStream_t st) {
     const DevPlan& P = hp.d;
     if (!hp.fft) return cudaErrorInvalidValue;
     const FftDev& D = *hp.fft;
-    const T* map = (const T*)d_map;
+    bool side_work = D.n_direct > 0, main_work = false;
+    for (int l = MIN_LOG; l <= MAX_LOG; ++l) {
+        if (D.n_blue[l] && l <= D.side_from) side_work = true;
+        if (D.n_pow2[l] || (D.n_blue[l] && l > D.side_from)) main_work = true;
+    }
+    const bool fork = side_work && main_work;
+    cudaStream_t side = fork ? D.side : st;
+    cudaError_t e;
+    if (fork) {
+        if ((e = cudaEventRecord(D.ev_fork, st)) != cudaSuccess) return e;
+        if ((e = cudaStreamWaitEvent(side, D.ev_fork, 0)) != cudaSuccess) return e;
+    }
     // largest rings first: they dominate the run time
-    launch_class_analysis<T, 13>(P, D, map, d_w, use_w, st);
-    launch_class_analysis<T, 12>(P, D, map, d_w, use_w, st);
-    launch_class_analysis<T, 11>(P, D, map, d_w, use_w, st);
-    launch_class_analysis<T, 10>(P, D, map, d_w, use_w, st);
-    launch_class_analysis<T, 9>(P, D, map, d_w, use_w, st);
-    launch_class_analysis<T, 8>(P, D, map, d_w, use_w, st);
-    if (D.n_direct)
-        ring_direct_analysis_kernel<T><<<dim3(D.n_direct, P.batch), FFT_THREADS, (size_t)DIRECT_MAX_N * 3 * sizeof(T), st>>>(
-            P, D.direct, map, d_w, use_w);
-    return cudaGetLastError();
-}
-
-template <typename T>
-static cudaError_t run_fft_synthesis(const HostPlan& hp, void* d_map, const double* d_w, int use_w, cudaStream_t st) {
-    const DevPlan& P = hp.d;
-    if (!hp.fft) return cudaErrorInvalidValue;
-    const FftDev& D = *hp.fft;
-    T* map = (T*)d_map;
-    launch_class_synthesis<T, 13>(P, D, map, d_w, use_w, st);
-    launch_class_synthesis<T, 12>(P, D, map, d_w, use_w, st);
-    launch_class_synthesis<T, 11>(P, D, map, d_w, use_w, st);
-    launch_class_synthesis<T, 10>(P, D, map, d_w, use_w, st);
-    launch_class_synthesis<T, 9>(P, D, map, d_w, use_w, st);
-    launch_class_synthesis<T, 8>(P, D, map, d_w, use_w, st);
-    if (D.n_direct)
-        ring_direct_synthesis_kernel<T><<<dim3(D.n_direct, P.batch), FFT_THREADS,
-                                          ((size_t)DIRECT_MAX_N + D.max_mcut_direct + 1) * 2 * sizeof(T), st>>>(P, D.direct, map, d_w, use_w);
-    return cudaGetLastError();
+    launch_class<T, ANALYSIS, 13>(P, D, map, d_w, use_w, st, side);
+    launch_class<T, ANALYSIS, 12>(P, D, map, d_w, use_w, st, side);
+    launch_class<T, ANALYSIS, 11>(P, D, map, d_w, use_w, st, side);
+    launch_class<T, ANALYSIS, 10>(P, D, map, d_w, use_w, st, side);
+    launch_class<T, ANALYSIS, 9>(P, D, map, d_w, use_w, st, side);
+    launch_class<T, ANALYSIS, 8>(P, D, map, d_w, use_w, st, side);
+    if (D.n_direct) {
+        if (ANALYSIS)
+            ring_direct_analysis_kernel<T><<<dim3(D.n_direct, P.batch), FFT_THREADS, (size_t)DIRECT_MAX_N * 3 * sizeof(T), side>>>(
+                P, D.direct, map, d_w, use_w);
+        else
+            ring_direct_synthesis_kernel<T><<<dim3(D.n_direct, P.batch), FFT_THREADS,
+                                              ((size_t)DIRECT_MAX_N + D.max_mcut_direct + 1) * 2 * sizeof(T), side>>>(P, D.direct, map, d_w, use_w);
+    }
+    if ((e = cudaGetLastError()) != cudaSuccess) return e;
+    if (fork) {
+        if ((e = cudaEventRecord(D.ev_join, side)) != cudaSuccess) return e;
+        if ((e = cudaStreamWaitEvent(st, D.ev_join, 0)) != cudaSuccess) return e;
+    }
+    return cudaSuccess;
 }
 
 cudaError_t launch_fft_analysis(const HostPlan& hp, const void* d_map, const double* d_w, int use_w, cudaStream_t st) {
-    return hp.dtype == CUHPX_F64 ? run_fft_analysis<double>(hp, d_map, d_w, use_w, st)
-                                 : run_fft_analysis<float>(hp, d_map, d_w, use_w, st);
+    // analysis kernels only read the map; one launcher template serves both directions
+    return hp.dtype == CUHPX_F64 ? run_fft_stage<double, true>(hp, (double*)const_cast<void*>(d_map), d_w, use_w, st)
+                                 : run_fft_stage<float, true>(hp, (float*)const_cast<void*>(d_map), d_w, use_w, st);
 }
 
 cudaError_t launch_fft_synthesis(const HostPlan& hp, void* d_map, const double* d_w, int use_w, cudaStream_t st) {
-    return hp.dtype == CUHPX_F64 ? run_fft_synthesis<double>(hp, d_map, d_w, use_w, st)
-                                 : run_fft_synthesis<float>(hp, d_map, d_w, use_w, st);
+    return hp.dtype == CUHPX_F64 ? run_fft_stage<double, false>(hp, (double*)d_map, d_w, use_w, st)
+                                 : run_fft_stage<float, false>(hp, (float*)d_map, d_w, use_w, st);
 }
 
 }  // namespace cuhpx
