@@ -10,6 +10,7 @@
 // registers.  cos(theta) enters as x p = p - y p with y = 1 - cos(theta) (R3).
 #include <cuda_runtime.h>
 #include <math.h>
+#include <stdlib.h>
 
 #include "cuhpx_internal.h"
 
@@ -405,6 +406,20 @@ __global__ void __launch_bounds__(NT, 512 / NT >= 3 ? 3 : 2) legendre_analysis_k
 // resident F tile (F_N + F_S for even l - m, F_N - F_S for odd) as a register-blocked SGEMM: warp = 32 rings of K,
 // thread = 4 degrees (one parity) x 4 columns, one LDS.128 of lambda + one of F per 16 FFMA; the 8 warps' partial
 // tiles meet in shared memory.  lambda is converted to fp32 once per (l, ring) for all 8 channels.
+// packed fp32 FMA of sm_100a (PTX fma.rn.f32x2 -> SASS FFMA2): d = {s * b.x + c.x, s * b.y + c.y} in one issue slot
+__device__ __forceinline__ float2 fma2(float s, float2 b, float2 c) {
+    float2 d;
+    asm("{\n\t.reg .b64 ra, rb, rc, rd;\n\t"
+        "mov.b64 ra, {%2, %2};\n\t"
+        "mov.b64 rb, {%3, %4};\n\t"
+        "mov.b64 rc, {%5, %6};\n\t"
+        "fma.rn.f32x2 rd, ra, rb, rc;\n\t"
+        "mov.b64 {%0, %1}, rd;\n\t}"
+        : "=f"(d.x), "=f"(d.y)
+        : "f"(s), "f"(b.x), "f"(b.y), "f"(c.x), "f"(c.y));
+    return d;
+}
+
 constexpr int GK = 256;    // ring pairs per CTA (= threads)
 constexpr int GTL = 32;    // degrees per tile
 constexpr int GROW = 20;   // floats per lambda row: 16 + 4 padding (conflict-free 16-byte stores at 80-byte pitch)
@@ -510,11 +525,9 @@ __global__ void __launch_bounds__(GK, 3) legendre_analysis_gemm_kernel(LegArgs a
             *reinterpret_cast<float4*>(&sLam[(1 * GK + tid) * GROW + 4 * q]) = make_float4(o[0], o[1], o[2], o[3]);
         }
         const bool any = __any_sync(0xffffffffu, sc == 0);  // also orders the warp's stores before its loads
-        float acc[4][4];
+        float2 acc[4][2];  // [degree][column pair]: packed FMAs (FFMA2), lambda is the broadcast scalar
 #pragma unroll
-        for (int x = 0; x < 4; ++x)
-#pragma unroll
-            for (int z = 0; z < 4; ++z) acc[x][z] = 0.f;
+        for (int x = 0; x < 4; ++x) acc[x][0] = acc[x][1] = make_float2(0.f, 0.f);
         if (any) {
             const float* lp = &sLam[(par * GK + warp * 32) * GROW + 4 * lquad];
             const float* fp = &sF[par][warp * 32][4 * cq];
@@ -522,17 +535,19 @@ __global__ void __launch_bounds__(GK, 3) legendre_analysis_gemm_kernel(LegArgs a
             for (int kk = 0; kk < 32; ++kk) {
                 const float4 l4 = *reinterpret_cast<const float4*>(lp + kk * GROW);
                 const float4 f4 = *reinterpret_cast<const float4*>(fp + kk * GNC);
-                const float lv[4] = {l4.x, l4.y, l4.z, l4.w}, fv[4] = {f4.x, f4.y, f4.z, f4.w};
+                const float lv[4] = {l4.x, l4.y, l4.z, l4.w};
+                const float2 f01 = make_float2(f4.x, f4.y), f23 = make_float2(f4.z, f4.w);
 #pragma unroll
-                for (int x = 0; x < 4; ++x)
-#pragma unroll
-                    for (int z = 0; z < 4; ++z) acc[x][z] = fmaf(lv[x], fv[z], acc[x][z]);
+                for (int x = 0; x < 4; ++x) {
+                    acc[x][0] = fma2(lv[x], f01, acc[x][0]);
+                    acc[x][1] = fma2(lv[x], f23, acc[x][1]);
+                }
             }
         }
         __syncwarp();  // the warp is done reading its lambda rows
 #pragma unroll
         for (int x = 0; x < 4; ++x)
-            *reinterpret_cast<float4*>(&wred[lane * 16 + 4 * x]) = make_float4(acc[x][0], acc[x][1], acc[x][2], acc[x][3]);
+            *reinterpret_cast<float4*>(&wred[lane * 16 + 4 * x]) = make_float4(acc[x][0].x, acc[x][0].y, acc[x][1].x, acc[x][1].y);
         __syncthreads();
 #pragma unroll
         for (int rep = 0; rep < 2; ++rep) {
@@ -725,6 +740,157 @@ __global__ void __launch_bounds__(NT) legendre_synthesis_kernel(LegArgs a) {
     }
 }
 
+// ------------------------------------------------------------------ synthesis, batched fp32 (row s1), packed FMAs
+// sm_100a has a packed fp32 FMA (PTX fma.rn.f32x2 -> SASS FFMA2: two FMAs per lane and issue slot, one operand may
+// be a broadcast scalar).  (re, im) of one channel is exactly such a pair: E/O[r][c] += lambda * a_lm[c] is ONE
+// instruction per (l, ring pair, channel), which leaves issue slots for the fp64 recurrence, the conversion and
+// the shared-memory broadcasts of a_lm.  Same walk and exponent windows as legendre_synthesis_kernel<float>.
+template <int BT, int R, int NT, int MINB>
+__global__ void __launch_bounds__(NT, MINB) legendre_synthesis_f32x2_kernel(LegArgs a) {
+    using T = float;
+    const DevPlan& P = a.p;
+    const int m = blockIdx.x;
+    const int chunk = blockIdx.y;
+    const int ch0 = blockIdx.z * BT;
+    const int tid = threadIdx.x;
+    const int jbase = P.jmin[m] + chunk * (NT * R);
+    if (jbase >= P.npairs) return;
+
+    __shared__ double sA[CT];
+    __shared__ __align__(16) float2 sAlm[CT][BT];
+
+    double cur[R], prev[R], y[R];
+    int sc[R];
+    float2 E[R][BT], O[R][BT];
+    const double pref_hi = P.pref_hi[m], pref_lo = P.pref_lo[m];
+#pragma unroll
+    for (int r = 0; r < R; ++r) {
+        const int j = jbase + tid + NT * r;
+#pragma unroll
+        for (int c = 0; c < BT; ++c) E[r][c] = O[r][c] = make_float2(0.f, 0.f);
+        if (j < P.npairs) {
+            y[r] = P.y[j];
+            lambda_seed<T>(m, pref_hi, pref_lo, P.ls_hi[j], P.ls_lo[j], cur[r], sc[r]);
+            prev[r] = 0.0;
+        } else {
+            y[r] = 1.0;
+            cur[r] = 0.0;
+            prev[r] = 0.0;
+            sc[r] = -1;
+        }
+    }
+    const T inscale = (a.adjoint && m > 0) ? 0.5f : 1.f;
+    const long long abase = (long long)m * (2LL * P.lmax + 1 - m) / 2;
+    const T* alm = reinterpret_cast<const T*>(a.in);
+    const int nl = P.lmax - m + 1;
+
+    constexpr int NP = (CT * BT * 2 + NT - 1) / NT;
+    double nA = 0.0, nScl[NP];
+    T nAlm[NP];
+    auto fetch = [&](int tn) {
+        nA = (tid < CT && tn + 1 + tid < nl) ? P.coef_alpha[abase + m + tn + 1 + tid] : 0.0;
+#pragma unroll
+        for (int q = 0; q < NP; ++q) {
+            const int e = tid + NT * q;
+            const int i = e / (BT * 2), c = (e / 2) % BT, ri = e & 1;
+            const int k = tn + i, ch = ch0 + c;
+            const bool ok = e < CT * BT * 2 && k < nl && ch < P.batch;
+            nScl[q] = ok ? P.coef_scale[abase + m + k] : 0.0;
+            nAlm[q] = ok ? alm[((size_t)ch * P.nalm + abase + m + k) * 2 + ri] : 0.f;
+        }
+    };
+    fetch(0);
+    float* sAlmf = reinterpret_cast<float*>(&sAlm[0][0]);
+    for (int t0 = 0; t0 < nl; t0 += CT) {
+        __syncthreads();  // previous tile fully consumed
+        if (tid < CT) sA[tid] = nA;
+#pragma unroll
+        for (int q = 0; q < NP; ++q) {
+            const int e = tid + NT * q;
+            if (e < CT * BT * 2) {
+                T v = (T)((double)inscale * nScl[q] * (double)nAlm[q]);  // a_lm s_l
+                if (m == 0 && (e & 1)) v = 0;                              // Im a_l0 is ignored
+                sAlmf[e] = v;
+            }
+        }
+        __syncthreads();
+        fetch(t0 + CT);
+        const int tend = min(CT, nl - t0);
+        for (int s0 = 0; s0 < tend; s0 += CHECK_EVERY) {
+            bool any = false;
+#pragma unroll
+            for (int r = 0; r < R; ++r) {
+                if (sc[r] < 0) {
+                    if (fabs(cur[r]) > pow2c(ScaleCfg<T>::THR)) {
+                        cur[r] *= pow2c(-ScaleCfg<T>::K);
+                        prev[r] *= pow2c(-ScaleCfg<T>::K);
+                        ++sc[r];
+                    }
+#pragma unroll
+                    for (int c = 0; c < BT; ++c) E[r][c] = O[r][c] = make_float2(0.f, 0.f);
+                }
+                any |= (sc[r] == 0);
+            }
+            const bool warp_active = __any_sync(0xffffffffu, any);
+            if (warp_active) {
+#pragma unroll
+                for (int i = 0; i < CHECK_EVERY; ++i) {
+                    const double A = sA[s0 + i];
+                    float2 al[BT];
+#pragma unroll
+                    for (int c = 0; c < BT; ++c) al[c] = sAlm[s0 + i][c];
+#pragma unroll
+                    for (int r = 0; r < R; ++r) {
+                        const float lam = (float)cur[r];
+#pragma unroll
+                        for (int c = 0; c < BT; ++c) {
+                            if ((i & 1) == 0) E[r][c] = fma2(lam, al[c], E[r][c]);
+                            else O[r][c] = fma2(lam, al[c], O[r][c]);
+                        }
+                        const double xl = fma(-y[r], cur[r], cur[r]);
+                        const double nx = fma(A, xl, -prev[r]);
+                        prev[r] = cur[r];
+                        cur[r] = nx;
+                    }
+                }
+            } else {
+#pragma unroll
+                for (int i = 0; i < CHECK_EVERY; ++i) {
+                    const double A = sA[s0 + i];
+#pragma unroll
+                    for (int r = 0; r < R; ++r) {
+                        const double xl = fma(-y[r], cur[r], cur[r]);
+                        const double nx = fma(A, xl, -prev[r]);
+                        prev[r] = cur[r];
+                        cur[r] = nx;
+                    }
+                }
+            }
+        }
+    }
+
+    float2* spectra = reinterpret_cast<float2*>(P.spectra);
+#pragma unroll
+    for (int r = 0; r < R; ++r) {
+        const int j = jbase + tid + NT * r;
+        if (j >= P.npairs) continue;
+        const int rn = j, rs = P.nrings - 1 - j;
+        const bool live = sc[r] == 0;
+#pragma unroll
+        for (int c = 0; c < BT; ++c) {
+            const int ch = ch0 + c;
+            if (ch >= P.batch) continue;
+            float2 gn = make_float2(0.f, 0.f), gs = gn;
+            if (live) {
+                gn = make_float2(E[r][c].x + O[r][c].x, E[r][c].y + O[r][c].y);
+                gs = make_float2(E[r][c].x - O[r][c].x, E[r][c].y - O[r][c].y);
+            }
+            spectra[((size_t)ch * P.nrings + rn) * P.mstride + m] = gn;
+            if (rs != rn) spectra[((size_t)ch * P.nrings + rs) * P.mstride + m] = gs;
+        }
+    }
+}
+
 // ------------------------------------------------------------------ launch configuration
 // R (ring pairs per thread) and LT (l values per reduction tile) per instantiation.
 template <typename T, int BT> struct LegCfg;
@@ -810,8 +976,39 @@ cudaError_t launch_legendre_analysis(const HostPlan& hp, void* d_alm, int adjoin
     return run_analysis<float, 1>(hp, d_alm, adjoint, st);
 }
 
+template <int BT, int R, int NT, int MINB>
+static cudaError_t run_synthesis_f32x2(const HostPlan& hp, const void* d_alm, int adjoint, cudaStream_t st) {
+    const DevPlan& P = hp.d;
+    LegArgs a;
+    a.p = P;
+    a.in = d_alm;
+    a.out = nullptr;
+    a.adjoint = adjoint;
+    a.to_partial = 0;
+    const int chunk = NT * R;
+    dim3 grid(P.mmax + 1, (P.npairs + chunk - 1) / chunk, (P.batch + BT - 1) / BT);
+    legendre_synthesis_f32x2_kernel<BT, R, NT, MINB><<<grid, NT, 0, st>>>(a);
+    return cudaGetLastError();
+}
+
+static int tune_variant(const char* name) {  // TUNING ONLY (removed once the configuration is fixed)
+    const char* v = getenv(name);
+    return v ? atoi(v) : -1;
+}
+
 cudaError_t launch_legendre_synthesis(const HostPlan& hp, const void* d_alm, int adjoint, cudaStream_t st) {
     if (hp.dtype == CUHPX_F64) return run_synthesis<double, 1>(hp, d_alm, adjoint, st);
+    if (hp.d.batch >= 4) {
+        switch (tune_variant("CUHPX_SYN_VARIANT")) {
+            case 1: return run_synthesis_f32x2<8, 2, 128, 4>(hp, d_alm, adjoint, st);
+            case 2: return run_synthesis_f32x2<8, 4, 128, 2>(hp, d_alm, adjoint, st);
+            case 3: return run_synthesis_f32x2<4, 4, 128, 3>(hp, d_alm, adjoint, st);
+            case 4: return run_synthesis_f32x2<4, 2, 256, 2>(hp, d_alm, adjoint, st);
+            case 5: return run_synthesis_f32x2<8, 2, 256, 2>(hp, d_alm, adjoint, st);
+            case 6: return run_synthesis_f32x2<8, 1, 256, 3>(hp, d_alm, adjoint, st);
+            default: break;
+        }
+    }
     // 8 channels per CTA pay off when there are few (m, ring chunk) CTAs to fill the GPU with (measured: cfg3 yes, cfg4 no)
     if (hp.d.batch >= 8 && hp.d.lmax < 1024) return run_synthesis<float, 8>(hp, d_alm, adjoint, st);
     if (hp.d.batch >= 4) return run_synthesis<float, 4>(hp, d_alm, adjoint, st);
