@@ -209,16 +209,16 @@ __device__ __forceinline__ void warp_reduce_split(T (&v)[NV], int lane) {
     }
 }
 
-template <typename T, int BT, int R, int LT, int NT>
-__global__ void __launch_bounds__(NT, 512 / NT >= 3 ? 3 : 2) legendre_analysis_kernel(LegArgs a) {
+template <typename T, int BT, int R, int LT, int NT, int GL = GROUP_L>
+__global__ void __launch_bounds__(NT, 384 / NT) legendre_analysis_kernel(LegArgs a) {
     using T2 = typename Vec2<T>::type;
     constexpr int NW = NT / 32;
     constexpr int NV = LT * BT * 2;
     constexpr int HV = NV / 2;
     constexpr int Q = HV >= 16 ? HV / 16 : 1;
     constexpr int SH = HV >= 16 ? 0 : (HV == 8 ? 1 : HV == 4 ? 2 : HV == 2 ? 3 : 4);
-    constexpr int TPG = GROUP_L / LT;  // tiles per group
-    static_assert(CHECK_EVERY % LT == 0 && CT % GROUP_L == 0 && GROUP_L % CHECK_EVERY == 0, "tile sizes");
+    constexpr int TPG = GL / LT;  // tiles per group
+    static_assert(CHECK_EVERY % LT == 0 && CT % GL == 0 && GL % CHECK_EVERY == 0, "tile sizes");
     static_assert(NV >= 4, "reduction tile");
     const DevPlan& P = a.p;
     const int m = blockIdx.x;
@@ -301,7 +301,7 @@ __global__ void __launch_bounds__(NT, 512 / NT >= 3 ? 3 : 2) legendre_analysis_k
         }
         __syncthreads();
         const int tend = min(CT, nl - t0);
-        for (int g0 = 0; g0 < tend; g0 += GROUP_L) {
+        for (int g0 = 0; g0 < tend; g0 += GL) {
             // s_l of this thread's output element, requested before the group's arithmetic
             double oscl[NOUT];
 #pragma unroll
@@ -571,6 +571,170 @@ __global__ void __launch_bounds__(GK, 3) legendre_analysis_gemm_kernel(LegArgs a
     }
 }
 
+// ------------------------------------------------------------------ analysis, batched fp32: 64-degree tiles
+// Same contraction as legendre_analysis_gemm_kernel with the shared-memory traffic per FMA halved (ncu on the
+// 32-degree version: 6 shared-memory wavefronts per 16 FFMA issue slots and warp -> the LSU, not the FMA pipe, was the
+// limit): a tile is 64 degrees (32 per parity), a thread owns 8 degrees x 4 columns (16 packed FMAs per ring from
+// two LDS.128 of lambda and one of F), the two parities of both tiles sit 16 / 64 bytes apart modulo the bank
+// period so that the half-warps of different parity never collide, and the per-warp partial tiles are exchanged
+// through a swizzled layout (conflict-free STS.128, two-wavefront LDS.64).
+constexpr int HTL = 64;                  // degrees per tile
+constexpr int HROW = HTL / 2 + 4;        // floats per lambda row: 32 degrees of one parity + 4 padding (144-byte pitch)
+constexpr int HPS = GK * HROW + 4;       // parity stride of the lambda tile (floats): + 16 bytes
+constexpr int HFS = GK * GNC + 16;       // parity stride of the F tile (floats): + 64 bytes
+constexpr size_t HSMEM = sizeof(float) * (2 * HPS + 2 * HFS) + sizeof(double) * 4 * HTL;
+
+__device__ __forceinline__ int hswz(int x, int ln) { return (x + (ln & 3) + 4 * ((ln >> 2) & 3) + 4 * (ln >> 4)) & 7; }
+
+__global__ void __launch_bounds__(GK, 2) legendre_analysis_gemm64_kernel(LegArgs a) {
+    const DevPlan& P = a.p;
+    const int m = blockIdx.x;
+    const int chunk = blockIdx.y;
+    const int ch0 = blockIdx.z * GNCH;
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const int jbase = P.jmin[m] + chunk * GK;
+    if (jbase >= P.npairs) return;
+
+    extern __shared__ __align__(16) unsigned char gemm_smem[];
+    float* sLam = reinterpret_cast<float*>(gemm_smem);  // [parity][ring][HROW]; rows reused for the cross-warp sums
+    float* sF = sLam + 2 * HPS;                         // [parity][ring][GNC]: F_N + F_S, F_N - F_S
+    double(*sA)[HTL] = reinterpret_cast<double(*)[HTL]>(sF + 2 * HFS);
+    double(*sS)[HTL] = sA + 2;  // outscale * s_l of the tile's degrees
+
+    const float2* spectra = reinterpret_cast<const float2*>(P.spectra);
+    const int j = jbase + tid;
+    const bool valid = j < P.npairs;
+    double cur = 0.0, prev = 0.0, y = 1.0;
+    int sc = -1;
+    {
+        float fsum[GNC], fdif[GNC];
+#pragma unroll
+        for (int c = 0; c < GNC; ++c) fsum[c] = fdif[c] = 0.f;
+        if (valid) {
+            y = P.y[j];
+            lambda_seed<float>(m, P.pref_hi[m], P.pref_lo[m], P.ls_hi[j], P.ls_lo[j], cur, sc);
+            const int rn = j, rs = P.nrings - 1 - j;
+#pragma unroll
+            for (int c = 0; c < GNCH; ++c) {
+                if (ch0 + c < P.batch) {
+                    const float2 fn = spectra[((size_t)(ch0 + c) * P.nrings + rn) * P.mstride + m];
+                    float2 fv = make_float2(0.f, 0.f);
+                    if (rs != rn) fv = spectra[((size_t)(ch0 + c) * P.nrings + rs) * P.mstride + m];
+                    fsum[2 * c] = fn.x + fv.x;
+                    fsum[2 * c + 1] = fn.y + fv.y;
+                    fdif[2 * c] = fn.x - fv.x;
+                    fdif[2 * c + 1] = fn.y - fv.y;
+                }
+            }
+        }
+#pragma unroll
+        for (int c = 0; c < GNC; c += 4) {
+            *reinterpret_cast<float4*>(&sF[tid * GNC + c]) = make_float4(fsum[c], fsum[c + 1], fsum[c + 2], fsum[c + 3]);
+            *reinterpret_cast<float4*>(&sF[HFS + tid * GNC + c]) = make_float4(fdif[c], fdif[c + 1], fdif[c + 2], fdif[c + 3]);
+        }
+    }
+    const double outscale = (a.adjoint && m > 0) ? 2.0 : 1.0;
+    const long long abase = (long long)m * (2LL * P.lmax + 1 - m) / 2;
+    float* out = reinterpret_cast<float*>(a.out);
+    if (a.to_partial) out += (size_t)chunk * P.batch * P.nalm * 2;
+    const int nl = P.lmax - m + 1;
+
+    if (tid < HTL) {
+        sA[0][tid] = (1 + tid < nl) ? P.coef_alpha[abase + m + 1 + tid] : 0.0;
+        sS[0][tid] = (tid < nl) ? outscale * P.coef_scale[abase + m + tid] : 0.0;
+    }
+    __syncthreads();
+
+    // contraction-phase coordinates: lane = (parity, degree octet, column quad)
+    const int dq = lane >> 2, cq = lane & 3, par = dq >> 2, oc = dq & 3;
+    const float* lp = sLam + par * HPS + (warp * 32) * HROW + 8 * oc;
+    const float* fp = sF + par * HFS + (warp * 32) * GNC + 4 * cq;
+    float* wred = sLam + (warp * 32) * HROW;  // this warp's partial tile (1024 floats), aliased on its own lambda rows
+
+    for (int t0 = 0, tb = 0; t0 < nl; t0 += HTL, tb ^= 1) {
+        if (tid < HTL) {  // alpha / scale of the next tile (visible after this tile's barriers)
+            sA[tb ^ 1][tid] = (t0 + HTL + 1 + tid < nl) ? P.coef_alpha[abase + m + t0 + HTL + 1 + tid] : 0.0;
+            sS[tb ^ 1][tid] = (t0 + HTL + tid < nl) ? outscale * P.coef_scale[abase + m + t0 + HTL + tid] : 0.0;
+        }
+        // ---- generate 64 degrees of this thread's ring
+#pragma unroll
+        for (int q = 0; q < HTL / 8; ++q) {
+            if (sc < 0 && fabs(cur) > pow2c(ScaleCfg<float>::THR)) {
+                cur *= pow2c(-ScaleCfg<float>::K);
+                prev *= pow2c(-ScaleCfg<float>::K);
+                ++sc;
+            }
+            float e[4], o[4];
+#pragma unroll
+            for (int p = 0; p < 4; ++p) {
+                e[p] = sc == 0 ? (float)cur : 0.f;
+                double xl = fma(-y, cur, cur);
+                double nx = fma(sA[tb][8 * q + 2 * p], xl, -prev);
+                prev = cur;
+                cur = nx;
+                o[p] = sc == 0 ? (float)cur : 0.f;
+                xl = fma(-y, cur, cur);
+                nx = fma(sA[tb][8 * q + 2 * p + 1], xl, -prev);
+                prev = cur;
+                cur = nx;
+            }
+            *reinterpret_cast<float4*>(&sLam[tid * HROW + 4 * q]) = make_float4(e[0], e[1], e[2], e[3]);
+            *reinterpret_cast<float4*>(&sLam[HPS + tid * HROW + 4 * q]) = make_float4(o[0], o[1], o[2], o[3]);
+        }
+        const bool any = __any_sync(0xffffffffu, sc == 0);  // also orders the warp's stores before its loads
+        float2 acc[8][2];
+#pragma unroll
+        for (int x = 0; x < 8; ++x) acc[x][0] = acc[x][1] = make_float2(0.f, 0.f);
+        if (any) {
+#pragma unroll 4
+            for (int kk = 0; kk < 32; ++kk) {
+                const float4 la = *reinterpret_cast<const float4*>(lp + kk * HROW);
+                const float4 lb = *reinterpret_cast<const float4*>(lp + kk * HROW + 4);
+                const float4 f4 = *reinterpret_cast<const float4*>(fp + kk * GNC);
+                const float lv[8] = {la.x, la.y, la.z, la.w, lb.x, lb.y, lb.z, lb.w};
+                const float2 f01 = make_float2(f4.x, f4.y), f23 = make_float2(f4.z, f4.w);
+#pragma unroll
+                for (int x = 0; x < 8; ++x) {
+                    acc[x][0] = fma2(lv[x], f01, acc[x][0]);
+                    acc[x][1] = fma2(lv[x], f23, acc[x][1]);
+                }
+            }
+        }
+        __syncwarp();  // the warp is done reading its lambda rows
+#pragma unroll
+        for (int x = 0; x < 8; ++x)
+            *reinterpret_cast<float4*>(&wred[lane * 32 + 4 * hswz(x, lane)]) =
+                make_float4(acc[x][0].x, acc[x][0].y, acc[x][1].x, acc[x][1].y);
+        __syncthreads();
+#pragma unroll
+        for (int rep = 0; rep < 2; ++rep) {
+            // 512 complex outputs of the tile: 4 consecutive degrees x 8 channels per warp-wide store (32-byte sectors)
+            const int idx = tid + GK * rep;
+            const int il = idx & 3, chl = (idx >> 2) & 7, ih = idx >> 5;
+            const int i = ih * 4 + il;  // l - m - t0
+            const int opar = i & 1, d = i >> 1, ooc = d >> 3, x = d & 7;
+            const int ln = (opar * 4 + ooc) * 4 + (chl >> 1);
+            const float* src = sLam + ln * 32 + 4 * hswz(x, ln) + 2 * (chl & 1);
+            float2 sum = make_float2(0.f, 0.f);
+#pragma unroll
+            for (int w = 0; w < GK / 32; ++w) {
+                const float2 v = *reinterpret_cast<const float2*>(src + (w * 32) * HROW);
+                sum.x += v.x;
+                sum.y += v.y;
+            }
+            const int ch = ch0 + chl;
+            const int k = t0 + i;
+            if (k < nl && ch < P.batch) {
+                const double s = sS[tb][i];
+                float2 o = make_float2((float)(s * (double)sum.x), (float)(s * (double)sum.y));
+                if (m == 0) o.y = 0.f;  // Im a_l0 is exactly zero
+                *reinterpret_cast<float2*>(&out[((size_t)ch * P.nalm + abase + m + k) * 2]) = o;
+            }
+        }
+        __syncthreads();  // partial tiles consumed before the next tile overwrites the lambda rows
+    }
+}
+
 // sum the per-chunk partial results: alm[b][idx] = sum_c partial[c][b][idx], c < nchunks(m)
 template <typename T>
 __global__ void combine_partials_kernel(DevPlan P, const T* __restrict__ partial, T* __restrict__ alm) {
@@ -644,6 +808,7 @@ __global__ void __launch_bounds__(NT) legendre_synthesis_kernel(LegArgs a) {
         }
     };
     fetch(0);
+    bool all_on = false;  // every ring pair of this warp is active (sc == 0)
     for (int t0 = 0; t0 < nl; t0 += CT) {
         __syncthreads();  // previous tile fully consumed
         if (tid < CT) sA[tid] = nA;
@@ -662,22 +827,27 @@ __global__ void __launch_bounds__(NT) legendre_synthesis_kernel(LegArgs a) {
         fetch(t0 + CT);
         const int tend = min(CT, nl - t0);
         for (int s0 = 0; s0 < tend; s0 += CHECK_EVERY) {
-            bool any = false;
+            bool warp_active = true;
+            if (!all_on) {  // warp-uniform: skipped for good once every ring pair of the warp is significant
+                bool any = false, all = true;
 #pragma unroll
-            for (int r = 0; r < R; ++r) {
-                if (sc[r] < 0) {
-                    if (fabs(cur[r]) > pow2c(ScaleCfg<T>::THR)) {
-                        cur[r] *= pow2c(-ScaleCfg<T>::K);
-                        prev[r] *= pow2c(-ScaleCfg<T>::K);
-                        ++sc[r];
+                for (int r = 0; r < R; ++r) {
+                    if (sc[r] < 0) {
+                        if (fabs(cur[r]) > pow2c(ScaleCfg<T>::THR)) {
+                            cur[r] *= pow2c(-ScaleCfg<T>::K);
+                            prev[r] *= pow2c(-ScaleCfg<T>::K);
+                            ++sc[r];
+                        }
+                        // whatever was accumulated while the ring was inactive is noise below 2^-200 / 2^-44: drop it
+#pragma unroll
+                        for (int c = 0; c < BT; ++c) E[r][c][0] = E[r][c][1] = O[r][c][0] = O[r][c][1] = 0;
                     }
-                    // whatever was accumulated while the ring was inactive is noise below 2^-200 / 2^-44: drop it
-#pragma unroll
-                    for (int c = 0; c < BT; ++c) E[r][c][0] = E[r][c][1] = O[r][c][0] = O[r][c][1] = 0;
+                    any |= (sc[r] == 0);
+                    all &= (sc[r] == 0);
                 }
-                any |= (sc[r] == 0);
+                warp_active = __any_sync(0xffffffffu, any);
+                all_on = __all_sync(0xffffffffu, all);
             }
-            const bool warp_active = __any_sync(0xffffffffu, any);
             if (warp_active) {
 #pragma unroll
                 for (int i = 0; i < CHECK_EVERY; ++i) {
@@ -800,6 +970,7 @@ __global__ void __launch_bounds__(NT, MINB) legendre_synthesis_f32x2_kernel(LegA
         }
     };
     fetch(0);
+    bool all_on = false;  // every ring pair of this warp is active (sc == 0)
     float* sAlmf = reinterpret_cast<float*>(&sAlm[0][0]);
     for (int t0 = 0; t0 < nl; t0 += CT) {
         __syncthreads();  // previous tile fully consumed
@@ -817,21 +988,26 @@ __global__ void __launch_bounds__(NT, MINB) legendre_synthesis_f32x2_kernel(LegA
         fetch(t0 + CT);
         const int tend = min(CT, nl - t0);
         for (int s0 = 0; s0 < tend; s0 += CHECK_EVERY) {
-            bool any = false;
+            bool warp_active = true;
+            if (!all_on) {  // warp-uniform: skipped for good once every ring pair of the warp is significant
+                bool any = false, all = true;
 #pragma unroll
-            for (int r = 0; r < R; ++r) {
-                if (sc[r] < 0) {
-                    if (fabs(cur[r]) > pow2c(ScaleCfg<T>::THR)) {
-                        cur[r] *= pow2c(-ScaleCfg<T>::K);
-                        prev[r] *= pow2c(-ScaleCfg<T>::K);
-                        ++sc[r];
+                for (int r = 0; r < R; ++r) {
+                    if (sc[r] < 0) {
+                        if (fabs(cur[r]) > pow2c(ScaleCfg<T>::THR)) {
+                            cur[r] *= pow2c(-ScaleCfg<T>::K);
+                            prev[r] *= pow2c(-ScaleCfg<T>::K);
+                            ++sc[r];
+                        }
+#pragma unroll
+                        for (int c = 0; c < BT; ++c) E[r][c] = O[r][c] = make_float2(0.f, 0.f);
                     }
-#pragma unroll
-                    for (int c = 0; c < BT; ++c) E[r][c] = O[r][c] = make_float2(0.f, 0.f);
+                    any |= (sc[r] == 0);
+                    all &= (sc[r] == 0);
                 }
-                any |= (sc[r] == 0);
+                warp_active = __any_sync(0xffffffffu, any);
+                all_on = __all_sync(0xffffffffu, all);
             }
-            const bool warp_active = __any_sync(0xffffffffu, any);
             if (warp_active) {
 #pragma unroll
                 for (int i = 0; i < CHECK_EVERY; ++i) {
@@ -945,6 +1121,47 @@ static cudaError_t run_synthesis(const HostPlan& hp, const void* d_alm, int adjo
     return cudaGetLastError();
 }
 
+static int tune_variant(const char* name) {  // TUNING ONLY (removed once the configuration is fixed)
+    const char* v = getenv(name);
+    return v ? atoi(v) : -1;
+}
+
+template <typename T, int BT, int R, int LT, int NT, int GL>
+static cudaError_t run_analysis_cfg(const HostPlan& hp, void* d_alm, int adjoint, cudaStream_t st) {
+    const DevPlan& P = hp.d;
+    LegArgs a;
+    a.p = P;
+    a.in = nullptr;
+    a.adjoint = adjoint;
+    a.to_partial = P.nchunk_max > 1;
+    a.out = a.to_partial ? P.partial : d_alm;
+    dim3 grid(P.mmax + 1, P.nchunk_max, (P.batch + BT - 1) / BT);
+    legendre_analysis_kernel<T, BT, R, LT, NT, GL><<<grid, NT, 0, st>>>(a);
+    cudaError_t e = cudaGetLastError();
+    if (e != cudaSuccess) return e;
+    if (a.to_partial) {
+        dim3 g2(P.mmax + 1, P.batch);
+        combine_partials_kernel<T><<<g2, 256, 0, st>>>(P, reinterpret_cast<const T*>(P.partial), reinterpret_cast<T*>(d_alm));
+        e = cudaGetLastError();
+    }
+    return e;
+}
+
+template <typename T, int BT, int RS, int NTS>
+static cudaError_t run_synthesis_cfg(const HostPlan& hp, const void* d_alm, int adjoint, cudaStream_t st) {
+    const DevPlan& P = hp.d;
+    LegArgs a;
+    a.p = P;
+    a.in = d_alm;
+    a.out = nullptr;
+    a.adjoint = adjoint;
+    a.to_partial = 0;
+    const int chunk = NTS * RS;
+    dim3 grid(P.mmax + 1, (P.npairs + chunk - 1) / chunk, (P.batch + BT - 1) / BT);
+    legendre_synthesis_kernel<T, BT, RS, NTS><<<grid, NTS, 0, st>>>(a);
+    return cudaGetLastError();
+}
+
 static cudaError_t run_analysis_gemm(const HostPlan& hp, void* d_alm, int adjoint, cudaStream_t st) {
     const DevPlan& P = hp.d;
     LegArgs a;
@@ -957,7 +1174,13 @@ static cudaError_t run_analysis_gemm(const HostPlan& hp, void* d_alm, int adjoin
     constexpr size_t smem = sizeof(float) * (2 * GK * GROW + 2 * GK * GNC) + sizeof(double) * 4 * GTL;
     cudaError_t e = cudaFuncSetAttribute(legendre_analysis_gemm_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return e;
-    legendre_analysis_gemm_kernel<<<grid, GK, smem, st>>>(a);
+    if (tune_variant("CUHPX_ANA_VARIANT") == 1) {
+        legendre_analysis_gemm_kernel<<<grid, GK, smem, st>>>(a);
+    } else {
+        e = cudaFuncSetAttribute(legendre_analysis_gemm64_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)HSMEM);
+        if (e != cudaSuccess) return e;
+        legendre_analysis_gemm64_kernel<<<grid, GK, HSMEM, st>>>(a);
+    }
     e = cudaGetLastError();
     if (e != cudaSuccess) return e;
     if (a.to_partial) {
@@ -970,7 +1193,14 @@ static cudaError_t run_analysis_gemm(const HostPlan& hp, void* d_alm, int adjoin
 }
 
 cudaError_t launch_legendre_analysis(const HostPlan& hp, void* d_alm, int adjoint, cudaStream_t st) {
-    if (hp.dtype == CUHPX_F64) return run_analysis<double, 1>(hp, d_alm, adjoint, st);
+    if (hp.dtype == CUHPX_F64) {
+        switch (tune_variant("CUHPX_ANA64_VARIANT")) {
+            case 1: return run_analysis_cfg<double, 1, 8, 8, 128, 64>(hp, d_alm, adjoint, st);
+            case 2: return run_analysis_cfg<double, 1, 8, 4, 128, 32>(hp, d_alm, adjoint, st);
+            case 3: return run_analysis_cfg<double, 1, 8, 4, 128, 64>(hp, d_alm, adjoint, st);
+            default: return run_analysis<double, 1>(hp, d_alm, adjoint, st);
+        }
+    }
     if (hp.d.batch >= 5) return run_analysis_gemm(hp, d_alm, adjoint, st);
     if (hp.d.batch >= 4) return run_analysis<float, 4>(hp, d_alm, adjoint, st);
     return run_analysis<float, 1>(hp, d_alm, adjoint, st);
@@ -991,13 +1221,16 @@ static cudaError_t run_synthesis_f32x2(const HostPlan& hp, const void* d_alm, in
     return cudaGetLastError();
 }
 
-static int tune_variant(const char* name) {  // TUNING ONLY (removed once the configuration is fixed)
-    const char* v = getenv(name);
-    return v ? atoi(v) : -1;
-}
-
 cudaError_t launch_legendre_synthesis(const HostPlan& hp, const void* d_alm, int adjoint, cudaStream_t st) {
-    if (hp.dtype == CUHPX_F64) return run_synthesis<double, 1>(hp, d_alm, adjoint, st);
+    if (hp.dtype == CUHPX_F64) {
+        switch (tune_variant("CUHPX_SYN64_VARIANT")) {
+            case 1: return run_synthesis_cfg<double, 1, 8, 128>(hp, d_alm, adjoint, st);
+            case 2: return run_synthesis_cfg<double, 1, 4, 128>(hp, d_alm, adjoint, st);
+            case 3: return run_synthesis_cfg<double, 1, 6, 128>(hp, d_alm, adjoint, st);
+            case 4: return run_synthesis_cfg<double, 1, 2, 256>(hp, d_alm, adjoint, st);
+            default: return run_synthesis<double, 1>(hp, d_alm, adjoint, st);
+        }
+    }
     if (hp.d.batch >= 4) {
         switch (tune_variant("CUHPX_SYN_VARIANT")) {
             case 1: return run_synthesis_f32x2<8, 2, 128, 4>(hp, d_alm, adjoint, st);
@@ -1006,7 +1239,10 @@ cudaError_t launch_legendre_synthesis(const HostPlan& hp, const void* d_alm, int
             case 4: return run_synthesis_f32x2<4, 2, 256, 2>(hp, d_alm, adjoint, st);
             case 5: return run_synthesis_f32x2<8, 2, 256, 2>(hp, d_alm, adjoint, st);
             case 6: return run_synthesis_f32x2<8, 1, 256, 3>(hp, d_alm, adjoint, st);
-            default: break;
+            case 0: break;
+            default:
+                if (hp.d.batch >= 8) return run_synthesis_f32x2<8, 2, 128, 4>(hp, d_alm, adjoint, st);
+                break;
         }
     }
     // 8 channels per CTA pay off when there are few (m, ring chunk) CTAs to fill the GPU with (measured: cfg3 yes, cfg4 no)
