@@ -90,6 +90,17 @@ int cuhpx_map2alm_adjoint(int nside, int lmax, int mmax, int batch, cuhpx_dtype_
                           void* d_gmap, const double* d_ring_weights, void* d_workspace, size_t workspace_bytes,
                           cuhpx_stream_t stream);
 
+/* ---- iterative refinement of the analysis (Eq. 4; the paper's "future work")
+ *   a^(0) = A f;   r^(k+1) = f - S a^(k);   a^(k+1) = a^(k) + A r^(k+1),   k = 0 .. n_iter - 1
+ * with A = cuhpx_map2alm (ring weights as given) and S = cuhpx_alm2map.  n_iter = 0 is cuhpx_map2alm.  Each
+ * iteration costs one synthesis and one analysis.  d_scratch_map ([batch][npix] real) and d_scratch_alm
+ * ([batch][nalm] complex) are caller-owned scratch buffers of the transform's dtype, overwritten; on return
+ * d_scratch_map holds the last residual r^(n_iter) (undefined for n_iter = 0).  Same conventions and error codes as
+ * the four operators; n_iter < 0 or a null scratch pointer with n_iter > 0 is CUHPX_EINVAL. */
+int cuhpx_map2alm_iter(int nside, int lmax, int mmax, int batch, cuhpx_dtype_t dtype, const void* d_map, void* d_alm,
+                       const double* d_ring_weights, int n_iter, void* d_scratch_map, void* d_scratch_alm,
+                       void* d_workspace, size_t workspace_bytes, cuhpx_stream_t stream);
+
 /* ---- the two stages of each direction, individually, for per-stage
  * measurement and stage-level parity tests.  The ring spectra live inside the workspace:
  *   spectra[b][ring][m], m = 0..m_cut(ring) (entries above m_cut(ring) are neither written nor read: there

@@ -171,6 +171,17 @@ def map2alm_adjoint(nside: int, lmax: int, mmax: int, galm, ring_weights=None) -
     return out
 
 
+def map2alm_iter(nside: int, lmax: int, mmax: int, hmap, n_iter: int, ring_weights=None) -> np.ndarray:
+    """Iterative refinement of the analysis, Eq. 4 step by step in the paper's notation:
+    a^(0) = A f;  r^(k+1) = f - S a^(k);  a^(k+1) = a^(k) + A r^(k+1)."""
+    f = _f64(hmap)
+    a = map2alm(nside, lmax, mmax, f, ring_weights)
+    for _ in range(n_iter):
+        r = f - alm2map(nside, lmax, mmax, a)
+        a = a + map2alm(nside, lmax, mmax, r, ring_weights)
+    return a
+
+
 def map2alm_subset(nside, lmax, mmax, hmap, sel_l, sel_m, ring_weights=None) -> np.ndarray:
     hmap = _f64(hmap)
     sel_l, sel_m = _i32(sel_l), _i32(sel_m)

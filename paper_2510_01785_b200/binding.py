@@ -24,6 +24,7 @@ EXPORTS = [
     "cuhpx_alm2map_adjoint", "cuhpx_map2alm_adjoint", "cuhpx_spectra_stride", "cuhpx_workspace_spectra",
     "cuhpx_workspace_mcut", "cuhpx_analysis_fft_stage", "cuhpx_analysis_legendre_stage",
     "cuhpx_synthesis_legendre_stage", "cuhpx_synthesis_fft_stage", "cuhpx_fma_peak_probe", "cuhpx_workspace_stats",
+    "cuhpx_map2alm_iter",
 ]
 
 
@@ -59,6 +60,7 @@ def _load() -> ctypes.CDLL:
     lib.cuhpx_alm2map.argtypes = [i, i, i, i, i, vp, vp, vp, sz, vp]
     lib.cuhpx_alm2map_adjoint.argtypes = [i, i, i, i, i, vp, vp, vp, sz, vp]
     lib.cuhpx_map2alm_adjoint.argtypes = [i, i, i, i, i, vp, vp, vp, vp, sz, vp]
+    lib.cuhpx_map2alm_iter.argtypes = [i, i, i, i, i, vp, vp, vp, i, vp, vp, vp, sz, vp]
     lib.cuhpx_spectra_stride.restype = sz
     lib.cuhpx_spectra_stride.argtypes = [i]
     lib.cuhpx_workspace_spectra.restype = vp
@@ -161,6 +163,14 @@ def cuhpx_map2alm(nside, lmax, mmax, batch, dtype, d_map, d_alm, d_ring_weights,
     p, n = _ws_args(workspace)
     _check(_lib.cuhpx_map2alm(nside, lmax, mmax, batch, dtype, _dev_ptr(d_map), _dev_ptr(d_alm),
                               _dev_ptr(d_ring_weights), p, n, _stream_ptr(stream)), "cuhpx_map2alm")
+
+
+def cuhpx_map2alm_iter(nside, lmax, mmax, batch, dtype, d_map, d_alm, d_ring_weights, n_iter, d_scratch_map,
+                       d_scratch_alm, workspace, stream=None) -> None:
+    p, n = _ws_args(workspace)
+    _check(_lib.cuhpx_map2alm_iter(nside, lmax, mmax, batch, dtype, _dev_ptr(d_map), _dev_ptr(d_alm),
+                                   _dev_ptr(d_ring_weights), int(n_iter), _dev_ptr(d_scratch_map),
+                                   _dev_ptr(d_scratch_alm), p, n, _stream_ptr(stream)), "cuhpx_map2alm_iter")
 
 
 def cuhpx_alm2map(nside, lmax, mmax, batch, dtype, d_alm, d_map, workspace, stream=None) -> None:
@@ -269,6 +279,15 @@ class Transform:
         assert hmap.shape == (self.batch, self.npix) and hmap.dtype == self.rdtype
         alm = torch.empty(self.batch, self.nalm, dtype=self.cdtype, device=self.device) if out is None else out
         cuhpx_map2alm(*self._args(), hmap, alm, self.ring_weights, self.workspace)
+        return alm
+
+    def map2alm_iter(self, hmap: torch.Tensor, n_iter: int, out: torch.Tensor | None = None) -> torch.Tensor:
+        """Analysis with n_iter refinement iterations a <- a + A (f - S a) (Eq. 4)."""
+        assert hmap.shape == (self.batch, self.npix) and hmap.dtype == self.rdtype
+        alm = torch.empty(self.batch, self.nalm, dtype=self.cdtype, device=self.device) if out is None else out
+        smap = torch.empty_like(hmap) if n_iter > 0 else None
+        salm = torch.empty_like(alm) if n_iter > 0 else None
+        cuhpx_map2alm_iter(*self._args(), hmap, alm, self.ring_weights, n_iter, smap, salm, self.workspace)
         return alm
 
     def alm2map(self, alm: torch.Tensor, out: torch.Tensor | None = None) -> torch.Tensor:

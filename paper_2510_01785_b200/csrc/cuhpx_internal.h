@@ -87,6 +87,10 @@ bool fft_supported(int nside, cuhpx_dtype_t dt);
 // launches per FFT-stage call and bytes of constant tables it reads
 void fft_stage_stats(const HostPlan& hp, int* launches, double* table_bytes);
 
+// elementwise steps of the iterative refinement (Eq. 4): r[i] = f[i] - r[i];  a[i] += d[i]
+cudaError_t launch_residual(cuhpx_dtype_t dt, const void* f, void* r, size_t n, cudaStream_t st);
+cudaError_t launch_accumulate(cuhpx_dtype_t dt, const void* d, void* a, size_t n, cudaStream_t st);
+
 cudaError_t fma_peak_probe(cuhpx_dtype_t dt, int iters, float* ms, double* count, cudaStream_t st);
 
 }  // namespace cuhpx

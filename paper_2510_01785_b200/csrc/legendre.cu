@@ -604,14 +604,16 @@ __global__ void __launch_bounds__(GK, 2) legendre_analysis_gemm64_kernel(LegArgs
     const float2* spectra = reinterpret_cast<const float2*>(P.spectra);
     const int j = jbase + tid;
     const bool valid = j < P.npairs;
-    double cur = 0.0, prev = 0.0, y = 1.0;
+    // fp32 output: cos(theta) = 1 - y rounded to double is accurate enough (the y-form of DESIGN.md R3 is for the
+    // 1e-11 bar), and alpha_l x is off the dependent chain: ONE fp64 FMA of latency per degree instead of two
+    double cur = 0.0, prev = 0.0, cx = 0.0;
     int sc = -1;
     {
         float fsum[GNC], fdif[GNC];
 #pragma unroll
         for (int c = 0; c < GNC; ++c) fsum[c] = fdif[c] = 0.f;
         if (valid) {
-            y = P.y[j];
+            cx = 1.0 - P.y[j];
             lambda_seed<float>(m, P.pref_hi[m], P.pref_lo[m], P.ls_hi[j], P.ls_lo[j], cur, sc);
             const int rn = j, rs = P.nrings - 1 - j;
 #pragma unroll
@@ -651,37 +653,61 @@ __global__ void __launch_bounds__(GK, 2) legendre_analysis_gemm64_kernel(LegArgs
     const float* fp = sF + par * HFS + (warp * 32) * GNC + 4 * cq;
     float* wred = sLam + (warp * 32) * HROW;  // this warp's partial tile (1024 floats), aliased on its own lambda rows
 
+    bool all_on = false;  // warp-uniform: every ring of this warp is significant (sc == 0)
     for (int t0 = 0, tb = 0; t0 < nl; t0 += HTL, tb ^= 1) {
-        if (tid < HTL) {  // alpha / scale of the next tile (visible after this tile's barriers)
-            sA[tb ^ 1][tid] = (t0 + HTL + 1 + tid < nl) ? P.coef_alpha[abase + m + t0 + HTL + 1 + tid] : 0.0;
-            sS[tb ^ 1][tid] = (t0 + HTL + tid < nl) ? outscale * P.coef_scale[abase + m + t0 + HTL + tid] : 0.0;
+        // alpha / scale of the next tile: requested now, parked in shared memory after the contraction (a store right
+        // here would stall warps 0-1 for the full global-load latency in every tile, and the CTA with them)
+        double nA = 0.0, nS = 0.0;
+        if (tid < HTL) {
+            nA = (t0 + HTL + 1 + tid < nl) ? P.coef_alpha[abase + m + t0 + HTL + 1 + tid] : 0.0;
+            nS = (t0 + HTL + tid < nl) ? outscale * P.coef_scale[abase + m + t0 + HTL + tid] : 0.0;
         }
         // ---- generate 64 degrees of this thread's ring
+        if (all_on) {  // every ring of the warp is significant: no rescale checks, no selects
 #pragma unroll
-        for (int q = 0; q < HTL / 8; ++q) {
-            if (sc < 0 && fabs(cur) > pow2c(ScaleCfg<float>::THR)) {
-                cur *= pow2c(-ScaleCfg<float>::K);
-                prev *= pow2c(-ScaleCfg<float>::K);
-                ++sc;
-            }
-            float e[4], o[4];
+            for (int q = 0; q < HTL / 8; ++q) {
+                float e[4], o[4];
 #pragma unroll
-            for (int p = 0; p < 4; ++p) {
-                e[p] = sc == 0 ? (float)cur : 0.f;
-                double xl = fma(-y, cur, cur);
-                double nx = fma(sA[tb][8 * q + 2 * p], xl, -prev);
-                prev = cur;
-                cur = nx;
-                o[p] = sc == 0 ? (float)cur : 0.f;
-                xl = fma(-y, cur, cur);
-                nx = fma(sA[tb][8 * q + 2 * p + 1], xl, -prev);
-                prev = cur;
-                cur = nx;
+                for (int p = 0; p < 4; ++p) {
+                    e[p] = (float)cur;
+                    double nx = fma(sA[tb][8 * q + 2 * p] * cx, cur, -prev);
+                    prev = cur;
+                    cur = nx;
+                    o[p] = (float)cur;
+                    nx = fma(sA[tb][8 * q + 2 * p + 1] * cx, cur, -prev);
+                    prev = cur;
+                    cur = nx;
+                }
+                *reinterpret_cast<float4*>(&sLam[tid * HROW + 4 * q]) = make_float4(e[0], e[1], e[2], e[3]);
+                *reinterpret_cast<float4*>(&sLam[HPS + tid * HROW + 4 * q]) = make_float4(o[0], o[1], o[2], o[3]);
             }
-            *reinterpret_cast<float4*>(&sLam[tid * HROW + 4 * q]) = make_float4(e[0], e[1], e[2], e[3]);
-            *reinterpret_cast<float4*>(&sLam[HPS + tid * HROW + 4 * q]) = make_float4(o[0], o[1], o[2], o[3]);
+        } else {
+#pragma unroll
+            for (int q = 0; q < HTL / 8; ++q) {
+                if (sc < 0 && fabs(cur) > pow2c(ScaleCfg<float>::THR)) {
+                    cur *= pow2c(-ScaleCfg<float>::K);
+                    prev *= pow2c(-ScaleCfg<float>::K);
+                    ++sc;
+                }
+                float e[4], o[4];
+#pragma unroll
+                for (int p = 0; p < 4; ++p) {
+                    e[p] = sc == 0 ? (float)cur : 0.f;
+                    double nx = fma(sA[tb][8 * q + 2 * p] * cx, cur, -prev);
+                    prev = cur;
+                    cur = nx;
+                    o[p] = sc == 0 ? (float)cur : 0.f;
+                    nx = fma(sA[tb][8 * q + 2 * p + 1] * cx, cur, -prev);
+                    prev = cur;
+                    cur = nx;
+                }
+                *reinterpret_cast<float4*>(&sLam[tid * HROW + 4 * q]) = make_float4(e[0], e[1], e[2], e[3]);
+                *reinterpret_cast<float4*>(&sLam[HPS + tid * HROW + 4 * q]) = make_float4(o[0], o[1], o[2], o[3]);
+            }
+            all_on = __all_sync(0xffffffffu, sc == 0);
         }
-        const bool any = __any_sync(0xffffffffu, sc == 0);  // also orders the warp's stores before its loads
+        const bool any = all_on || __any_sync(0xffffffffu, sc == 0);
+        __syncwarp();  // orders the warp's lambda stores before its loads
         float2 acc[8][2];
 #pragma unroll
         for (int x = 0; x < 8; ++x) acc[x][0] = acc[x][1] = make_float2(0.f, 0.f);
@@ -701,6 +727,10 @@ __global__ void __launch_bounds__(GK, 2) legendre_analysis_gemm64_kernel(LegArgs
             }
         }
         __syncwarp();  // the warp is done reading its lambda rows
+        if (tid < HTL) {
+            sA[tb ^ 1][tid] = nA;
+            sS[tb ^ 1][tid] = nS;
+        }
 #pragma unroll
         for (int x = 0; x < 8; ++x)
             *reinterpret_cast<float4*>(&wred[lane * 32 + 4 * hswz(x, lane)]) =
@@ -915,6 +945,13 @@ __global__ void __launch_bounds__(NT) legendre_synthesis_kernel(LegArgs a) {
 // be a broadcast scalar).  (re, im) of one channel is exactly such a pair: E/O[r][c] += lambda * a_lm[c] is ONE
 // instruction per (l, ring pair, channel), which leaves issue slots for the fp64 recurrence, the conversion and
 // the shared-memory broadcasts of a_lm.  Same walk and exponent windows as legendre_synthesis_kernel<float>.
+// 8-byte asynchronous copy global -> shared memory (LDGSTS): the data never passes through registers
+__device__ __forceinline__ void cp_async8(void* smem_dst, const void* gmem_src) {
+    asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" ::"r"((unsigned)__cvta_generic_to_shared(smem_dst)), "l"(gmem_src) : "memory");
+}
+__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
+__device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wait_group 0;" ::: "memory"); }
+
 template <int BT, int R, int NT, int MINB>
 __global__ void __launch_bounds__(NT, MINB) legendre_synthesis_f32x2_kernel(LegArgs a) {
     using T = float;
@@ -928,6 +965,8 @@ __global__ void __launch_bounds__(NT, MINB) legendre_synthesis_f32x2_kernel(LegA
 
     __shared__ double sA[CT];
     __shared__ __align__(16) float2 sAlm[CT][BT];
+    __shared__ __align__(16) float2 rAlm[CT][BT];  // staging (cp.async targets): raw a_lm, s_l, alpha of the next tile
+    __shared__ double rScl[CT], rA[CT];
 
     double cur[R], prev[R], y[R];
     int sc[R];
@@ -939,11 +978,12 @@ __global__ void __launch_bounds__(NT, MINB) legendre_synthesis_f32x2_kernel(LegA
 #pragma unroll
         for (int c = 0; c < BT; ++c) E[r][c] = O[r][c] = make_float2(0.f, 0.f);
         if (j < P.npairs) {
-            y[r] = P.y[j];
+            y[r] = 1.0 - P.y[j];  // cos(theta): fp32 output does not need the y-form (R3); alpha_l cos(theta) is
+                                  // off the dependent chain, which is then one fp64 FMA per degree
             lambda_seed<T>(m, pref_hi, pref_lo, P.ls_hi[j], P.ls_lo[j], cur[r], sc[r]);
             prev[r] = 0.0;
         } else {
-            y[r] = 1.0;
+            y[r] = 0.0;
             cur[r] = 0.0;
             prev[r] = 0.0;
             sc[r] = -1;
@@ -954,38 +994,48 @@ __global__ void __launch_bounds__(NT, MINB) legendre_synthesis_f32x2_kernel(LegA
     const T* alm = reinterpret_cast<const T*>(a.in);
     const int nl = P.lmax - m + 1;
 
-    constexpr int NP = (CT * BT * 2 + NT - 1) / NT;
-    double nA = 0.0, nScl[NP];
-    T nAlm[NP];
-    auto fetch = [&](int tn) {
-        nA = (tid < CT && tn + 1 + tid < nl) ? P.coef_alpha[abase + m + tn + 1 + tid] : 0.0;
+    // Tile t0 + CT travels global -> shared memory by cp.async while tile t0 is consumed: no registers are held
+    // across the arithmetic (a register prefetch was spilled by ptxas, and the spill store waited for the load).
+    // A thread owns ONE degree of the tile (one s_l) and CPT channels of it.
+    constexpr int TPL = NT / CT, CPT = BT / TPL;
+    static_assert(NT % CT == 0 && BT % TPL == 0 && NT >= 2 * CT, "staging mapping");
+    const int fi = tid / TPL, fc0 = (tid % TPL) * CPT;
+    auto request = [&](int tn) {
+        const int k = tn + fi;
 #pragma unroll
-        for (int q = 0; q < NP; ++q) {
-            const int e = tid + NT * q;
-            const int i = e / (BT * 2), c = (e / 2) % BT, ri = e & 1;
-            const int k = tn + i, ch = ch0 + c;
-            const bool ok = e < CT * BT * 2 && k < nl && ch < P.batch;
-            nScl[q] = ok ? P.coef_scale[abase + m + k] : 0.0;
-            nAlm[q] = ok ? alm[((size_t)ch * P.nalm + abase + m + k) * 2 + ri] : 0.f;
+        for (int q = 0; q < CPT; ++q) {
+            const int ch = ch0 + fc0 + q;
+            if (k < nl && ch < P.batch) cp_async8(&rAlm[fi][fc0 + q], &alm[((size_t)ch * P.nalm + abase + m + k) * 2]);
+            else rAlm[fi][fc0 + q] = make_float2(0.f, 0.f);
         }
+        if (tid < CT) {
+            if (tn + 1 + tid < nl) cp_async8(&rA[tid], &P.coef_alpha[abase + m + tn + 1 + tid]);
+            else rA[tid] = 0.0;
+        } else if (tid < 2 * CT) {
+            const int i = tid - CT;
+            if (tn + i < nl) cp_async8(&rScl[i], &P.coef_scale[abase + m + tn + i]);
+            else rScl[i] = 0.0;
+        }
+        cp_async_commit();
     };
-    fetch(0);
+    request(0);
     bool all_on = false;  // every ring pair of this warp is active (sc == 0)
-    float* sAlmf = reinterpret_cast<float*>(&sAlm[0][0]);
     for (int t0 = 0; t0 < nl; t0 += CT) {
-        __syncthreads();  // previous tile fully consumed
-        if (tid < CT) sA[tid] = nA;
+        cp_async_wait_all();
+        __syncthreads();  // staged tile landed; previous tile fully consumed
+        if (tid < CT) sA[tid] = rA[tid];
+        {
+            const float sl = (float)((double)inscale * rScl[fi]);  // a_lm s_l: the kernel sums mu_l = lambda_l / s_l
 #pragma unroll
-        for (int q = 0; q < NP; ++q) {
-            const int e = tid + NT * q;
-            if (e < CT * BT * 2) {
-                T v = (T)((double)inscale * nScl[q] * (double)nAlm[q]);  // a_lm s_l
-                if (m == 0 && (e & 1)) v = 0;                              // Im a_l0 is ignored
-                sAlmf[e] = v;
+            for (int q = 0; q < CPT; ++q) {
+                const float2 r = rAlm[fi][fc0 + q];
+                float2 v = make_float2(sl * r.x, sl * r.y);
+                if (m == 0) v.y = 0.f;  // Im a_l0 is ignored
+                sAlm[fi][fc0 + q] = v;
             }
         }
         __syncthreads();
-        fetch(t0 + CT);
+        request(t0 + CT);
         const int tend = min(CT, nl - t0);
         for (int s0 = 0; s0 < tend; s0 += CHECK_EVERY) {
             bool warp_active = true;
@@ -1023,8 +1073,7 @@ __global__ void __launch_bounds__(NT, MINB) legendre_synthesis_f32x2_kernel(LegA
                             if ((i & 1) == 0) E[r][c] = fma2(lam, al[c], E[r][c]);
                             else O[r][c] = fma2(lam, al[c], O[r][c]);
                         }
-                        const double xl = fma(-y[r], cur[r], cur[r]);
-                        const double nx = fma(A, xl, -prev[r]);
+                        const double nx = fma(A * y[r], cur[r], -prev[r]);  // y[] holds cos(theta) here
                         prev[r] = cur[r];
                         cur[r] = nx;
                     }
@@ -1035,8 +1084,7 @@ __global__ void __launch_bounds__(NT, MINB) legendre_synthesis_f32x2_kernel(LegA
                     const double A = sA[s0 + i];
 #pragma unroll
                     for (int r = 0; r < R; ++r) {
-                        const double xl = fma(-y[r], cur[r], cur[r]);
-                        const double nx = fma(A, xl, -prev[r]);
+                        const double nx = fma(A * y[r], cur[r], -prev[r]);  // y[] holds cos(theta) here
                         prev[r] = cur[r];
                         cur[r] = nx;
                     }
@@ -1198,7 +1246,8 @@ cudaError_t launch_legendre_analysis(const HostPlan& hp, void* d_alm, int adjoin
             case 1: return run_analysis_cfg<double, 1, 8, 8, 128, 64>(hp, d_alm, adjoint, st);
             case 2: return run_analysis_cfg<double, 1, 8, 4, 128, 32>(hp, d_alm, adjoint, st);
             case 3: return run_analysis_cfg<double, 1, 8, 4, 128, 64>(hp, d_alm, adjoint, st);
-            default: return run_analysis<double, 1>(hp, d_alm, adjoint, st);
+            case 0: return run_analysis<double, 1>(hp, d_alm, adjoint, st);
+            default: return run_analysis_cfg<double, 1, 8, 8, 128, 64>(hp, d_alm, adjoint, st);
         }
     }
     if (hp.d.batch >= 5) return run_analysis_gemm(hp, d_alm, adjoint, st);
@@ -1228,7 +1277,8 @@ cudaError_t launch_legendre_synthesis(const HostPlan& hp, const void* d_alm, int
             case 2: return run_synthesis_cfg<double, 1, 4, 128>(hp, d_alm, adjoint, st);
             case 3: return run_synthesis_cfg<double, 1, 6, 128>(hp, d_alm, adjoint, st);
             case 4: return run_synthesis_cfg<double, 1, 2, 256>(hp, d_alm, adjoint, st);
-            default: return run_synthesis<double, 1>(hp, d_alm, adjoint, st);
+            case 0: return run_synthesis<double, 1>(hp, d_alm, adjoint, st);
+            default: return run_synthesis_cfg<double, 1, 4, 128>(hp, d_alm, adjoint, st);
         }
     }
     if (hp.d.batch >= 4) {
@@ -1239,9 +1289,10 @@ cudaError_t launch_legendre_synthesis(const HostPlan& hp, const void* d_alm, int
             case 4: return run_synthesis_f32x2<4, 2, 256, 2>(hp, d_alm, adjoint, st);
             case 5: return run_synthesis_f32x2<8, 2, 256, 2>(hp, d_alm, adjoint, st);
             case 6: return run_synthesis_f32x2<8, 1, 256, 3>(hp, d_alm, adjoint, st);
+            case 7: return run_synthesis_f32x2<8, 2, 128, 3>(hp, d_alm, adjoint, st);
             case 0: break;
             default:
-                if (hp.d.batch >= 8) return run_synthesis_f32x2<8, 2, 128, 4>(hp, d_alm, adjoint, st);
+                if (hp.d.batch >= 8) return run_synthesis_f32x2<8, 2, 128, 3>(hp, d_alm, adjoint, st);
                 break;
         }
     }
@@ -1249,6 +1300,33 @@ cudaError_t launch_legendre_synthesis(const HostPlan& hp, const void* d_alm, int
     if (hp.d.batch >= 8 && hp.d.lmax < 1024) return run_synthesis<float, 8>(hp, d_alm, adjoint, st);
     if (hp.d.batch >= 4) return run_synthesis<float, 4>(hp, d_alm, adjoint, st);
     return run_synthesis<float, 1>(hp, d_alm, adjoint, st);
+}
+
+// ------------------------------------------------------------------ iterative refinement, elementwise steps (Eq. 4)
+template <typename T, bool RESIDUAL>
+__global__ void __launch_bounds__(256) refine_elementwise_kernel(const T* __restrict__ x, T* __restrict__ y, size_t n) {
+    const size_t stride = (size_t)gridDim.x * blockDim.x;
+    for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += stride)
+        y[i] = RESIDUAL ? x[i] - y[i] : y[i] + x[i];  // r = f - S a   |   a += A r
+}
+
+template <bool RESIDUAL>
+static cudaError_t run_refine(cuhpx_dtype_t dt, const void* x, void* y, size_t n, cudaStream_t st) {
+    int dev = 0, sms = 0;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e != cudaSuccess) return e;
+    if ((e = cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev)) != cudaSuccess) return e;
+    const size_t want = (n + 255) / 256;
+    const unsigned blocks = (unsigned)(want < (size_t)sms * 8 ? (want ? want : 1) : (size_t)sms * 8);
+    if (dt == CUHPX_F64) refine_elementwise_kernel<double, RESIDUAL><<<blocks, 256, 0, st>>>((const double*)x, (double*)y, n);
+    else refine_elementwise_kernel<float, RESIDUAL><<<blocks, 256, 0, st>>>((const float*)x, (float*)y, n);
+    return cudaGetLastError();
+}
+cudaError_t launch_residual(cuhpx_dtype_t dt, const void* f, void* r, size_t n, cudaStream_t st) {
+    return run_refine<true>(dt, f, r, n, st);
+}
+cudaError_t launch_accumulate(cuhpx_dtype_t dt, const void* d, void* a, size_t n, cudaStream_t st) {
+    return run_refine<false>(dt, d, a, n, st);
 }
 
 // ------------------------------------------------------------------ FMA peak probe

@@ -473,6 +473,35 @@ int cuhpx_map2alm_adjoint(int nside, int lmax, int mmax, int batch, cuhpx_dtype_
     return CUHPX_OK;
 }
 
+int cuhpx_map2alm_iter(int nside, int lmax, int mmax, int batch, cuhpx_dtype_t dt, const void* d_map, void* d_alm,
+                       const double* d_w, int n_iter, void* d_scratch_map, void* d_scratch_alm, void* ws,
+                       size_t ws_bytes, cuhpx_stream_t stream) {
+    HostPlan* hp = nullptr;
+    int rc = check_call(&hp, nside, lmax, mmax, batch, dt, d_map, d_alm, ws, ws_bytes);
+    if (rc) return rc;
+    if (d_w && ((uintptr_t)d_w & 7)) return CUHPX_EINVAL;
+    if (n_iter < 0) return CUHPX_EINVAL;
+    if (n_iter > 0 && (!d_scratch_map || !d_scratch_alm || ((uintptr_t)d_scratch_map & 15) || ((uintptr_t)d_scratch_alm & 15) ||
+                       d_scratch_map == d_map || d_scratch_alm == d_alm))
+        return CUHPX_EINVAL;
+    cudaStream_t st = (cudaStream_t)stream;
+    // a^(0) = A f
+    CUDA_OR_FAIL(launch_fft_analysis(*hp, d_map, d_w, 1, st));
+    CUDA_OR_FAIL(launch_legendre_analysis(*hp, d_alm, 0, st));
+    const size_t nmap = (size_t)hp->d.batch * (size_t)hp->d.npix, nalm2 = 2 * (size_t)hp->d.batch * (size_t)hp->d.nalm;
+    for (int k = 0; k < n_iter; ++k) {
+        // r = f - S a
+        CUDA_OR_FAIL(launch_legendre_synthesis(*hp, d_alm, 0, st));
+        CUDA_OR_FAIL(launch_fft_synthesis(*hp, d_scratch_map, nullptr, 0, st));
+        CUDA_OR_FAIL(launch_residual(dt, d_map, d_scratch_map, nmap, st));
+        // a += A r
+        CUDA_OR_FAIL(launch_fft_analysis(*hp, d_scratch_map, d_w, 1, st));
+        CUDA_OR_FAIL(launch_legendre_analysis(*hp, d_scratch_alm, 0, st));
+        CUDA_OR_FAIL(launch_accumulate(dt, d_scratch_alm, d_alm, nalm2, st));
+    }
+    return CUHPX_OK;
+}
+
 int cuhpx_fma_peak_probe(cuhpx_dtype_t dt, int iters, float* ms, double* fma_count, cuhpx_stream_t stream) {
     if ((dt != CUHPX_F32 && dt != CUHPX_F64) || iters < 1 || !ms || !fma_count) return CUHPX_EINVAL;
     CUDA_OR_FAIL(fma_peak_probe(dt, iters, ms, fma_count, (cudaStream_t)stream));

@@ -307,6 +307,37 @@ def test_operators_vs_dense_matrices(nside, lmax, mmax):
     np.testing.assert_allclose(np.concatenate([got.real, got.imag]), aa, atol=tol)
 
 
+@pytest.mark.parametrize("nside,lmax,n_iter", [(2, 4, 1), (2, 5, 3), (4, 8, 2)])
+def test_iterative_refinement_equals_gradient_descent_form(nside, lmax, n_iter):
+    """Eq. 4 against its 'equivalent gradient descent form' Eq. 5 written with the dense scipy
+    matrix: a^(k+1) = (4 pi / N) S* f + (I - (4 pi / N) S* S) a^(k), S* = Y^dagger = D^-1 S^T on the stored m >= 0
+    half (R4), a^(0) = (4 pi / N) S* f.  Pins the oracle's map2alm_iter (a dropped sign, A and S swapped
+    or a residual formed the other way round all fail)."""
+    S, cm = dense_S(nside, lmax, lmax)
+    npix = 12 * nside * nside
+    f = synth.normal(6, 2, npix)
+    cc = np.concatenate([cm, cm])
+    A = (4 * np.pi / npix) * (S.T / cc[:, None])
+    v = A @ f
+    for _ in range(n_iter):
+        v = A @ f + (np.eye(A.shape[0]) - A @ S) @ v
+    got = oracle.map2alm_iter(nside, lmax, lmax, f, n_iter)
+    ms = synth.alm_lm(lmax, lmax)[1]
+    ref = v[: len(ms)] + 1j * v[len(ms):]
+    np.testing.assert_allclose(got, ref, atol=1e-12 * np.abs(ref).max())
+    assert np.all(got.imag[ms == 0] == 0.0)
+
+
+def test_iterative_refinement_converges_on_band_limited_input():
+    """P:59 / P:400: 'accuracy improved by increasing the number of iterations' -- for f = S a with lmax <= 2 nside
+    the error |a^(k) - a| falls with every iteration."""
+    nside, lmax = 8, 12
+    a = synth.powerlaw_alm(8, lmax, lmax)[0]
+    f = oracle.alm2map(nside, lmax, lmax, a)
+    errs = [np.abs(oracle.map2alm_iter(nside, lmax, lmax, f, k) - a).max() for k in range(4)]
+    assert all(e1 < 0.5 * e0 for e0, e1 in zip(errs, errs[1:])), errs
+
+
 @pytest.mark.parametrize("nside,lmax", [(8, 16), (16, 40)])
 def test_adjoint_dot_product_identities(nside, lmax):
     """<S a, g> = <a, S^T g> and <A f, b> = <f, A^T b> (north_star)."""
