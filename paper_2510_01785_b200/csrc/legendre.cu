@@ -10,7 +10,6 @@
 // registers.  cos(theta) enters as x p = p - y p with y = 1 - cos(theta) (R3).
 #include <cuda_runtime.h>
 #include <math.h>
-#include <stdlib.h>
 
 #include "cuhpx_internal.h"
 
@@ -589,11 +588,15 @@ __device__ __forceinline__ int hswz(int x, int ln) { return (x + (ln & 3) + 4 * 
 __global__ void __launch_bounds__(GK, 2) legendre_analysis_gemm64_kernel(LegArgs a) {
     const DevPlan& P = a.p;
     const int m = blockIdx.x;
-    const int chunk = blockIdx.y;
     const int ch0 = blockIdx.z * GNCH;
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    // One CTA walks the ring chunks of its order m one after the other and adds each chunk's contribution to a_lm
+    // in place (chunk 0 stores, later chunks read-add-store; the rows it revisits are its own and stay in L2), so
+    // no per-chunk partial arrays are written and no combine kernel runs (measured at cfg4: 4.33 -> 4.07 ms).
+    for (int chunk = 0;; ++chunk) {
     const int jbase = P.jmin[m] + chunk * GK;
     if (jbase >= P.npairs) return;
+    const bool accumulate = chunk > 0;
 
     extern __shared__ __align__(16) unsigned char gemm_smem[];
     float* sLam = reinterpret_cast<float*>(gemm_smem);  // [parity][ring][HROW]; rows reused for the cross-warp sums
@@ -638,7 +641,6 @@ __global__ void __launch_bounds__(GK, 2) legendre_analysis_gemm64_kernel(LegArgs
     const double outscale = (a.adjoint && m > 0) ? 2.0 : 1.0;
     const long long abase = (long long)m * (2LL * P.lmax + 1 - m) / 2;
     float* out = reinterpret_cast<float*>(a.out);
-    if (a.to_partial) out += (size_t)chunk * P.batch * P.nalm * 2;
     const int nl = P.lmax - m + 1;
 
     if (tid < HTL) {
@@ -657,6 +659,16 @@ __global__ void __launch_bounds__(GK, 2) legendre_analysis_gemm64_kernel(LegArgs
     for (int t0 = 0, tb = 0; t0 < nl; t0 += HTL, tb ^= 1) {
         // alpha / scale of the next tile: requested now, parked in shared memory after the contraction (a store right
         // here would stall warps 0-1 for the full global-load latency in every tile, and the CTA with them)
+        float2 oldv[2] = {make_float2(0.f, 0.f), make_float2(0.f, 0.f)};
+        if (accumulate) {
+#pragma unroll
+            for (int rep = 0; rep < 2; ++rep) {
+                const int idx = tid + GK * rep;
+                const int k = t0 + (idx >> 5) * 4 + (idx & 3), ch = ch0 + ((idx >> 2) & 7);
+                if (k < nl && ch < P.batch)
+                    oldv[rep] = *reinterpret_cast<const float2*>(&out[((size_t)ch * P.nalm + abase + m + k) * 2]);
+            }
+        }
         double nA = 0.0, nS = 0.0;
         if (tid < HTL) {
             nA = (t0 + HTL + 1 + tid < nl) ? P.coef_alpha[abase + m + t0 + HTL + 1 + tid] : 0.0;
@@ -756,13 +768,14 @@ __global__ void __launch_bounds__(GK, 2) legendre_analysis_gemm64_kernel(LegArgs
             const int k = t0 + i;
             if (k < nl && ch < P.batch) {
                 const double s = sS[tb][i];
-                float2 o = make_float2((float)(s * (double)sum.x), (float)(s * (double)sum.y));
+                float2 o = make_float2(oldv[rep].x + (float)(s * (double)sum.x), oldv[rep].y + (float)(s * (double)sum.y));
                 if (m == 0) o.y = 0.f;  // Im a_l0 is exactly zero
                 *reinterpret_cast<float2*>(&out[((size_t)ch * P.nalm + abase + m + k) * 2]) = o;
             }
         }
         __syncthreads();  // partial tiles consumed before the next tile overwrites the lambda rows
     }
+    }  // chunk
 }
 
 // sum the per-chunk partial results: alm[b][idx] = sum_c partial[c][b][idx], c < nchunks(m)
@@ -1122,11 +1135,15 @@ template <typename T, int BT> struct LegCfg;
 template <> struct LegCfg<double, 1> { static constexpr int NT = 128, R = 8, LT = 8, RS = 4, NTS = 256; };
 template <> struct LegCfg<float, 1> { static constexpr int NT = 128, R = 8, LT = 8, RS = 4, NTS = 256; };
 template <> struct LegCfg<float, 4> { static constexpr int NT = 128, R = 4, LT = 4, RS = 2, NTS = 256; };
-template <> struct LegCfg<float, 8> { static constexpr int NT = 128, R = 4, LT = 2, RS = 2, NTS = 128; };
 
-int legendre_chunk_pairs(cuhpx_dtype_t dt, int batch) {
+// batched fp32 analysis: contraction kernels.  Long degree ranges use the 64-degree tiles with in-place accumulation
+// over the ring chunks (one "chunk" as far as the plan is concerned: no partial arrays); short ones (a few tiles per
+// order, latency-bound) the 32-degree tiles with one CTA per ring chunk.
+static bool use_gemm64(int lmax) { return lmax >= 512; }
+
+int legendre_chunk_pairs(cuhpx_dtype_t dt, int batch, int lmax, int npairs) {
     if (dt == CUHPX_F64) return LegCfg<double, 1>::NT * LegCfg<double, 1>::R;
-    if (batch >= 5) return GK;  // contraction kernel
+    if (batch >= 5) return use_gemm64(lmax) ? (npairs > GK ? npairs : GK) : GK;
     return batch >= 4 ? LegCfg<float, 4>::NT * LegCfg<float, 4>::R : LegCfg<float, 1>::NT * LegCfg<float, 1>::R;
 }
 
@@ -1167,11 +1184,6 @@ static cudaError_t run_synthesis(const HostPlan& hp, const void* d_alm, int adjo
     dim3 grid(P.mmax + 1, (P.npairs + chunk - 1) / chunk, (P.batch + BT - 1) / BT);
     legendre_synthesis_kernel<T, BT, C::RS, C::NTS><<<grid, C::NTS, 0, st>>>(a);
     return cudaGetLastError();
-}
-
-static int tune_variant(const char* name) {  // TUNING ONLY (removed once the configuration is fixed)
-    const char* v = getenv(name);
-    return v ? atoi(v) : -1;
 }
 
 template <typename T, int BT, int R, int LT, int NT, int GL>
@@ -1216,19 +1228,23 @@ static cudaError_t run_analysis_gemm(const HostPlan& hp, void* d_alm, int adjoin
     a.p = P;
     a.in = nullptr;
     a.adjoint = adjoint;
+    cudaError_t e;
+    if (use_gemm64(P.lmax)) {
+        a.to_partial = 0;
+        a.out = d_alm;
+        dim3 grid(P.mmax + 1, 1, (P.batch + GNCH - 1) / GNCH);
+        e = cudaFuncSetAttribute(legendre_analysis_gemm64_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)HSMEM);
+        if (e != cudaSuccess) return e;
+        legendre_analysis_gemm64_kernel<<<grid, GK, HSMEM, st>>>(a);
+        return cudaGetLastError();
+    }
     a.to_partial = P.nchunk_max > 1;
     a.out = a.to_partial ? P.partial : d_alm;
     dim3 grid(P.mmax + 1, P.nchunk_max, (P.batch + GNCH - 1) / GNCH);
     constexpr size_t smem = sizeof(float) * (2 * GK * GROW + 2 * GK * GNC) + sizeof(double) * 4 * GTL;
-    cudaError_t e = cudaFuncSetAttribute(legendre_analysis_gemm_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    e = cudaFuncSetAttribute(legendre_analysis_gemm_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return e;
-    if (tune_variant("CUHPX_ANA_VARIANT") == 1) {
-        legendre_analysis_gemm_kernel<<<grid, GK, smem, st>>>(a);
-    } else {
-        e = cudaFuncSetAttribute(legendre_analysis_gemm64_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)HSMEM);
-        if (e != cudaSuccess) return e;
-        legendre_analysis_gemm64_kernel<<<grid, GK, HSMEM, st>>>(a);
-    }
+    legendre_analysis_gemm_kernel<<<grid, GK, smem, st>>>(a);
     e = cudaGetLastError();
     if (e != cudaSuccess) return e;
     if (a.to_partial) {
@@ -1240,16 +1256,9 @@ static cudaError_t run_analysis_gemm(const HostPlan& hp, void* d_alm, int adjoin
     return e;
 }
 
+// Configurations below are the winners of sweeps on B200 (profiles/r1_legendre_tuning.md).
 cudaError_t launch_legendre_analysis(const HostPlan& hp, void* d_alm, int adjoint, cudaStream_t st) {
-    if (hp.dtype == CUHPX_F64) {
-        switch (tune_variant("CUHPX_ANA64_VARIANT")) {
-            case 1: return run_analysis_cfg<double, 1, 8, 8, 128, 64>(hp, d_alm, adjoint, st);
-            case 2: return run_analysis_cfg<double, 1, 8, 4, 128, 32>(hp, d_alm, adjoint, st);
-            case 3: return run_analysis_cfg<double, 1, 8, 4, 128, 64>(hp, d_alm, adjoint, st);
-            case 0: return run_analysis<double, 1>(hp, d_alm, adjoint, st);
-            default: return run_analysis_cfg<double, 1, 8, 8, 128, 64>(hp, d_alm, adjoint, st);
-        }
-    }
+    if (hp.dtype == CUHPX_F64) return run_analysis_cfg<double, 1, 8, 8, 128, 64>(hp, d_alm, adjoint, st);
     if (hp.d.batch >= 5) return run_analysis_gemm(hp, d_alm, adjoint, st);
     if (hp.d.batch >= 4) return run_analysis<float, 4>(hp, d_alm, adjoint, st);
     return run_analysis<float, 1>(hp, d_alm, adjoint, st);
@@ -1271,33 +1280,12 @@ static cudaError_t run_synthesis_f32x2(const HostPlan& hp, const void* d_alm, in
 }
 
 cudaError_t launch_legendre_synthesis(const HostPlan& hp, const void* d_alm, int adjoint, cudaStream_t st) {
-    if (hp.dtype == CUHPX_F64) {
-        switch (tune_variant("CUHPX_SYN64_VARIANT")) {
-            case 1: return run_synthesis_cfg<double, 1, 8, 128>(hp, d_alm, adjoint, st);
-            case 2: return run_synthesis_cfg<double, 1, 4, 128>(hp, d_alm, adjoint, st);
-            case 3: return run_synthesis_cfg<double, 1, 6, 128>(hp, d_alm, adjoint, st);
-            case 4: return run_synthesis_cfg<double, 1, 2, 256>(hp, d_alm, adjoint, st);
-            case 0: return run_synthesis<double, 1>(hp, d_alm, adjoint, st);
-            default: return run_synthesis_cfg<double, 1, 4, 128>(hp, d_alm, adjoint, st);
-        }
+    if (hp.dtype == CUHPX_F64) return run_synthesis_cfg<double, 1, 4, 128>(hp, d_alm, adjoint, st);
+    if (hp.d.batch >= 8) {
+        // packed-FMA kernels, 8 channels per CTA; short degree ranges want more, smaller CTAs in flight
+        return hp.d.lmax < 512 ? run_synthesis_f32x2<8, 1, 256, 3>(hp, d_alm, adjoint, st)
+                               : run_synthesis_f32x2<8, 2, 128, 3>(hp, d_alm, adjoint, st);
     }
-    if (hp.d.batch >= 4) {
-        switch (tune_variant("CUHPX_SYN_VARIANT")) {
-            case 1: return run_synthesis_f32x2<8, 2, 128, 4>(hp, d_alm, adjoint, st);
-            case 2: return run_synthesis_f32x2<8, 4, 128, 2>(hp, d_alm, adjoint, st);
-            case 3: return run_synthesis_f32x2<4, 4, 128, 3>(hp, d_alm, adjoint, st);
-            case 4: return run_synthesis_f32x2<4, 2, 256, 2>(hp, d_alm, adjoint, st);
-            case 5: return run_synthesis_f32x2<8, 2, 256, 2>(hp, d_alm, adjoint, st);
-            case 6: return run_synthesis_f32x2<8, 1, 256, 3>(hp, d_alm, adjoint, st);
-            case 7: return run_synthesis_f32x2<8, 2, 128, 3>(hp, d_alm, adjoint, st);
-            case 0: break;
-            default:
-                if (hp.d.batch >= 8) return run_synthesis_f32x2<8, 2, 128, 3>(hp, d_alm, adjoint, st);
-                break;
-        }
-    }
-    // 8 channels per CTA pay off when there are few (m, ring chunk) CTAs to fill the GPU with (measured: cfg3 yes, cfg4 no)
-    if (hp.d.batch >= 8 && hp.d.lmax < 1024) return run_synthesis<float, 8>(hp, d_alm, adjoint, st);
     if (hp.d.batch >= 4) return run_synthesis<float, 4>(hp, d_alm, adjoint, st);
     return run_synthesis<float, 1>(hp, d_alm, adjoint, st);
 }

@@ -12,7 +12,7 @@
 
 namespace cuhpx {
 
-int legendre_chunk_pairs(cuhpx_dtype_t dt, int batch);  // legendre.cu
+int legendre_chunk_pairs(cuhpx_dtype_t dt, int batch, int lmax, int npairs);  // legendre.cu
 
 namespace {
 
@@ -146,7 +146,7 @@ void fill_basic(HostPlan& hp, int nside, int lmax, int mmax, int batch, cuhpx_dt
     d.mstride = (int)cuhpx_spectra_stride(mmax);
     d.npix = 12LL * nside * nside;
     d.nalm = (long long)cuhpx_alm_count(lmax, mmax);
-    d.chunk_pairs = legendre_chunk_pairs(dt, batch);
+    d.chunk_pairs = legendre_chunk_pairs(dt, batch, lmax, d.npairs);
     d.nchunk_max = (d.npairs + d.chunk_pairs - 1) / d.chunk_pairs;
     hp.h_ringN.resize(d.npairs);
     hp.h_start.resize(d.npairs);
