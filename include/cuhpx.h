@@ -101,6 +101,17 @@ int cuhpx_map2alm_iter(int nside, int lmax, int mmax, int batch, cuhpx_dtype_t d
                        const double* d_ring_weights, int n_iter, void* d_scratch_map, void* d_scratch_alm,
                        void* d_workspace, size_t workspace_bytes, cuhpx_stream_t stream);
 
+/* ---- layout reordering NESTED <-> RING (paper section III-B, via (x, y, f) P:118-123)
+ * NESTED: index = f nside^2 + Z-order (Morton) interleave of (x, y) inside base face f (x on the even bits), P:109;
+ * RING: as everywhere else in this header.  d_in / d_out: [batch][npix] elements of `dtype` (moved as bits,
+ * 4 or 8 bytes each), DEVICE pointers, 16-byte aligned, must not alias.  direction: CUHPX_NEST2RING reads NESTED and
+ * writes RING, CUHPX_RING2NEST the reverse.  No workspace.  Errors as for the operators. */
+typedef enum { CUHPX_NEST2RING = 0, CUHPX_RING2NEST = 1 } cuhpx_reorder_t;
+int cuhpx_reorder(int nside, int batch, cuhpx_dtype_t dtype, int direction, const void* d_in, void* d_out,
+                  cuhpx_stream_t stream);
+/* host helper: RING index of NESTED pixel ipnest; -1 on bad arguments */
+long long cuhpx_nest2ring_index(int nside, long long ipnest);
+
 /* ---- the two stages of each direction, individually, for per-stage
  * measurement and stage-level parity tests.  The ring spectra live inside the workspace:
  *   spectra[b][ring][m], m = 0..m_cut(ring) (entries above m_cut(ring) are neither written nor read: there

@@ -24,8 +24,9 @@ EXPORTS = [
     "cuhpx_alm2map_adjoint", "cuhpx_map2alm_adjoint", "cuhpx_spectra_stride", "cuhpx_workspace_spectra",
     "cuhpx_workspace_mcut", "cuhpx_analysis_fft_stage", "cuhpx_analysis_legendre_stage",
     "cuhpx_synthesis_legendre_stage", "cuhpx_synthesis_fft_stage", "cuhpx_fma_peak_probe", "cuhpx_workspace_stats",
-    "cuhpx_map2alm_iter",
+    "cuhpx_map2alm_iter", "cuhpx_reorder", "cuhpx_nest2ring_index",
 ]
+CUHPX_NEST2RING, CUHPX_RING2NEST = 0, 1
 
 
 class CuhpxError(RuntimeError):
@@ -61,6 +62,9 @@ def _load() -> ctypes.CDLL:
     lib.cuhpx_alm2map_adjoint.argtypes = [i, i, i, i, i, vp, vp, vp, sz, vp]
     lib.cuhpx_map2alm_adjoint.argtypes = [i, i, i, i, i, vp, vp, vp, vp, sz, vp]
     lib.cuhpx_map2alm_iter.argtypes = [i, i, i, i, i, vp, vp, vp, i, vp, vp, vp, sz, vp]
+    lib.cuhpx_reorder.argtypes = [i, i, i, i, vp, vp, vp]
+    lib.cuhpx_nest2ring_index.restype = ctypes.c_longlong
+    lib.cuhpx_nest2ring_index.argtypes = [i, ctypes.c_longlong]
     lib.cuhpx_spectra_stride.restype = sz
     lib.cuhpx_spectra_stride.argtypes = [i]
     lib.cuhpx_workspace_spectra.restype = vp
@@ -190,6 +194,29 @@ def cuhpx_map2alm_adjoint(nside, lmax, mmax, batch, dtype, d_galm, d_gmap, d_rin
     p, n = _ws_args(workspace)
     _check(_lib.cuhpx_map2alm_adjoint(nside, lmax, mmax, batch, dtype, _dev_ptr(d_galm), _dev_ptr(d_gmap),
                                       _dev_ptr(d_ring_weights), p, n, _stream_ptr(stream)), "cuhpx_map2alm_adjoint")
+
+
+def cuhpx_reorder(nside, batch, dtype, direction, d_in, d_out, stream=None) -> None:
+    _check(_lib.cuhpx_reorder(nside, batch, dtype, int(direction), _dev_ptr(d_in), _dev_ptr(d_out), _stream_ptr(stream)),
+           "cuhpx_reorder")
+
+
+def cuhpx_nest2ring_index(nside: int, ipnest: int) -> int:
+    return int(_lib.cuhpx_nest2ring_index(nside, ipnest))
+
+
+def nest2ring(hmap: torch.Tensor, nside: int) -> torch.Tensor:
+    """[batch, npix] NESTED -> RING (paper section III-B)."""
+    out = torch.empty_like(hmap)
+    cuhpx_reorder(nside, hmap.shape[0], _dtype_code(hmap.dtype), CUHPX_NEST2RING, hmap, out)
+    return out
+
+
+def ring2nest(hmap: torch.Tensor, nside: int) -> torch.Tensor:
+    """[batch, npix] RING -> NESTED (paper section III-B)."""
+    out = torch.empty_like(hmap)
+    cuhpx_reorder(nside, hmap.shape[0], _dtype_code(hmap.dtype), CUHPX_RING2NEST, hmap, out)
+    return out
 
 
 def cuhpx_analysis_fft_stage(d_map, d_ring_weights, use_weights, workspace, stream=None) -> None:

@@ -91,6 +91,10 @@ void fft_stage_stats(const HostPlan& hp, int* launches, double* table_bytes);
 cudaError_t launch_residual(cuhpx_dtype_t dt, const void* f, void* r, size_t n, cudaStream_t st);
 cudaError_t launch_accumulate(cuhpx_dtype_t dt, const void* d, void* a, size_t n, cudaStream_t st);
 
+// layout reordering (reorder.cu)
+cudaError_t launch_reorder(int nside, int batch, cuhpx_dtype_t dt, int to_ring, const void* in, void* out, cudaStream_t st);
+long long nest_to_ring_index(int nside, long long ipnest);
+
 cudaError_t fma_peak_probe(cuhpx_dtype_t dt, int iters, float* ms, double* count, cudaStream_t st);
 
 }  // namespace cuhpx

@@ -502,6 +502,20 @@ int cuhpx_map2alm_iter(int nside, int lmax, int mmax, int batch, cuhpx_dtype_t d
     return CUHPX_OK;
 }
 
+int cuhpx_reorder(int nside, int batch, cuhpx_dtype_t dt, int direction, const void* d_in, void* d_out,
+                  cuhpx_stream_t stream) {
+    if (nside < 1 || !is_pow2(nside) || nside > (1 << 13) || batch < 1 || (dt != CUHPX_F32 && dt != CUHPX_F64)) return CUHPX_EINVAL;
+    if (direction != CUHPX_NEST2RING && direction != CUHPX_RING2NEST) return CUHPX_EINVAL;
+    if (!d_in || !d_out || d_in == d_out || ((uintptr_t)d_in & 15) || ((uintptr_t)d_out & 15)) return CUHPX_EINVAL;
+    CUDA_OR_FAIL(launch_reorder(nside, batch, dt, direction == CUHPX_NEST2RING, d_in, d_out, (cudaStream_t)stream));
+    return CUHPX_OK;
+}
+
+long long cuhpx_nest2ring_index(int nside, long long ipnest) {
+    if (nside < 1 || !is_pow2(nside) || nside > (1 << 13) || ipnest < 0 || ipnest >= 12LL * nside * nside) return -1;
+    return nest_to_ring_index(nside, ipnest);
+}
+
 int cuhpx_fma_peak_probe(cuhpx_dtype_t dt, int iters, float* ms, double* fma_count, cuhpx_stream_t stream) {
     if ((dt != CUHPX_F32 && dt != CUHPX_F64) || iters < 1 || !ms || !fma_count) return CUHPX_EINVAL;
     CUDA_OR_FAIL(fma_peak_probe(dt, iters, ms, fma_count, (cudaStream_t)stream));

@@ -33,7 +33,7 @@ def test_gradients_match_oracle_adjoints_fp64():
     ref = -2.0 * oracle.alm2map_adjoint(nside, lmax, lmax, res)
     got = x.grad.cpu().numpy()[0]
     assert np.abs(got - ref).max() / np.abs(ref).max() <= 1e-11
-    assert abs(float(loss) - float((res ** 2).sum())) <= 1e-11 * float((res ** 2).sum())
+    assert abs(float(loss.detach()) - float((res ** 2).sum())) <= 1e-11 * float((res ** 2).sum())
 
     # L = sum |A f - b|^2  ->  dL/df = 2 A^T (A f - b)
     f = torch.from_numpy(y).cuda().requires_grad_(True)
@@ -82,6 +82,6 @@ def test_one_layer_demo_loss_falls_monotonically():
         (g,) = torch.autograd.grad(loss, x)
         with torch.no_grad():
             x -= step * g
-        losses.append(float(loss))
+        losses.append(float(loss.detach()))
     assert all(b < a for a, b in zip(losses, losses[1:])), losses
     assert losses[-1] < 1e-2 * losses[0]
