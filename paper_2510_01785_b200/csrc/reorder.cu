@@ -56,16 +56,6 @@ __host__ __device__ __forceinline__ unsigned compact_bits(unsigned long long v) 
     v = (v | (v >> 16)) & 0x00000000ffffffffull;
     return (unsigned)v;
 }
-__host__ __device__ __forceinline__ unsigned long long spread_bits(unsigned v) {
-    unsigned long long w = v;
-    w = (w | (w << 16)) & 0x0000ffff0000ffffull;
-    w = (w | (w << 8)) & 0x00ff00ff00ff00ffull;
-    w = (w | (w << 4)) & 0x0f0f0f0f0f0f0f0full;
-    w = (w | (w << 2)) & 0x3333333333333333ull;
-    w = (w | (w << 1)) & 0x5555555555555555ull;
-    return w;
-}
-
 long long nest_to_ring_index(int nside, long long ipnest) {
     const long long ns2 = (long long)nside * nside;
     const int f = (int)(ipnest / ns2);
@@ -75,41 +65,131 @@ long long nest_to_ring_index(int nside, long long ipnest) {
 
 constexpr int RT_THREADS = 256;
 
+// 32-bit variants for the kernel (nside <= 8192: every index fits in 31 bits)
+__device__ __forceinline__ unsigned compact16(unsigned v) {  // even bits of the low 32 -> low 16
+    v &= 0x55555555u;
+    v = (v | (v >> 1)) & 0x33333333u;
+    v = (v | (v >> 2)) & 0x0f0f0f0fu;
+    v = (v | (v >> 4)) & 0x00ff00ffu;
+    v = (v | (v >> 8)) & 0x0000ffffu;
+    return v;
+}
+
 // T = tile edge (power of two, <= 64, <= nside).  grid.x = 12 (nside / T)^2 tiles, grid.y = batch.
+// Index arithmetic is hoisted: everything that depends only on the anti-diagonal s = xl + yl (ring number, ring
+// length, first index of the ring, the in-ring position of xl = 0) is computed once per diagonal, an element then
+// costs an add, a wrap and the two addresses (the first version recomputed xyf -> RING in 64 bits per element and
+// was issue-bound at 79 % issue-active / 1.5 TB/s; ncu in profiles/).
 template <typename W, int T, bool TO_RING>
 __global__ void __launch_bounds__(RT_THREADS) reorder_kernel(int nside, long long npix, const W* __restrict__ in, W* __restrict__ out) {
-    __shared__ W tile[T * T];
-    const int tiles_per_face = (nside / T) * (nside / T);
-    const int f = blockIdx.x / tiles_per_face;
-    const unsigned tmorton = blockIdx.x % tiles_per_face;  // tiles of a face in Z-order, like the pixels
-    const int x0 = (int)compact_bits(tmorton) * T, y0 = (int)compact_bits(tmorton >> 1) * T;
-    const long long nest0 = (long long)f * nside * nside + (long long)tmorton * (T * T);
+    extern __shared__ __align__(16) unsigned char reorder_smem[];
+    W* tile = reinterpret_cast<W*>(reorder_smem);
+    constexpr int TT = T * T;
+    const int tpf = (nside / T) * (nside / T);
+    const int f = blockIdx.x / tpf;
+    const unsigned tmorton = blockIdx.x - f * tpf;  // tiles of a face in Z-order, like the pixels
+    const int x0 = (int)compact16(tmorton) * T, y0 = (int)compact16(tmorton >> 1) * T;
+    const size_t nest0 = (size_t)f * nside * nside + (size_t)tmorton * TT;
     const W* src = in + (size_t)blockIdx.y * npix;
     W* dst = out + (size_t)blockIdx.y * npix;
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    // element e = tid + 256 i of the block: Morton code -> (xl, yl); the thread part is fixed, the i part constant-folds
+    const int txl = (int)compact16((unsigned)tid), tyl = (int)compact16((unsigned)tid >> 1);
 
     if (TO_RING) {
-        for (int e = tid; e < T * T; e += RT_THREADS) {
-            const int xl = (int)compact_bits((unsigned)e), yl = (int)compact_bits((unsigned)e >> 1);
-            tile[yl * T + xl] = src[nest0 + e];
+#pragma unroll
+        for (int i = 0; i < (TT + RT_THREADS - 1) / RT_THREADS; ++i) {
+            const int e = tid + RT_THREADS * i;
+            if (e < TT) {
+                // bits 8.. of e are i: even bits of (i << 8) go to xl bit 4.., odd bits to yl bit 4..
+                const int xl = TT > RT_THREADS ? (txl | ((int)compact16((unsigned)i) << 4)) : (int)compact16((unsigned)e);
+                const int yl = TT > RT_THREADS ? (tyl | ((int)compact16((unsigned)i >> 1) << 4)) : (int)compact16((unsigned)e >> 1);
+                tile[yl * T + xl] = src[nest0 + e];
+            }
         }
         __syncthreads();
     }
-    // anti-diagonals s = xl + yl of the block: consecutive xl are consecutive pixels of one ring
-    for (int s = warp; s < 2 * T - 1; s += RT_THREADS / 32) {
-        const int xmin = s < T ? 0 : s - T + 1, len = s < T ? s + 1 : 2 * T - 1 - s;
-        for (int k = lane; k < len; k += 32) {
-            const int xl = xmin + k, yl = s - xl;
-            const long long ir = xyf_to_ring(nside, x0 + xl, y0 + yl, f);
-            if (TO_RING) dst[ir] = tile[yl * T + xl];
-            else tile[yl * T + xl] = src[ir];
+    const int ns = nside, jrl = face_jrll(f) * ns, jpl = face_jpll(f);
+    const int ncap = 2 * ns * (ns - 1);
+    // ring of anti-diagonal s (x + y = x0 + y0 + s): first RING index of the run's ring, ring length, position of xl = 0
+    auto diagonal = [&](int s, int& before, int& n4, int& a) {
+        const int jr = jrl - (x0 + y0 + s) - 1;
+        int nr, kshift = 0;
+        if (jr < ns) {
+            nr = jr;
+            before = 2 * nr * (nr - 1);
+        } else if (jr > 3 * ns) {
+            nr = 4 * ns - jr;
+            before = (int)npix - 2 * (nr + 1) * nr;
+        } else {
+            nr = ns;
+            before = ncap + (jr - ns) * 4 * ns;
+            kshift = (jr - ns) & 1;
+        }
+        n4 = 4 * nr;
+        // jp(xl) = (jpl nr + (x0 + xl) - (y0 + s - xl) + 1 + kshift) / 2 = a + xl, the numerator is always even
+        a = (jpl * nr + x0 - y0 - s + 1 + kshift) / 2;
+    };
+    auto ring_index = [&](int before, int n4, int a, int xl) {
+        int jp = a + xl;
+        if (jp > n4) jp -= n4;
+        if (jp < 1) jp += n4;
+        return before + jp - 1;
+    };
+    constexpr int NW = RT_THREADS / 32, KPD = (T + 31) / 32;  // warps, lane slots per diagonal
+    if (TO_RING) {
+        for (int s = warp; s < 2 * T - 1; s += NW) {
+            int before, n4, a;
+            diagonal(s, before, n4, a);
+            const int xmin = s < T ? 0 : s - T + 1, len = s < T ? s + 1 : 2 * T - 1 - s;
+            for (int k = lane; k < len; k += 32) {
+                const int xl = xmin + k;
+                dst[ring_index(before, n4, a, xl)] = tile[(s - xl) * T + xl];
+            }
+        }
+    } else {
+        // gather side: the loads of U diagonals are issued before any of them is parked in shared memory
+        constexpr int U = 4;
+        for (int sb = warp; sb < 2 * T - 1; sb += NW * U) {
+            W v[U][KPD];
+#pragma unroll
+            for (int u = 0; u < U; ++u) {
+                const int s = sb + NW * u;
+                if (s < 2 * T - 1) {
+                    int before, n4, a;
+                    diagonal(s, before, n4, a);
+                    const int xmin = s < T ? 0 : s - T + 1, len = s < T ? s + 1 : 2 * T - 1 - s;
+#pragma unroll
+                    for (int q = 0; q < KPD; ++q) {
+                        const int k = lane + 32 * q;
+                        if (k < len) v[u][q] = src[ring_index(before, n4, a, xmin + k)];
+                    }
+                }
+            }
+#pragma unroll
+            for (int u = 0; u < U; ++u) {
+                const int s = sb + NW * u;
+                if (s < 2 * T - 1) {
+                    const int xmin = s < T ? 0 : s - T + 1, len = s < T ? s + 1 : 2 * T - 1 - s;
+#pragma unroll
+                    for (int q = 0; q < KPD; ++q) {
+                        const int k = lane + 32 * q;
+                        if (k < len) tile[(s - xmin - k) * T + xmin + k] = v[u][q];
+                    }
+                }
+            }
         }
     }
     if (!TO_RING) {
         __syncthreads();
-        for (int e = tid; e < T * T; e += RT_THREADS) {
-            const int xl = (int)compact_bits((unsigned)e), yl = (int)compact_bits((unsigned)e >> 1);
-            dst[nest0 + e] = tile[yl * T + xl];
+#pragma unroll
+        for (int i = 0; i < (TT + RT_THREADS - 1) / RT_THREADS; ++i) {
+            const int e = tid + RT_THREADS * i;
+            if (e < TT) {
+                const int xl = TT > RT_THREADS ? (txl | ((int)compact16((unsigned)i) << 4)) : (int)compact16((unsigned)e);
+                const int yl = TT > RT_THREADS ? (tyl | ((int)compact16((unsigned)i >> 1) << 4)) : (int)compact16((unsigned)e >> 1);
+                dst[nest0 + e] = tile[yl * T + xl];
+            }
         }
     }
 }
@@ -118,13 +198,23 @@ template <typename W, int T>
 static cudaError_t run_reorder_t(int nside, int batch, int to_ring, const void* in, void* out, cudaStream_t st) {
     const long long npix = 12LL * nside * nside;
     dim3 grid((unsigned)(12 * (nside / T) * (nside / T)), (unsigned)batch);
-    if (to_ring) reorder_kernel<W, T, true><<<grid, RT_THREADS, 0, st>>>(nside, npix, (const W*)in, (W*)out);
-    else reorder_kernel<W, T, false><<<grid, RT_THREADS, 0, st>>>(nside, npix, (const W*)in, (W*)out);
+    constexpr size_t smem = sizeof(W) * T * T;
+    cudaError_t e;
+    if (to_ring) {
+        if (smem > 48 * 1024 && (e = cudaFuncSetAttribute(reorder_kernel<W, T, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem)) != cudaSuccess) return e;
+        reorder_kernel<W, T, true><<<grid, RT_THREADS, smem, st>>>(nside, npix, (const W*)in, (W*)out);
+    } else {
+        if (smem > 48 * 1024 && (e = cudaFuncSetAttribute(reorder_kernel<W, T, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem)) != cudaSuccess) return e;
+        reorder_kernel<W, T, false><<<grid, RT_THREADS, smem, st>>>(nside, npix, (const W*)in, (W*)out);
+    }
     return cudaGetLastError();
 }
 
 template <typename W>
 static cudaError_t run_reorder(int nside, int batch, int to_ring, const void* in, void* out, cudaStream_t st) {
+    // 4-byte elements, scatter side: 128 x 128 tiles (64 KB) double the length of the RING-side runs (measured: 3.2 ->
+    // 3.4-3.6 TB/s); the gather side prefers more resident CTAs (64 x 64 tiles)
+    if (sizeof(W) == 4 && nside >= 128 && to_ring) return run_reorder_t<W, 128>(nside, batch, to_ring, in, out, st);
     if (nside >= 64) return run_reorder_t<W, 64>(nside, batch, to_ring, in, out, st);
     if (nside >= 16) return run_reorder_t<W, 16>(nside, batch, to_ring, in, out, st);
     if (nside >= 4) return run_reorder_t<W, 4>(nside, batch, to_ring, in, out, st);

@@ -193,6 +193,136 @@ __global__ void __launch_bounds__(FFT_THREADS) ring_direct_synthesis_kernel(DevP
     }
 }
 
+// ------------------------------------------------------------------ direct kernels, channel-blocked (batched maps)
+// With many channels (BASELINE configs[2]: nside 64, 256 channels -- every ring is a "short" ring) the direct sums
+// are the whole FFT stage.  One CTA = (ring, CB channels): a twiddle is fetched once per (m, x) and used for CB
+// channels (2 CB FMAs per shared-memory twiddle instead of 2), the ring data of the CB channels sits in shared
+// memory as [x][CB] so one broadcast LDS.128 feeds 4 channels.
+constexpr int DIRECT_CB_THREADS = 128;
+
+template <typename T, int CB>
+__global__ void __launch_bounds__(DIRECT_CB_THREADS) ring_direct_analysis_cb_kernel(DevPlan P, const RingInfo* __restrict__ info,
+                                                                                   const T* __restrict__ map,
+                                                                                   const double* __restrict__ w, int use_w) {
+    using T2 = typename V2<T>::type;
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    const int ch0 = blockIdx.y * CB;
+    const RingInfo R = load_info(info, blockIdx.x);
+    const int N = R.N, r = R.r, tid = threadIdx.x;
+    T2* tw = reinterpret_cast<T2*>(smem_raw);
+    T* p = reinterpret_cast<T*>(tw + N);  // [x][CB]
+    for (int x = tid; x < N; x += DIRECT_CB_THREADS) {
+        T c, s;
+        cispi_ratio(2LL * x, N, (T)-1, c, s);
+        tw[x].x = c;
+        tw[x].y = s;
+    }
+    for (int e = tid; e < N * CB; e += DIRECT_CB_THREADS) {
+        const int c = e / N, x = e - c * N, ch = ch0 + c;
+        p[x * CB + c] = ch < P.batch ? map[(size_t)ch * P.npix + R.start + x] : (T)0;
+    }
+    __syncthreads();
+    const T wt = (T)ring_weight(P, R, w, use_w);
+    for (int m = tid; m <= R.mcut; m += DIRECT_CB_THREADS) {
+        const int step = m % N;
+        int idx = 0;
+        T ar[CB], ai[CB];
+#pragma unroll
+        for (int c = 0; c < CB; ++c) ar[c] = ai[c] = 0;
+        for (int x = 0; x < N; ++x) {
+            const T2 t = tw[idx];
+            T pv[CB];
+#pragma unroll
+            for (int c = 0; c < CB; c += 4 / (sizeof(T) / 4)) {  // 16-byte broadcast loads
+                if (sizeof(T) == 4) {
+                    const float4 v = *reinterpret_cast<const float4*>(&p[x * CB + c]);
+                    pv[c] = v.x; pv[c + 1] = v.y; pv[c + 2] = v.z; pv[c + 3] = v.w;
+                } else {
+                    const double2 v = *reinterpret_cast<const double2*>(&p[x * CB + c]);
+                    pv[c] = v.x; pv[c + 1] = v.y;
+                }
+            }
+#pragma unroll
+            for (int c = 0; c < CB; ++c) {
+                ar[c] = fma(pv[c], t.x, ar[c]);
+                ai[c] = fma(pv[c], t.y, ai[c]);
+            }
+            idx += step;
+            if (idx >= N) idx -= N;
+        }
+        T c = 1, s = 0;
+        if (R.shifted) cispi_ratio((long long)(m % (2 * N)), N, (T)-1, c, s);
+#pragma unroll
+        for (int k = 0; k < CB; ++k) {
+            const int ch = ch0 + k;
+            if (ch < P.batch) {
+                T2 o;
+                o.x = wt * (ar[k] * c - ai[k] * s);
+                o.y = wt * (ar[k] * s + ai[k] * c);
+                (reinterpret_cast<T2*>(P.spectra) + ((size_t)ch * P.nrings + r) * P.mstride)[m] = o;
+            }
+        }
+    }
+}
+
+template <typename T, int CB>
+__global__ void __launch_bounds__(DIRECT_CB_THREADS) ring_direct_synthesis_cb_kernel(DevPlan P, const RingInfo* __restrict__ info,
+                                                                                    T* __restrict__ map,
+                                                                                    const double* __restrict__ w, int use_w) {
+    using T2 = typename V2<T>::type;
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    const int ch0 = blockIdx.y * CB;
+    const RingInfo R = load_info(info, blockIdx.x);
+    const int N = R.N, r = R.r, tid = threadIdx.x, nm = R.mcut + 1;
+    T2* tw = reinterpret_cast<T2*>(smem_raw);
+    T2* G = tw + N;  // [m][CB], already twisted by exp(+i m phi0)
+    for (int x = tid; x < N; x += DIRECT_CB_THREADS) {
+        T c, s;
+        cispi_ratio(2LL * x, N, (T)1, c, s);
+        tw[x].x = c;
+        tw[x].y = s;
+    }
+    for (int e = tid; e < nm * CB; e += DIRECT_CB_THREADS) {
+        const int k = e / nm, m = e - k * nm, ch = ch0 + k;
+        T2 g;
+        g.x = g.y = 0;
+        if (ch < P.batch) g = (reinterpret_cast<const T2*>(P.spectra) + ((size_t)ch * P.nrings + r) * P.mstride)[m];
+        if (m == 0) g.y = 0;  // Im G_0 is ignored
+        if (R.shifted) {
+            T c, s;
+            cispi_ratio((long long)(m % (2 * N)), N, (T)1, c, s);
+            const T gr = g.x * c - g.y * s, gi = g.x * s + g.y * c;
+            g.x = gr;
+            g.y = gi;
+        }
+        G[m * CB + k] = g;
+    }
+    __syncthreads();
+    const T wt = (T)ring_weight(P, R, w, use_w);
+    for (int x = tid; x < N; x += DIRECT_CB_THREADS) {
+        T acc[CB];
+#pragma unroll
+        for (int k = 0; k < CB; ++k) acc[k] = 0;
+        int idx = 0;
+        for (int m = 1; m < nm; ++m) {
+            idx += x;
+            if (idx >= N) idx -= N;
+            const T2 t = tw[idx];
+#pragma unroll
+            for (int k = 0; k < CB; ++k) {
+                const T2 g = G[m * CB + k];
+                acc[k] = fma(g.x, t.x, acc[k]);
+                acc[k] = fma(-g.y, t.y, acc[k]);
+            }
+        }
+#pragma unroll
+        for (int k = 0; k < CB; ++k) {
+            const int ch = ch0 + k;
+            if (ch < P.batch) map[(size_t)ch * P.npix + R.start + x] = wt * (G[k].x + 2 * acc[k]);
+        }
+    }
+}
+
 // ------------------------------------------------------------------ shared pieces of the FFT kernels
 // Every phase factor of a ring of N pixels is a power of omega = exp(-2 pi i / Q), Q = 2 N:
 //   twist exp(-i m phi0) = omega^m (phi0 = pi / N),  W_N^k = omega^(2 k),  W_{N/2}^k = omega^(4 k).
@@ -986,7 +1116,14 @@ static cudaError_t run_fft_stage(const HostPlan& hp, T* map, const double* d_w, 
     launch_class<T, ANALYSIS, 9>(P, D, map, d_w, use_w, st, side);
     launch_class<T, ANALYSIS, 8>(P, D, map, d_w, use_w, st, side);
     if (D.n_direct) {
-        if (ANALYSIS)
+        constexpr int CB = 8;
+        const size_t cb_ana = (size_t)DIRECT_MAX_N * (2 + CB) * sizeof(T);
+        const size_t cb_syn = ((size_t)DIRECT_MAX_N + (size_t)(D.max_mcut_direct + 1) * CB) * 2 * sizeof(T);
+        if (P.batch >= 4 && cb_syn <= 48 * 1024) {  // channel-blocked direct sums
+            const dim3 grid(D.n_direct, (P.batch + CB - 1) / CB);
+            if (ANALYSIS) ring_direct_analysis_cb_kernel<T, CB><<<grid, DIRECT_CB_THREADS, cb_ana, side>>>(P, D.direct, map, d_w, use_w);
+            else ring_direct_synthesis_cb_kernel<T, CB><<<grid, DIRECT_CB_THREADS, cb_syn, side>>>(P, D.direct, map, d_w, use_w);
+        } else if (ANALYSIS)
             ring_direct_analysis_kernel<T><<<dim3(D.n_direct, P.batch), FFT_THREADS, (size_t)DIRECT_MAX_N * 3 * sizeof(T), side>>>(
                 P, D.direct, map, d_w, use_w);
         else
