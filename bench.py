@@ -245,11 +245,12 @@ def main():
             dist.barrier()
         torch.cuda.synchronize()
 
+    # the sampler starts before the warm-up so that short workloads (a step of < 1 ms) still get samples under load
+    sampler = ClockSampler(local)
+    sampler.start()
     for _ in range(max(args.warmup, 3)):
         step()
     barrier()
-    sampler = ClockSampler(local)
-    sampler.start()
     ev = []
     e0 = torch.cuda.Event(enable_timing=True)
     e1 = torch.cuda.Event(enable_timing=True)
