@@ -112,6 +112,14 @@ int cuhpx_reorder(int nside, int batch, cuhpx_dtype_t dtype, int direction, cons
 /* host helper: RING index of NESTED pixel ipnest; -1 on bad arguments */
 long long cuhpx_nest2ring_index(int nside, long long ipnest);
 
+/* ---- spectral resampling ("upsampling and downsampling ... by truncating or extending
+ * spherical harmonic coefficients before applying the iSHT").  d_alm_out(l, m) = d_alm_in(l, m) for l <= lmax_in and
+ * m <= mmax_in, 0 elsewhere; both arrays [batch][nalm] complex, m-major packed for their own (lmax, mmax), DEVICE
+ * pointers, 16-byte aligned, no aliasing.  Resampling a map from nside_a to nside_b is then
+ * cuhpx_map2alm (nside_a) -> cuhpx_alm_resize -> cuhpx_alm2map (nside_b). */
+int cuhpx_alm_resize(int lmax_in, int mmax_in, int lmax_out, int mmax_out, int batch, cuhpx_dtype_t dtype,
+                     const void* d_alm_in, void* d_alm_out, cuhpx_stream_t stream);
+
 /* ---- the two stages of each direction, individually, for per-stage
  * measurement and stage-level parity tests.  The ring spectra live inside the workspace:
  *   spectra[b][ring][m], m = 0..m_cut(ring) (entries above m_cut(ring) are neither written nor read: there

@@ -91,3 +91,15 @@ def nest2ring(hmap_nest: np.ndarray, nside: int) -> np.ndarray:
 def ring2nest(hmap_ring: np.ndarray, nside: int) -> np.ndarray:
     """Reorder [..., npix] from RING to NESTED."""
     return hmap_ring[..., nest2ring_table(nside)]
+
+
+def alm_resize(alm: np.ndarray, lmax_in: int, mmax_in: int, lmax_out: int, mmax_out: int) -> np.ndarray:
+    """Truncate / zero-extend coefficients, the definition written out: every (l, m) of the output that
+    the input has is copied, the others are 0.  alm: [..., nalm_in], m-major packed index m (2 lmax + 1 - m) / 2 + l."""
+    nout = (mmax_out + 1) * (lmax_out + 1) - mmax_out * (mmax_out + 1) // 2
+    out = np.zeros(alm.shape[:-1] + (nout,), dtype=alm.dtype)
+    for m in range(mmax_out + 1):
+        for l in range(m, lmax_out + 1):
+            if m <= mmax_in and l <= lmax_in:
+                out[..., m * (2 * lmax_out + 1 - m) // 2 + l] = alm[..., m * (2 * lmax_in + 1 - m) // 2 + l]
+    return out

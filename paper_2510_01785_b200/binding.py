@@ -24,7 +24,7 @@ EXPORTS = [
     "cuhpx_alm2map_adjoint", "cuhpx_map2alm_adjoint", "cuhpx_spectra_stride", "cuhpx_workspace_spectra",
     "cuhpx_workspace_mcut", "cuhpx_analysis_fft_stage", "cuhpx_analysis_legendre_stage",
     "cuhpx_synthesis_legendre_stage", "cuhpx_synthesis_fft_stage", "cuhpx_fma_peak_probe", "cuhpx_workspace_stats",
-    "cuhpx_map2alm_iter", "cuhpx_reorder", "cuhpx_nest2ring_index",
+    "cuhpx_map2alm_iter", "cuhpx_reorder", "cuhpx_nest2ring_index", "cuhpx_alm_resize",
 ]
 CUHPX_NEST2RING, CUHPX_RING2NEST = 0, 1
 
@@ -63,6 +63,7 @@ def _load() -> ctypes.CDLL:
     lib.cuhpx_map2alm_adjoint.argtypes = [i, i, i, i, i, vp, vp, vp, vp, sz, vp]
     lib.cuhpx_map2alm_iter.argtypes = [i, i, i, i, i, vp, vp, vp, i, vp, vp, vp, sz, vp]
     lib.cuhpx_reorder.argtypes = [i, i, i, i, vp, vp, vp]
+    lib.cuhpx_alm_resize.argtypes = [i, i, i, i, i, i, vp, vp, vp]
     lib.cuhpx_nest2ring_index.restype = ctypes.c_longlong
     lib.cuhpx_nest2ring_index.argtypes = [i, ctypes.c_longlong]
     lib.cuhpx_spectra_stride.restype = sz
@@ -199,6 +200,18 @@ def cuhpx_map2alm_adjoint(nside, lmax, mmax, batch, dtype, d_galm, d_gmap, d_rin
 def cuhpx_reorder(nside, batch, dtype, direction, d_in, d_out, stream=None) -> None:
     _check(_lib.cuhpx_reorder(nside, batch, dtype, int(direction), _dev_ptr(d_in), _dev_ptr(d_out), _stream_ptr(stream)),
            "cuhpx_reorder")
+
+
+def cuhpx_alm_resize(lmax_in, mmax_in, lmax_out, mmax_out, batch, dtype, d_in, d_out, stream=None) -> None:
+    _check(_lib.cuhpx_alm_resize(lmax_in, mmax_in, lmax_out, mmax_out, batch, dtype, _dev_ptr(d_in), _dev_ptr(d_out),
+                                 _stream_ptr(stream)), "cuhpx_alm_resize")
+
+
+def alm_resize(alm: torch.Tensor, lmax_in: int, mmax_in: int, lmax_out: int, mmax_out: int) -> torch.Tensor:
+    """Truncate / zero-extend [batch, nalm] coefficients to another (lmax, mmax)."""
+    out = torch.empty(alm.shape[0], cuhpx_alm_count(lmax_out, mmax_out), dtype=alm.dtype, device=alm.device)
+    cuhpx_alm_resize(lmax_in, mmax_in, lmax_out, mmax_out, alm.shape[0], _dtype_code(alm.dtype), alm, out)
+    return out
 
 
 def cuhpx_nest2ring_index(nside: int, ipnest: int) -> int:

@@ -94,6 +94,8 @@ cudaError_t launch_accumulate(cuhpx_dtype_t dt, const void* d, void* a, size_t n
 // layout reordering (reorder.cu)
 cudaError_t launch_reorder(int nside, int batch, cuhpx_dtype_t dt, int to_ring, const void* in, void* out, cudaStream_t st);
 long long nest_to_ring_index(int nside, long long ipnest);
+cudaError_t launch_alm_resize(int lmax_in, int mmax_in, int lmax_out, int mmax_out, int batch, cuhpx_dtype_t dt,
+                              const void* in, void* out, cudaStream_t st);
 
 cudaError_t fma_peak_probe(cuhpx_dtype_t dt, int iters, float* ms, double* count, cudaStream_t st);
 

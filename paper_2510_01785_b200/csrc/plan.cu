@@ -511,6 +511,15 @@ int cuhpx_reorder(int nside, int batch, cuhpx_dtype_t dt, int direction, const v
     return CUHPX_OK;
 }
 
+int cuhpx_alm_resize(int lmax_in, int mmax_in, int lmax_out, int mmax_out, int batch, cuhpx_dtype_t dt,
+                     const void* d_in, void* d_out, cuhpx_stream_t stream) {
+    if (lmax_in < 0 || mmax_in < 0 || mmax_in > lmax_in || lmax_out < 0 || mmax_out < 0 || mmax_out > lmax_out) return CUHPX_EINVAL;
+    if (batch < 1 || (dt != CUHPX_F32 && dt != CUHPX_F64)) return CUHPX_EINVAL;
+    if (!d_in || !d_out || d_in == d_out || ((uintptr_t)d_in & 15) || ((uintptr_t)d_out & 15)) return CUHPX_EINVAL;
+    CUDA_OR_FAIL(launch_alm_resize(lmax_in, mmax_in, lmax_out, mmax_out, batch, dt, d_in, d_out, (cudaStream_t)stream));
+    return CUHPX_OK;
+}
+
 long long cuhpx_nest2ring_index(int nside, long long ipnest) {
     if (nside < 1 || !is_pow2(nside) || nside > (1 << 13) || ipnest < 0 || ipnest >= 12LL * nside * nside) return -1;
     return nest_to_ring_index(nside, ipnest);

@@ -11,6 +11,7 @@
 // index arithmetic is needed (the reverse direction reads along the same runs).  Roofline: HBM, 2 x map bytes.
 #include <cuda_runtime.h>
 #include <stdint.h>
+#include <string.h>
 
 #include "cuhpx_internal.h"
 
@@ -224,6 +225,33 @@ static cudaError_t run_reorder(int nside, int batch, int to_ring, const void* in
 cudaError_t launch_reorder(int nside, int batch, cuhpx_dtype_t dt, int to_ring, const void* in, void* out, cudaStream_t st) {
     return dt == CUHPX_F64 ? run_reorder<uint64_t>(nside, batch, to_ring, in, out, st)
                            : run_reorder<uint32_t>(nside, batch, to_ring, in, out, st);
+}
+
+// ------------------------------------------------------------------ spectral resampling
+// "upsampling and downsampling of HEALPix data by truncating or extending spherical harmonic coefficients before
+// applying the iSHT": out(l, m) = in(l, m) where the input has that coefficient, else 0.  W = one complex value.
+template <typename W>
+__global__ void __launch_bounds__(256) alm_resize_kernel(int lmax_in, int mmax_in, int lmax_out, long long nalm_in,
+                                                         long long nalm_out, const W* __restrict__ in, W* __restrict__ out) {
+    const int m = blockIdx.x, b = blockIdx.y;
+    const long long base_out = (long long)m * (2LL * lmax_out + 1 - m) / 2;  // index of (l = 0, m), m-major packed
+    const long long base_in = (long long)m * (2LL * lmax_in + 1 - m) / 2;
+    W zero;
+    memset(&zero, 0, sizeof(W));
+    for (int l = m + threadIdx.x; l <= lmax_out; l += blockDim.x) {
+        const bool have = m <= mmax_in && l <= lmax_in;
+        out[(size_t)b * nalm_out + base_out + l] = have ? in[(size_t)b * nalm_in + base_in + l] : zero;
+    }
+}
+
+cudaError_t launch_alm_resize(int lmax_in, int mmax_in, int lmax_out, int mmax_out, int batch, cuhpx_dtype_t dt,
+                              const void* in, void* out, cudaStream_t st) {
+    const long long nin = (long long)(mmax_in + 1) * (lmax_in + 1) - (long long)mmax_in * (mmax_in + 1) / 2;
+    const long long nout = (long long)(mmax_out + 1) * (lmax_out + 1) - (long long)mmax_out * (mmax_out + 1) / 2;
+    dim3 grid((unsigned)(mmax_out + 1), (unsigned)batch);
+    if (dt == CUHPX_F64) alm_resize_kernel<double2><<<grid, 256, 0, st>>>(lmax_in, mmax_in, lmax_out, nin, nout, (const double2*)in, (double2*)out);
+    else alm_resize_kernel<float2><<<grid, 256, 0, st>>>(lmax_in, mmax_in, lmax_out, nin, nout, (const float2*)in, (float2*)out);
+    return cudaGetLastError();
 }
 
 }  // namespace cuhpx
