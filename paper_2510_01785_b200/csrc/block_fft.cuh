@@ -39,6 +39,15 @@ template <> struct Xchg<double> {
         a = re[q];
         b = im[q];
     }
+    // q is already a padded position
+    __device__ __forceinline__ void stq(int q, double a, double b) const {
+        re[q] = a;
+        im[q] = b;
+    }
+    __device__ __forceinline__ void ldq(int q, double& a, double& b) const {
+        a = re[q];
+        b = im[q];
+    }
 };
 template <> struct Xchg<float> {
     float2* z;
@@ -47,6 +56,13 @@ template <> struct Xchg<float> {
     __device__ __forceinline__ void st(int p, float a, float b) const { z[padi(p)] = make_float2(a, b); }
     __device__ __forceinline__ void ld(int p, float& a, float& b) const {
         const float2 v = z[padi(p)];
+        a = v.x;
+        b = v.y;
+    }
+    // q is already a padded position
+    __device__ __forceinline__ void stq(int q, float a, float b) const { z[q] = make_float2(a, b); }
+    __device__ __forceinline__ void ldq(int q, float& a, float& b) const {
+        const float2 v = z[q];
         a = v.x;
         b = v.y;
     }
@@ -240,19 +256,41 @@ template <typename T, int LOGN, int LOGQ = LOGN> struct BlockFFT {
         return (int)(__brev((unsigned)p) >> (32 - LOGN));
     }
 
+    // Exchange positions of a thread's R registers in pass S are base + rho LR.  When LR is a multiple of 16 the
+    // padding p -> p + (p >> 4) is affine in rho, so ONE padded base per butterfly and compile-time offsets replace
+    // a shift-add per element (ncu: integer address arithmetic was ~22 % of the issued instructions of the fp32
+    // kernels, which are issue-bound).
     template <int S> static __device__ __forceinline__ void load(T (&re)[E], T (&im)[E], const Xchg<T>& x, int tid) {
-        constexpr int R = PassRadix<LOGN, S>::value;
+        constexpr int R = PassRadix<LOGN, S>::value, L = PassLen<LOGN, S>::value, LR = L / R;
 #pragma unroll
-        for (int c = 0; c < E / R; ++c)
+        for (int c = 0; c < E / R; ++c) {
+            const int u = tid + NT * c;
+            const int base = (u / LR) * L + (u % LR);
+            if constexpr (LR % 16 == 0) {
+                const int pb = padi(base);
 #pragma unroll
-            for (int r = 0; r < R; ++r) x.ld(pos<S>(tid, c, r), re[c * R + r], im[c * R + r]);
+                for (int r = 0; r < R; ++r) x.ldq(pb + r * (LR + LR / 16), re[c * R + r], im[c * R + r]);
+            } else {
+#pragma unroll
+                for (int r = 0; r < R; ++r) x.ld(base + r * LR, re[c * R + r], im[c * R + r]);
+            }
+        }
     }
     template <int S> static __device__ __forceinline__ void store(const T (&re)[E], const T (&im)[E], const Xchg<T>& x, int tid) {
-        constexpr int R = PassRadix<LOGN, S>::value;
+        constexpr int R = PassRadix<LOGN, S>::value, L = PassLen<LOGN, S>::value, LR = L / R;
 #pragma unroll
-        for (int c = 0; c < E / R; ++c)
+        for (int c = 0; c < E / R; ++c) {
+            const int u = tid + NT * c;
+            const int base = (u / LR) * L + (u % LR);
+            if constexpr (LR % 16 == 0) {
+                const int pb = padi(base);
 #pragma unroll
-            for (int r = 0; r < R; ++r) x.st(pos<S>(tid, c, r), re[c * R + r], im[c * R + r]);
+                for (int r = 0; r < R; ++r) x.stq(pb + r * (LR + LR / 16), re[c * R + r], im[c * R + r]);
+            } else {
+#pragma unroll
+                for (int r = 0; r < R; ++r) x.st(base + r * LR, re[c * R + r], im[c * R + r]);
+            }
+        }
     }
 
     template <int S> static __device__ __forceinline__ void fwd_pass(T (&re)[E], T (&im)[E], const Xchg<T>& x,
