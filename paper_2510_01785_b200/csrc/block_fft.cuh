@@ -110,6 +110,7 @@ __device__ __forceinline__ void fill_roots_any(typename V2<T>::type* base, int Q
 
 // radix plans: passes in DIF order
 template <int LOGN> struct FftPlan;
+template <> struct FftPlan<7> { static constexpr int NT = 32, NP = 4; static constexpr int R0 = 2, R1 = 4, R2 = 4, R3 = 4; };
 template <> struct FftPlan<8> { static constexpr int NT = 32, NP = 3; static constexpr int R0 = 8, R1 = 8, R2 = 4, R3 = 1; };
 template <> struct FftPlan<9> { static constexpr int NT = 64, NP = 3; static constexpr int R0 = 8, R1 = 8, R2 = 8, R3 = 1; };
 template <> struct FftPlan<10> { static constexpr int NT = 64, NP = 3; static constexpr int R0 = 16, R1 = 16, R2 = 4, R3 = 1; };

@@ -25,7 +25,7 @@ namespace cuhpx {
 
 constexpr int DIRECT_MAX_N = 256;
 constexpr int FFT_THREADS = 256;  // direct kernels
-constexpr int MIN_LOG = 8, MAX_LOG = 13;
+constexpr int MIN_LOG = 7, MAX_LOG = 13;  // LOG 7: the belt rings of nside 64 (N = 256) as one-warp FFTs
 
 // exp(sign * i * pi * num / den) from exact integers (num already reduced mod 2 den); direct kernels only
 __device__ __forceinline__ void cispi_ratio(long long num, long long den, double sign, double& c, double& s) {
@@ -850,8 +850,8 @@ static void classify(const HostPlan& hp, RingFftLists& L) {
         R.r = r;
         R.pad0 = R.pad1 = 0;
         const int N = R.N;
-        if (N <= DIRECT_MAX_N) L.direct.push_back(R);
-        else if (N == 4 * d.nside) L.pow2[ilog2_ceil(N) - 1].push_back(R);  // belt rings (N = 4 nside = 2^k)
+        if (N == 4 * d.nside && ilog2_ceil(N) - 1 >= MIN_LOG) L.pow2[ilog2_ceil(N) - 1].push_back(R);  // belt rings (N = 4 nside = 2^k)
+        else if (N <= DIRECT_MAX_N) L.direct.push_back(R);
         else {  // cap rings, chirp-z for every i (the few i = 2^k among them are not worth launches of their own)
             const int i = N / 4, lm = blue_logm(i);
             L.blue[lm].push_back(R);
@@ -961,13 +961,13 @@ template <typename T> static cudaError_t build_tables_t(FftDev& D, const RingFft
     if ((e = cudaGetDevice(&dev)) != cudaSuccess) return e;
     if ((e = cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev)) != cudaSuccess) return e;
 #define CUHPX_ATTR(LOG) if ((e = set_smem_attrs<T, LOG>(D, sms)) != cudaSuccess) return e;
-    CUHPX_ATTR(8) CUHPX_ATTR(9) CUHPX_ATTR(10) CUHPX_ATTR(11) CUHPX_ATTR(12) CUHPX_ATTR(13)
+    CUHPX_ATTR(7) CUHPX_ATTR(8) CUHPX_ATTR(9) CUHPX_ATTR(10) CUHPX_ATTR(11) CUHPX_ATTR(12) CUHPX_ATTR(13)
 #undef CUHPX_ATTR
     twiddle_table_kernel<T><<<(twlen + 255) / 256, 256, 0, st>>>((T2*)(base + Y.off_tw), twlen);
     twiddle_table_kernel<double><<<(twlen + 255) / 256, 256, 0, st>>>((double2*)(base + Y.off_tw64), twlen);
     if ((e = cudaGetLastError()) != cudaSuccess) return e;
 #define CUHPX_FILT(LOG) if ((e = build_filters<T, LOG>(L, Y, base, st, twlen)) != cudaSuccess) return e;
-    CUHPX_FILT(8) CUHPX_FILT(9) CUHPX_FILT(10) CUHPX_FILT(11) CUHPX_FILT(12) CUHPX_FILT(13)
+    CUHPX_FILT(7) CUHPX_FILT(8) CUHPX_FILT(9) CUHPX_FILT(10) CUHPX_FILT(11) CUHPX_FILT(12) CUHPX_FILT(13)
 #undef CUHPX_FILT
     return cudaSuccess;
 }
@@ -1115,6 +1115,7 @@ static cudaError_t run_fft_stage(const HostPlan& hp, T* map, const double* d_w, 
     launch_class<T, ANALYSIS, 10>(P, D, map, d_w, use_w, st, side);
     launch_class<T, ANALYSIS, 9>(P, D, map, d_w, use_w, st, side);
     launch_class<T, ANALYSIS, 8>(P, D, map, d_w, use_w, st, side);
+    launch_class<T, ANALYSIS, 7>(P, D, map, d_w, use_w, st, side);
     if (D.n_direct) {
         constexpr int CB = 8;
         const size_t cb_ana = (size_t)DIRECT_MAX_N * (2 + CB) * sizeof(T);
