@@ -570,7 +570,11 @@ template <typename T, int LOGM> struct BlueSmem {
     static constexpr size_t off_z = Xchg<T>::bytes(M);
     static constexpr size_t off_rq = off_z + sizeof(T) * 2 * ((size_t)M / 2 + 2);
     static constexpr size_t off_rm = off_rq + sizeof(T) * 2 * (size_t)roots_len(4 * M + 8);  // Q = 8 i <= 4 M + 8
-    static constexpr size_t total = off_rm + sizeof(T) * 2 * (size_t)roots_len(M);
+    static constexpr size_t off_cs = off_rm + sizeof(T) * 2 * (size_t)roots_len(M);
+    // fp32 only: the thread's own chirp factors [e][tid] (each is needed 4 times: before / after the convolution of
+    // both sub-sequences; ~20 instructions to rebuild, one LDS.64 to reload).  fp64 has no shared memory to spare.
+    static constexpr bool KEEP_CHIRP = sizeof(T) == 4 && LOGM <= 12;  // beyond, the table would halve the resident CTAs
+    static constexpr size_t total = off_cs + (KEEP_CHIRP ? sizeof(T) * 2 * (size_t)M : 0);
 };
 
 template <typename T, int LOGM>
@@ -599,6 +603,18 @@ __global__ void __launch_bounds__(FftPlan<LOGM>::NT, MinBlocks<T, LOGM>::blue) r
     const float inv_twoi = 1.0f / (float)(2 * i);
     __syncthreads();
     const Roots<T> rt(rq), rtM(rm);
+    T2* cs = reinterpret_cast<T2*>(smem_raw + SM::off_cs) + tid;  // [e * NT]: private to this thread
+    if constexpr (SM::KEEP_CHIRP) {
+#pragma unroll
+        for (int e = 0; e < E; ++e) {
+            const int u = F::index0(tid, e);
+            T2 v;
+            v.x = 1;
+            v.y = 0;
+            if (u < i) rt.template get<-1>(chirp_index(u, 2 * i, inv_twoi), v.x, v.y);
+            cs[e * NT] = v;
+        }
+    }
     T re[E], im[E];
 #pragma unroll 1
     for (int sub = 0; sub < 2; ++sub) {
@@ -610,7 +626,13 @@ __global__ void __launch_bounds__(FftPlan<LOGM>::NT, MinBlocks<T, LOGM>::blue) r
             if (u < i) {
                 const T2 z = src[2 * u + sub];
                 T c, s;
-                rt.template get<-1>(chirp_index(u, 2 * i, inv_twoi), c, s);
+                if constexpr (SM::KEEP_CHIRP) {
+                    const T2 v = cs[e * NT];
+                    c = v.x;
+                    s = v.y;
+                } else {
+                    rt.template get<-1>(chirp_index(u, 2 * i, inv_twoi), c, s);
+                }
                 re[e] = z.x * c - z.y * s;
                 im[e] = z.x * s + z.y * c;
             }
@@ -621,7 +643,13 @@ __global__ void __launch_bounds__(FftPlan<LOGM>::NT, MinBlocks<T, LOGM>::blue) r
             const int u = F::index0(tid, e);
             if (u < i) {
                 T c, s;
-                rt.template get<-1>(chirp_index(u, 2 * i, inv_twoi), c, s);
+                if constexpr (SM::KEEP_CHIRP) {
+                    const T2 v = cs[e * NT];
+                    c = v.x;
+                    s = v.y;
+                } else {
+                    rt.template get<-1>(chirp_index(u, 2 * i, inv_twoi), c, s);
+                }
                 const T vr = re[e] * c - im[e] * s, vi = re[e] * s + im[e] * c;
                 if (sub == 0) {
                     T2 v;
@@ -702,6 +730,18 @@ __global__ void __launch_bounds__(FftPlan<LOGM>::NT, MinBlocks<T, LOGM>::blue) r
     const float inv_twoi = 1.0f / (float)(2 * i);
     __syncthreads();
     const Roots<T> rt(rq), rtM(rm);
+    T2* cs = reinterpret_cast<T2*>(smem_raw + SM::off_cs) + tid;  // [e * NT]: private to this thread
+    if constexpr (SM::KEEP_CHIRP) {
+#pragma unroll
+        for (int e = 0; e < E; ++e) {
+            const int u = F::index0(tid, e);
+            T2 v;
+            v.x = 1;
+            v.y = 0;
+            if (u < i) rt.template get<-1>(chirp_index(u, 2 * i, inv_twoi), v.x, v.y);
+            cs[e * NT] = v;
+        }
+    }
     const T2* G = reinterpret_cast<const T2*>(P.spectra) + ((size_t)ch * P.nrings + R.r) * P.mstride;
     T re[E], im[E];
 #pragma unroll 1
@@ -715,7 +755,13 @@ __global__ void __launch_bounds__(FftPlan<LOGM>::NT, MinBlocks<T, LOGM>::blue) r
                 T yr, yi;
                 synth_packed_input<T, false>(G, 2 * u + sub, N, R.mcut, R.shifted, rt, yr, yi);
                 T c, s;
-                rt.template get<-1>(chirp_index(u, 2 * i, inv_twoi), c, s);
+                if constexpr (SM::KEEP_CHIRP) {
+                    const T2 v = cs[e * NT];
+                    c = v.x;
+                    s = v.y;
+                } else {
+                    rt.template get<-1>(chirp_index(u, 2 * i, inv_twoi), c, s);
+                }
                 re[e] = yr * c - yi * s;
                 im[e] = yr * s + yi * c;
             }
@@ -726,7 +772,13 @@ __global__ void __launch_bounds__(FftPlan<LOGM>::NT, MinBlocks<T, LOGM>::blue) r
             const int u = F::index0(tid, e);
             if (u < i) {
                 T c, s;
-                rt.template get<-1>(chirp_index(u, 2 * i, inv_twoi), c, s);
+                if constexpr (SM::KEEP_CHIRP) {
+                    const T2 v = cs[e * NT];
+                    c = v.x;
+                    s = v.y;
+                } else {
+                    rt.template get<-1>(chirp_index(u, 2 * i, inv_twoi), c, s);
+                }
                 const T vr = re[e] * c - im[e] * s, vi = re[e] * s + im[e] * c;
                 if (sub == 0) {
                     T2 v;
