@@ -451,7 +451,7 @@ __device__ __forceinline__ typename V2<T>::type analysis_unpack(T z1r, T z1i, T 
 template <typename T, int LOG> struct MinBlocks {
     static constexpr int NT = FftPlan<LOG>::NT;
     static constexpr int value = (sizeof(T) == 4 ? 1024 : 512) / NT > 16 ? 16 : (sizeof(T) == 4 ? 1024 : 512) / NT;
-    static constexpr int blue = 512 / NT;
+    static constexpr int blue = (sizeof(T) == 4 ? 768 : 512) / NT;  // fp32: 80 registers, 6 CTAs of 128 threads per SM (measured best of 4 / 6 / 8)
 };
 
 // ------------------------------------------------------------------ power-of-two rings
