@@ -169,6 +169,11 @@ def test_map2alm_iter_matches_oracle(nside, lmax, batch, dtype, n_iter, weighted
     (1, 0, 0, 1, "f64"), (1, 3, 3, 1, "f64"), (2, 8, 8, 2, "f64"), (4, 16, 16, 1, "f64"), (4, 11, 7, 3, "f64"),
     (8, 16, 0, 1, "f64"), (16, 40, 33, 1, "f64"), (16, 47, 47, 5, "f32"), (8, 23, 23, 1, "f32"),
     (64, 200, 150, 2, "f64"), (32, 95, 95, 7, "f32"), (128, 300, 300, 1, "f64"),
+    # kernel-selection corners: channel-blocked direct sums in fp64; 32-degree contraction with several ring chunks and
+    # the combine kernel; 64-degree contraction accumulating in place over ring chunks with mmax < lmax and a ragged
+    # channel group; packed-FMA synthesis with two channel groups, the second ragged (both CTA shapes)
+    (32, 64, 64, 5, "f64"), (256, 300, 300, 6, "f32"), (256, 600, 450, 6, "f32"), (64, 128, 128, 11, "f32"),
+    (128, 520, 520, 9, "f32"),
 ])
 def test_small_and_ragged_cases(nside, lmax, mmax, batch, dtype):
     """mmax < lmax, lmax far above 2 nside (every polar ring aliases), batch not a multiple of the channel
