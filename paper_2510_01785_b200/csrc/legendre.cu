@@ -208,7 +208,8 @@ __device__ __forceinline__ void warp_reduce_split(T (&v)[NV], int lane) {
     }
 }
 
-template <typename T, int BT, int R, int LT, int NT, int GL = GROUP_L>
+// SEQ: one CTA walks the ring chunks of its order m and accumulates a_lm in place (no partial arrays / combine kernel)
+template <typename T, int BT, int R, int LT, int NT, int GL = GROUP_L, bool SEQ = false>
 __global__ void __launch_bounds__(NT, 384 / NT) legendre_analysis_kernel(LegArgs a) {
     using T2 = typename Vec2<T>::type;
     constexpr int NW = NT / 32;
@@ -221,9 +222,10 @@ __global__ void __launch_bounds__(NT, 384 / NT) legendre_analysis_kernel(LegArgs
     static_assert(NV >= 4, "reduction tile");
     const DevPlan& P = a.p;
     const int m = blockIdx.x;
-    const int chunk = blockIdx.y;
     const int ch0 = blockIdx.z * BT;
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    int buf = 0;
+    for (int chunk = SEQ ? 0 : (int)blockIdx.y;; ++chunk) {
     const int jbase = P.jmin[m] + chunk * (NT * R);
     if (jbase >= P.npairs) return;
 
@@ -287,7 +289,6 @@ __global__ void __launch_bounds__(NT, 384 / NT) legendre_analysis_kernel(LegArgs
 
     const int nl = P.lmax - m + 1;  // l values of this m
     bool warp_active = __any_sync(0xffffffffu, nact > 0);
-    int buf = 0;
     // alpha of the steps that produce degrees l = m + t0 + 1 + i; the next tile is fetched into a register while
     // the current one is consumed, so no global-load latency sits between two tiles
     double nextA = (tid < CT && 1 + tid < nl) ? P.coef_alpha[abase + m + 1 + tid] : 0.0;
@@ -303,11 +304,17 @@ __global__ void __launch_bounds__(NT, 384 / NT) legendre_analysis_kernel(LegArgs
         for (int g0 = 0; g0 < tend; g0 += GL) {
             // s_l of this thread's output element, requested before the group's arithmetic
             double oscl[NOUT];
+            T oold[NOUT];  // SEQ: what the earlier ring chunks left in a_lm
 #pragma unroll
             for (int q = 0; q < NOUT; ++q) {
                 const int e = tid + NT * q;
                 const int k = t0 + g0 + (e / NV) * LT + (e % NV) / (BT * 2);
                 oscl[q] = (e < TPG * NV && k < nl) ? outscale * P.coef_scale[abase + m + k] : 0.0;
+                oold[q] = 0;
+                if (SEQ && chunk > 0) {
+                    const int v = e % NV, ch = ch0 + (v / 2) % BT;
+                    if (e < TPG * NV && k < nl && ch < P.batch) oold[q] = out[((size_t)ch * P.nalm + abase + m + k) * 2 + (v & 1)];
+                }
             }
 #pragma unroll 1
             for (int ti = 0; ti < TPG; ++ti) {
@@ -387,7 +394,7 @@ __global__ void __launch_bounds__(NT, 384 / NT) legendre_analysis_kernel(LegArgs
                 const int k = t0 + g0 + ti * LT + i;  // l - m
                 const int ch = ch0 + c;
                 if (k < nl && ch < P.batch) {
-                    T o = (T)(oscl[q] * (double)sum);  // lambda = s_l mu
+                    T o = oold[q] + (T)(oscl[q] * (double)sum);  // lambda = s_l mu
                     if (m == 0 && ri == 1) o = 0;  // Im a_l0 is exactly zero
                     out[((size_t)ch * P.nalm + abase + m + k) * 2 + ri] = o;
                 }
@@ -395,6 +402,9 @@ __global__ void __launch_bounds__(NT, 384 / NT) legendre_analysis_kernel(LegArgs
             buf ^= 1;
         }
     }
+    if (!SEQ) return;
+    __syncthreads();  // the next chunk reuses the shared tiles
+    }  // chunk
 }
 
 // ------------------------------------------------------------------ analysis, batched fp32 (row a3 as a contraction)
@@ -1142,7 +1152,8 @@ template <> struct LegCfg<float, 4> { static constexpr int NT = 128, R = 4, LT =
 static bool use_gemm64(int lmax) { return lmax >= 512; }
 
 int legendre_chunk_pairs(cuhpx_dtype_t dt, int batch, int lmax, int npairs) {
-    if (dt == CUHPX_F64) return LegCfg<double, 1>::NT * LegCfg<double, 1>::R;
+    // one "chunk" as far as the plan is concerned wherever the kernel walks the ring chunks itself
+    if (dt == CUHPX_F64) return npairs > LegCfg<double, 1>::NT * LegCfg<double, 1>::R ? npairs : LegCfg<double, 1>::NT * LegCfg<double, 1>::R;
     if (batch >= 5) return use_gemm64(lmax) ? (npairs > GK ? npairs : GK) : GK;
     return batch >= 4 ? LegCfg<float, 4>::NT * LegCfg<float, 4>::R : LegCfg<float, 1>::NT * LegCfg<float, 1>::R;
 }
@@ -1186,17 +1197,17 @@ static cudaError_t run_synthesis(const HostPlan& hp, const void* d_alm, int adjo
     return cudaGetLastError();
 }
 
-template <typename T, int BT, int R, int LT, int NT, int GL>
+template <typename T, int BT, int R, int LT, int NT, int GL, bool SEQ = false>
 static cudaError_t run_analysis_cfg(const HostPlan& hp, void* d_alm, int adjoint, cudaStream_t st) {
     const DevPlan& P = hp.d;
     LegArgs a;
     a.p = P;
     a.in = nullptr;
     a.adjoint = adjoint;
-    a.to_partial = P.nchunk_max > 1;
+    a.to_partial = !SEQ && P.nchunk_max > 1;
     a.out = a.to_partial ? P.partial : d_alm;
-    dim3 grid(P.mmax + 1, P.nchunk_max, (P.batch + BT - 1) / BT);
-    legendre_analysis_kernel<T, BT, R, LT, NT, GL><<<grid, NT, 0, st>>>(a);
+    dim3 grid(P.mmax + 1, SEQ ? 1 : P.nchunk_max, (P.batch + BT - 1) / BT);
+    legendre_analysis_kernel<T, BT, R, LT, NT, GL, SEQ><<<grid, NT, 0, st>>>(a);
     cudaError_t e = cudaGetLastError();
     if (e != cudaSuccess) return e;
     if (a.to_partial) {
@@ -1258,7 +1269,8 @@ static cudaError_t run_analysis_gemm(const HostPlan& hp, void* d_alm, int adjoin
 
 // Configurations below are the winners of sweeps on B200 (profiles/r1_legendre_tuning.md).
 cudaError_t launch_legendre_analysis(const HostPlan& hp, void* d_alm, int adjoint, cudaStream_t st) {
-    if (hp.dtype == CUHPX_F64) return run_analysis_cfg<double, 1, 8, 8, 128, 64>(hp, d_alm, adjoint, st);
+    // in-place accumulation over ring chunks (SEQ): cfg5 88.3 -> 87.0 ms, 3.7 GB of partial writes and 4.3 GB of workspace gone
+    if (hp.dtype == CUHPX_F64) return run_analysis_cfg<double, 1, 8, 8, 128, 64, true>(hp, d_alm, adjoint, st);
     if (hp.d.batch >= 5) return run_analysis_gemm(hp, d_alm, adjoint, st);
     if (hp.d.batch >= 4) return run_analysis<float, 4>(hp, d_alm, adjoint, st);
     return run_analysis<float, 1>(hp, d_alm, adjoint, st);
