@@ -809,8 +809,10 @@ template <typename T, int BT, int R, int NT>
 __global__ void __launch_bounds__(NT) legendre_synthesis_kernel(LegArgs a) {
     using T2 = typename Vec2<T>::type;
     const DevPlan& P = a.p;
-    const int m = blockIdx.x;
-    const int chunk = blockIdx.y;
+    // grid: x = ring chunk (fastest), y = m: the chunk-CTAs of one order run together and share its a_lm / alpha / s_l
+    // rows through L2 instead of each fetching them from DRAM
+    const int m = blockIdx.y;
+    const int chunk = blockIdx.x;
     const int ch0 = blockIdx.z * BT;
     const int tid = threadIdx.x;
     const int jbase = P.jmin[m] + chunk * (NT * R);
@@ -979,8 +981,10 @@ template <int BT, int R, int NT, int MINB>
 __global__ void __launch_bounds__(NT, MINB) legendre_synthesis_f32x2_kernel(LegArgs a) {
     using T = float;
     const DevPlan& P = a.p;
-    const int m = blockIdx.x;
-    const int chunk = blockIdx.y;
+    // grid: x = ring chunk (fastest), y = m: the chunk-CTAs of one order run together and share its a_lm / alpha / s_l
+    // rows through L2 instead of each fetching them from DRAM
+    const int m = blockIdx.y;
+    const int chunk = blockIdx.x;
     const int ch0 = blockIdx.z * BT;
     const int tid = threadIdx.x;
     const int jbase = P.jmin[m] + chunk * (NT * R);
@@ -1192,7 +1196,7 @@ static cudaError_t run_synthesis(const HostPlan& hp, const void* d_alm, int adjo
     a.adjoint = adjoint;
     a.to_partial = 0;
     const int chunk = C::NTS * C::RS;
-    dim3 grid(P.mmax + 1, (P.npairs + chunk - 1) / chunk, (P.batch + BT - 1) / BT);
+    dim3 grid((P.npairs + chunk - 1) / chunk, P.mmax + 1, (P.batch + BT - 1) / BT);
     legendre_synthesis_kernel<T, BT, C::RS, C::NTS><<<grid, C::NTS, 0, st>>>(a);
     return cudaGetLastError();
 }
@@ -1228,7 +1232,7 @@ static cudaError_t run_synthesis_cfg(const HostPlan& hp, const void* d_alm, int 
     a.adjoint = adjoint;
     a.to_partial = 0;
     const int chunk = NTS * RS;
-    dim3 grid(P.mmax + 1, (P.npairs + chunk - 1) / chunk, (P.batch + BT - 1) / BT);
+    dim3 grid((P.npairs + chunk - 1) / chunk, P.mmax + 1, (P.batch + BT - 1) / BT);
     legendre_synthesis_kernel<T, BT, RS, NTS><<<grid, NTS, 0, st>>>(a);
     return cudaGetLastError();
 }
@@ -1286,7 +1290,7 @@ static cudaError_t run_synthesis_f32x2(const HostPlan& hp, const void* d_alm, in
     a.adjoint = adjoint;
     a.to_partial = 0;
     const int chunk = NT * R;
-    dim3 grid(P.mmax + 1, (P.npairs + chunk - 1) / chunk, (P.batch + BT - 1) / BT);
+    dim3 grid((P.npairs + chunk - 1) / chunk, P.mmax + 1, (P.batch + BT - 1) / BT);
     legendre_synthesis_f32x2_kernel<BT, R, NT, MINB><<<grid, NT, 0, st>>>(a);
     return cudaGetLastError();
 }
