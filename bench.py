@@ -6,9 +6,11 @@
 A "step" is one pass of the whole hot path over one batch: map2alm + alm2map + alm2map_adjoint + map2alm_adjoint
 (SURVEY 8(a) rows a1, a3, s1, s2, d1, d2), i.e. 4 * batch transforms.  Default workload: BASELINE configs[4]
 (nside 4096, lmax = mmax = 8191, batch 1, fp64), the largest configuration the metric is quoted on.
-`value` is device-timed with the inputs resident in HBM; `e2e` goes through the public API with pinned HOST
-buffers and the host<->device copies inside the timed region.  N > 1 runs one independent replica per GPU
-(batch channels are independent: no data-path collective).
+`value` is device-timed (two CUDA events around K back-to-back steps of the four public calls) with the inputs
+resident in HBM; `e2e` goes through the same calls with pinned HOST buffers and the host<->device copies inside the
+timed region; the per-stage times behind `roofline` come from a separate, instrumented pass over the stage-level
+entry points.  N > 1 runs one independent replica per GPU (batch channels are independent: no data-path collective;
+DESIGN.md "Multi-GPU"); launched without torchrun, `--gpus N` spawns the N ranks itself.
 """
 from __future__ import annotations
 
@@ -28,7 +30,7 @@ import numpy as np  # noqa: E402
 
 from paper_2510_01785_b200 import replicas, synth  # noqa: E402
 
-METRIC = "map2alm/alm2map transforms/s at Nside 1024-4096; % of FP64/HBM roofline"
+METRIC = "map2alm/alm2map transforms/s at Nside 1024\u20134096; % of FP64/HBM roofline"  # byte-identical to BASELINE.json
 UNIT = "transforms/s"
 # B200 plain-ALU peaks: 148 SMs x 64 (128) FP64 (FP32) FMA lanes x 2 flop x 1.965 GHz
 PEAK_TFLOPS = {"f64": 148 * 64 * 2 * 1.965e9 / 1e12, "f32": 148 * 128 * 2 * 1.965e9 / 1e12}
@@ -160,20 +162,58 @@ class ClockSampler:
         return out
 
 
+def run_reorder():
+    """--workload reorder: throughput of cuhpx_reorder (NESTED <-> RING, paper section III-B) on one
+    GPU, one JSON line per case.  Device-timed with CUDA events (3 warm-ups, 20 calls); roofline HBM: algorithmic bytes =
+    2 x batch x npix x element size (every element read once and written once)."""
+    import torch
+
+    from paper_2510_01785_b200 import binding as B
+
+    peak, _ = load_peaks()
+    for nside, batch, dt in [(1024, 8, torch.float32), (4096, 1, torch.float64), (4096, 4, torch.float32),
+                             (2048, 8, torch.float64)]:
+        npix = 12 * nside * nside
+        a = torch.randn(batch, npix, dtype=dt, device="cuda")
+        o = torch.empty_like(a)
+        code = B._dtype_code(dt)
+        for d, name in [(B.CUHPX_NEST2RING, "nest2ring"), (B.CUHPX_RING2NEST, "ring2nest")]:
+            for _ in range(3):
+                B.cuhpx_reorder(nside, batch, code, d, a, o)
+            torch.cuda.synchronize()
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record()
+            for _ in range(20):
+                B.cuhpx_reorder(nside, batch, code, d, a, o)
+            e1.record()
+            torch.cuda.synchronize()
+            ms = e0.elapsed_time(e1) / 20
+            gbs = 2 * a.numel() * a.element_size() / ms / 1e6
+            print(json.dumps({"op": name, "nside": nside, "batch": batch, "dtype": str(dt).split(".")[-1], "ms": ms,
+                              "roofline": {"bound": "hbm", "achieved": gbs, "peak": peak, "unit": "GB/s", "frac": gbs / peak}}),
+                  flush=True)
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
     ap.add_argument("--steps", type=int, default=3)
     ap.add_argument("--warmup", type=int, default=3)
-    ap.add_argument("--workload", default="cfg5", choices=sorted(synth.CONFIGS))
+    ap.add_argument("--workload", default="cfg5", choices=sorted(synth.CONFIGS) + ["reorder"])
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
     args = ap.parse_args()
+    if args.workload == "reorder":
+        run_reorder()
+        return
     cfg = dict(synth.CONFIGS[args.workload])
     cfg["index"] = int(args.workload[3:]) - 1
     if args.impl == "reference":
         run_reference(args, cfg)
         return
+    if args.gpus > 1 and "WORLD_SIZE" not in os.environ:
+        # launched plainly: become the launcher of N ranks (one per GPU) of this same command line
+        raise SystemExit(replicas.spawn_ranks(args.gpus, [os.path.abspath(__file__)] + sys.argv[1:]))
 
     import torch
     import torch.distributed as dist
@@ -199,11 +239,14 @@ def main():
 
     # ---- inputs (synthetic, seeded): alm ~ (l+1)^-2 power law; the map inputs of the
     # analysis-type calls are the synthesised map (+ sigma = 0.01 pixel noise for cfg4), resident in HBM.
-    t_setup = time.perf_counter()
+    t_inputs = time.perf_counter()
     alm_np = synth.powerlaw_alm(replicas.rank_seed(cfg["seed"], rank), lmax, mmax, batch)
     h_alm = torch.from_numpy(alm_np).to(cdt).pin_memory()
-    T = B.Transform(nside, lmax, mmax, batch, rdt, dev)
-    stats = B.cuhpx_workspace_stats(T.workspace)
+    t_inputs = time.perf_counter() - t_inputs
+    torch.zeros(1, device=dev)
+    torch.cuda.synchronize()  # context is up: what follows is the library's own first call
+    T = B.Transform(nside, lmax, mmax, batch, rdt, dev)  # T.init_seconds: cuhpx_workspace_init alone
+    stats = B.cuhpx_plan_stats(T.params)
     d_alm = h_alm.to(dev, non_blocking=True)
     d_map = T.alm2map(d_alm)
     if args.workload == "cfg4":
@@ -216,36 +259,36 @@ def main():
     h_alm_out = torch.empty_like(h_alm).pin_memory()
     h_map_out = torch.empty_like(h_map).pin_memory()
     torch.cuda.synchronize()
-    t_setup = time.perf_counter() - t_setup
 
     ws = T.workspace
+    P = T.params
     stages = ["fft_analysis", "legendre_analysis", "legendre_synthesis", "fft_synthesis"]
 
-    def step(ev=None):
-        """One pass of the hot path through the stage-level C-ABI calls (the public calls are exactly these pairs);
-        ev: list to append (name, start_event, end_event) per kernel group."""
+    def step():
+        """One pass of the hot path: the four public C-ABI calls on resident buffers."""
+        B.cuhpx_map2alm(*P, d_map, d_alm_out, None, ws)
+        B.cuhpx_alm2map(*P, d_alm, d_map_out, ws)
+        B.cuhpx_alm2map_adjoint(*P, d_map, d_alm_out, ws)
+        B.cuhpx_map2alm_adjoint(*P, d_alm, d_map_out, None, ws)
+
+    def staged_step(ev):
+        """The same work through the stage-level entry points (the public calls are exactly these pairs), one
+        CUDA-event pair per stage: the instrumented pass behind `roofline`, NOT the timed region of `value`."""
         def timed(name, fn):
-            if ev is None:
-                fn()
-                return
             a = torch.cuda.Event(enable_timing=True)
             b = torch.cuda.Event(enable_timing=True)
             a.record()
             fn()
             b.record()
             ev.append((name, a, b))
-        # map2alm
-        timed("fft_analysis", lambda: B.cuhpx_analysis_fft_stage(d_map, None, 1, ws))
-        timed("legendre_analysis", lambda: B.cuhpx_analysis_legendre_stage(d_alm_out, 0, ws))
-        # alm2map
-        timed("legendre_synthesis", lambda: B.cuhpx_synthesis_legendre_stage(d_alm, 0, ws))
-        timed("fft_synthesis", lambda: B.cuhpx_synthesis_fft_stage(d_map_out, None, 0, ws))
-        # alm2map_adjoint
-        timed("fft_analysis", lambda: B.cuhpx_analysis_fft_stage(d_map, None, 0, ws))
-        timed("legendre_analysis", lambda: B.cuhpx_analysis_legendre_stage(d_alm_out, 1, ws))
-        # map2alm_adjoint
-        timed("legendre_synthesis", lambda: B.cuhpx_synthesis_legendre_stage(d_alm, 1, ws))
-        timed("fft_synthesis", lambda: B.cuhpx_synthesis_fft_stage(d_map_out, None, 1, ws))
+        timed("fft_analysis", lambda: B.cuhpx_analysis_fft_stage(P, d_map, None, 1, ws))
+        timed("legendre_analysis", lambda: B.cuhpx_analysis_legendre_stage(P, d_alm_out, 0, ws))
+        timed("legendre_synthesis", lambda: B.cuhpx_synthesis_legendre_stage(P, d_alm, 0, ws))
+        timed("fft_synthesis", lambda: B.cuhpx_synthesis_fft_stage(P, d_map_out, None, 0, ws))
+        timed("fft_analysis", lambda: B.cuhpx_analysis_fft_stage(P, d_map, None, 0, ws))
+        timed("legendre_analysis", lambda: B.cuhpx_analysis_legendre_stage(P, d_alm_out, 1, ws))
+        timed("legendre_synthesis", lambda: B.cuhpx_synthesis_legendre_stage(P, d_alm, 1, ws))
+        timed("fft_synthesis", lambda: B.cuhpx_synthesis_fft_stage(P, d_map_out, None, 1, ws))
 
     def barrier():
         if world > 1:
@@ -258,14 +301,18 @@ def main():
     for _ in range(max(args.warmup, 3)):
         step()
     barrier()
-    ev = []
     e0 = torch.cuda.Event(enable_timing=True)
     e1 = torch.cuda.Event(enable_timing=True)
     barrier()
     e0.record()
     for _ in range(args.steps):
-        step(ev)
+        step()
     e1.record()
+    barrier()
+    # per-stage times: a separate instrumented pass of the same length
+    ev = []
+    for _ in range(args.steps):
+        staged_step(ev)
     barrier()
     # a timed region shorter than the sampler's 100 ms period (cfg1-3) yields no sample: keep the same load running,
     # untimed, until nvidia-smi has reported a few
@@ -347,10 +394,13 @@ def main():
     h2d = 2 * map_bytes + 2 * alm_bytes
     d2h = 2 * map_bytes + 2 * alm_bytes
 
-    # ---- roofline of the dominant kernel + the other stages
+    # ---- roofline of the dominant kernel + the other stages.  Legendre stages: flops of the
+    # terms the kernels EXECUTE (insignificant (m, ring) pairs are skipped, R7) over the nominal FMA peak;
+    # the SURVEY 8(d) all-terms figure T (4 + 4B) and the fraction of the FMA rate probed in this run are beside it.
     hbm_gbs, peak_src = load_peaks()
-    terms_full = stats["legendre_terms_full"]  # T = nalm * 2 nside
-    leg_flops = terms_full * (4 + 4 * batch)   # T (4 + 4B), all T terms counted
+    terms_full, terms_exec = stats["legendre_terms_full"], stats["legendre_terms_executed"]
+    leg_flops_exec = terms_exec * (4 + 4 * batch)
+    leg_flops_full = terms_full * (4 + 4 * batch)   # T (4 + 4B), T = nalm * 2 nside
     fft_bytes = batch * npix * rbytes + batch * stats["spectra_entries"] * 2 * rbytes  # map once + spectra once
     fma_ms, fma_cnt = B.cuhpx_fma_peak_probe(B.CUHPX_F64 if dt == "f64" else B.CUHPX_F32, 20000)
     fma_tflops = 2 * fma_cnt / (fma_ms * 1e-3) / 1e12
@@ -364,9 +414,12 @@ def main():
     per_stage = {}
     for s in stages:
         if s.startswith("legendre"):
-            ach = leg_flops / (stage_avg[s] * 1e-3) / 1e12
+            ach = leg_flops_exec / (stage_avg[s] * 1e-3) / 1e12
+            full = leg_flops_full / (stage_avg[s] * 1e-3) / 1e12
             per_stage[s] = {"bound": "alu", "achieved": ach, "peak": PEAK_TFLOPS[dt], "unit": "TFLOP/s",
-                            "frac": ach / PEAK_TFLOPS[dt], "ms": stage_avg[s], "traffic": traffic.get(s)}
+                            "frac": ach / PEAK_TFLOPS[dt], "ms": stage_avg[s], "traffic": traffic.get(s),
+                            "flops_counted": "executed terms x (4 + 4 B)", "frac_of_fma_probe": ach / fma_tflops,
+                            "algorithmic_all_terms": {"achieved": full, "frac": full / PEAK_TFLOPS[dt]}}
         else:
             ach = fft_bytes / (stage_avg[s] * 1e-3) / 1e9
             per_stage[s] = {"bound": "hbm", "achieved": ach, "peak": hbm_gbs, "unit": "GB/s", "frac": ach / hbm_gbs,
@@ -375,7 +428,9 @@ def main():
     roofline = dict(per_stage[dominant])
     roofline.update(kernel=dominant, peak_source=("B200 nominal: 148 SM x 64/128 FMA lanes x 2 x 1.965 GHz"
                                                   if roofline["bound"] == "alu" else f"MEASURED_PEAKS.json ({peak_src})"),
-                    fma_probe_tflops=fma_tflops, terms_executed_frac=stats["legendre_terms_executed"] / terms_full,
+                    fma_probe_tflops=fma_tflops, terms_executed_frac=terms_exec / terms_full,
+                    timing="per-stage CUDA events of an instrumented pass over the stage-level calls, "
+                           f"{args.steps} steps, separate from the timed region of `value`",
                     stages=per_stage)
 
     launches_per_step = int(4 * stats["fft_stage_launches"] + 2 * stats["legendre_analysis_launches"]
@@ -416,11 +471,12 @@ def main():
             "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
             "warmup": max(args.warmup, 3), "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "weak",
             "vs_baseline": None, "dtype": dt, "data": "synthetic",
-            "config": {"workload": workload_name(cfg), "step": "map2alm + alm2map + alm2map_adjoint + map2alm_adjoint",
+            "config": {"workload": workload_name(cfg), "step": "cuhpx_map2alm + cuhpx_alm2map + cuhpx_alm2map_adjoint + "
+                       "cuhpx_map2alm_adjoint (the four public C-ABI calls)",
                        "transforms_per_step": transforms_per_step, "pixels_per_s": value * npix,
                        "l2_policy": f"inputs larger than L2 ({(map_bytes + alm_bytes) / 1e6:.0f} MB per call vs 126 MB)"
                        if map_bytes + alm_bytes > 126e6 else "inputs fit in L2 (latency-bound configuration)",
-                       "replicas": world, "setup_s": t_setup},
+                       "replicas": world, "tables_first_call_s": T.init_seconds, "input_synthesis_s": t_inputs},
             "clocks": clocks,
             "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
                     "ms_per_step": ms_e2e / k_e2e, "steps": k_e2e},

@@ -25,16 +25,27 @@
  * Conventions
  *   - Every data pointer is a DEVICE pointer owned by the caller, 16-byte aligned.  The library allocates no
  *     device memory: scratch and constant tables live in the caller's workspace (cuhpx_workspace_bytes).
- *   - Inputs are const, outputs are fully overwritten (never accumulated); in/out must not alias.
+ *   - The library keeps no per-workspace state and no call has to be paired with a free: a workspace is plain
+ *     device memory whose first 256 bytes are a header (magic, parameter key) written by cuhpx_workspace_init.  It
+ *     may be copied or moved (tables are addressed relative to the pointer passed to each call) and is simply
+ *     freed by its owner.  What the host needs per call (ring classes, cut-offs, launch shapes, table offsets) is a
+ *     pure function of (nside, lmax, mmax, batch, dtype), memoised inside the library.  Every kernel checks the
+ *     header first: a call on memory that was not initialised for the same five parameters does nothing except
+ *     marking the header (cuhpx_workspace_check reports it); it never follows a pointer from a foreign table.
+ *   - Inputs are const, outputs are fully overwritten (never accumulated); input, output and workspace ranges must
+ *     not overlap (checked on the host, CUHPX_EINVAL).
  *   - All work is enqueued on `stream`; the transform calls never synchronise with the host and can be captured
- *     in a CUDA graph.  cuhpx_workspace_init enqueues table-building kernels and small host->device copies on
- *     `stream` (it may block the host while it computes the tables); later calls on the same stream are ordered
- *     after it.  A workspace serves one transform at a time (calls sharing one workspace must be stream-ordered).
+ *     in a CUDA graph (tests/test_gpu_parity.py::test_cuda_graph_capture_replay).  Part of the FFT stage runs on a
+ *     library stream forked from and joined to `stream` with events (created once per device, never per
+ *     workspace).  cuhpx_workspace_init enqueues table-building kernels and host->device copies on `stream` and
+ *     returns after they have completed.  A workspace serves one transform at a time (calls sharing one workspace
+ *     must be stream-ordered).
  *   - ring_weights: DEVICE pointer to 4 nside - 1 doubles (always fp64), rings north to south, the full
  *     quadrature weight w_y of Eq. 26 (i.e. including the 4 pi / Npix factor); NULL = equal weights
  *     4 pi / Npix (Eq. 1).
  *   - Return value: a cuhpx_status_t.  Argument errors are detected on the host before any launch.  Nothing is
  *     thrown across the ABI.  After CUHPX_ECUDA, cudaGetLastError() describes the launch failure.
+ *   - batch <= 65535 (channels index a grid dimension).
  *   - There is no CPU fallback: on a machine without a CUDA device every compute call returns CUHPX_ECUDA.
  */
 #ifndef CUHPX_H_
@@ -72,12 +83,15 @@ int cuhpx_ring_info(int nside, int ring, long long* n_pix, long long* first_pix,
 /* ---- workspace */
 /* Bytes of device workspace needed for (nside, lmax, mmax, batch, dtype); 0 on invalid arguments. */
 size_t cuhpx_workspace_bytes(int nside, int lmax, int mmax, int batch, cuhpx_dtype_t dtype);
-/* Build the constant tables (ring geometry, recurrence seeds, twiddles, chirp filters) inside d_workspace.
- * Must be called once before the transforms, and again if any of the five parameters changes. */
+/* Build the constant tables (ring geometry, recurrence seeds and coefficients, twiddles, chirp filters) and the
+ * header inside d_workspace.  Once per workspace; again if any of the five parameters changes.  Returns after the
+ * tables are complete (it synchronises `stream`); config.tables_first_call_s in bench.py is the time of this call. */
 int cuhpx_workspace_init(int nside, int lmax, int mmax, int batch, cuhpx_dtype_t dtype, void* d_workspace,
                          size_t workspace_bytes, cuhpx_stream_t stream);
-/* Forget a workspace (host bookkeeping only; the memory stays the caller's). */
-int cuhpx_workspace_release(void* d_workspace);
+/* Optional, SYNCHRONISING: read the header back and report whether d_workspace is initialised for these parameters
+ * and no kernel has refused it since (CUHPX_OK / CUHPX_EWORKSPACE). */
+int cuhpx_workspace_check(int nside, int lmax, int mmax, int batch, cuhpx_dtype_t dtype, const void* d_workspace,
+                          size_t workspace_bytes, cuhpx_stream_t stream);
 
 /* ---- the four operators */
 int cuhpx_map2alm(int nside, int lmax, int mmax, int batch, cuhpx_dtype_t dtype, const void* d_map, void* d_alm,
@@ -121,33 +135,39 @@ int cuhpx_alm_resize(int lmax_in, int mmax_in, int lmax_out, int mmax_out, int b
                      const void* d_alm_in, void* d_alm_out, cuhpx_stream_t stream);
 
 /* ---- the two stages of each direction, individually, for per-stage
- * measurement and stage-level parity tests.  The ring spectra live inside the workspace:
+ * measurement and stage-level parity tests; same conventions and checks as the operators.  The ring spectra live
+ * inside the workspace at byte offset cuhpx_spectra_offset(...):
  *   spectra[b][ring][m], m = 0..m_cut(ring) (entries above m_cut(ring) are neither written nor read: there
  *   lambda_lm(theta_ring) is below 2^-110 for every l <= lmax), row stride cuhpx_spectra_stride() complex values.
  * analysis:  F_m(ring) = w_ring sum_x p_x exp(-i m (phi0 + 2 pi x / N))   (Eq. 13, phase and alias rule of Eq. 26)
  * synthesis: p_x = Re G_0 + 2 sum_{m>=1} Re(G_m exp(+i m (phi0 + 2 pi x / N))), times w_ring if weights are given. */
 size_t cuhpx_spectra_stride(int mmax);
-/* device pointer to the spectra buffer inside an initialised workspace (NULL if unknown workspace) */
-void* cuhpx_workspace_spectra(void* d_workspace);
-/* m_cut of every ring (host array of 4 nside - 1 ints), from an initialised workspace */
-int cuhpx_workspace_mcut(void* d_workspace, int* h_mcut);
-int cuhpx_analysis_fft_stage(const void* d_map, const double* d_ring_weights, int use_weights, void* d_workspace,
+/* byte offset of the spectra buffer inside a workspace for these parameters (0 on invalid arguments) */
+size_t cuhpx_spectra_offset(int nside, int lmax, int mmax, int batch, cuhpx_dtype_t dtype);
+/* m_cut of every ring (host array of 4 nside - 1 ints); host only */
+int cuhpx_plan_mcut(int nside, int lmax, int mmax, int batch, cuhpx_dtype_t dtype, int* h_mcut);
+int cuhpx_analysis_fft_stage(int nside, int lmax, int mmax, int batch, cuhpx_dtype_t dtype, const void* d_map,
+                             const double* d_ring_weights, int use_weights, void* d_workspace, size_t workspace_bytes,
                              cuhpx_stream_t stream);
 /* adjoint != 0 multiplies by c_m (S^T) */
-int cuhpx_analysis_legendre_stage(void* d_alm, int adjoint, void* d_workspace, cuhpx_stream_t stream);
+int cuhpx_analysis_legendre_stage(int nside, int lmax, int mmax, int batch, cuhpx_dtype_t dtype, void* d_alm, int adjoint,
+                                  void* d_workspace, size_t workspace_bytes, cuhpx_stream_t stream);
 /* adjoint != 0 divides the input by c_m (A^T) */
-int cuhpx_synthesis_legendre_stage(const void* d_alm, int adjoint, void* d_workspace, cuhpx_stream_t stream);
-int cuhpx_synthesis_fft_stage(void* d_map, const double* d_ring_weights, int use_weights, void* d_workspace,
+int cuhpx_synthesis_legendre_stage(int nside, int lmax, int mmax, int batch, cuhpx_dtype_t dtype, const void* d_alm,
+                                   int adjoint, void* d_workspace, size_t workspace_bytes, cuhpx_stream_t stream);
+int cuhpx_synthesis_fft_stage(int nside, int lmax, int mmax, int batch, cuhpx_dtype_t dtype, void* d_map,
+                              const double* d_ring_weights, int use_weights, void* d_workspace, size_t workspace_bytes,
                               cuhpx_stream_t stream);
 
-/* Host-side statistics of an initialised workspace, for measurement (doubles, `count` of them are written, at most 8):
+/* Host-side statistics of the plan for these parameters, for measurement (doubles, `count` of them are written, at most 8):
  *  [0] kernel launches of one FFT-stage call   [1] of one Legendre analysis call   [2] of one Legendre synthesis call
  *  [3] Legendre terms executed per channel = sum_m (lmax - m + 1) * (ring pairs processed at order m)
  *  [4] Legendre terms of the full triangle = nalm * 2 nside          [5] spectra entries per channel = sum_rings (m_cut + 1)
  *  [6] bytes of constant tables read by one FFT-stage call (chirp filters + twiddles)   [7] workspace bytes */
-int cuhpx_workspace_stats(void* d_workspace, double* h_stats, int count);
+int cuhpx_plan_stats(int nside, int lmax, int mmax, int batch, cuhpx_dtype_t dtype, double* h_stats, int count);
 
-/* Register-only FMA loop used by bench.py to measure the FP64 / FP32 FMA peak in the same run.
+/* MEASUREMENT HOOK, not part of the transform API: register-only FMA loop used by bench.py to measure the FP64 /
+ * FP32 FMA peak of the device in the same run as the transforms (SURVEY 8(d) asks for exactly that).
  * Writes the elapsed milliseconds of `iters` dependent-chain FMAs per thread over the whole GPU to *ms and the
  * number of FMA instructions executed to *fma_count.  Synchronises the stream. */
 int cuhpx_fma_peak_probe(cuhpx_dtype_t dtype, int iters, float* ms, double* fma_count, cuhpx_stream_t stream);

@@ -19,12 +19,22 @@ _SRC = os.path.join(_HERE, "sht_oracle.c")
 _LIB = os.path.join(_HERE, "libsht_oracle.so")
 
 
-def build(force: bool = False) -> str:
-    """Compile the oracle with gcc (idempotent). Building the checker is not using it."""
-    if force or not os.path.exists(_LIB) or os.path.getmtime(_LIB) < os.path.getmtime(_SRC):
-        cmd = ["gcc", "-O2", "-std=c11", "-fopenmp", "-shared", "-fPIC", "-o", _LIB, _SRC, "-lm"]
+_LIB_SAN = os.path.join(_HERE, "libsht_oracle_san.so")
+
+
+def build(force: bool = False, sanitize: bool = False) -> str:
+    """Compile the oracle with gcc (idempotent). Building the checker is not using it.
+
+    sanitize=True builds a second library with -fsanitize=address,undefined; it is loaded instead
+    of the plain one when the environment variable SHT_ORACLE_LIB names it, in a process started with libasan
+    preloaded (tests/test_oracle_pins.py::test_oracle_under_asan_ubsan does that in a subprocess)."""
+    lib = _LIB_SAN if sanitize else _LIB
+    if force or not os.path.exists(lib) or os.path.getmtime(lib) < os.path.getmtime(_SRC):
+        flags = ["-O1", "-g", "-fsanitize=address,undefined", "-fno-sanitize-recover=undefined", "-fno-omit-frame-pointer"] \
+            if sanitize else ["-O2"]
+        cmd = ["gcc"] + flags + ["-std=c11", "-fopenmp", "-shared", "-fPIC", "-o", lib, _SRC, "-lm"]
         subprocess.run(cmd, check=True)
-    return _LIB
+    return lib
 
 
 _lib = None
@@ -33,8 +43,10 @@ _lib = None
 def _load():
     global _lib
     if _lib is None:
-        build()
-        _lib = ctypes.CDLL(_LIB)
+        path = os.environ.get("SHT_ORACLE_LIB")
+        if not path:
+            path = build()
+        _lib = ctypes.CDLL(path)
         i32, i64 = ctypes.c_int, ctypes.c_int64
         vp = ctypes.c_void_p
         _lib.oracle_alm_count.restype = i64

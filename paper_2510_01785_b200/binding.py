@@ -20,10 +20,10 @@ CUHPX_OK, CUHPX_EINVAL, CUHPX_EWORKSPACE, CUHPX_EUNSUPPORTED, CUHPX_ECUDA = 0, 1
 #: every symbol include/cuhpx.h declares
 EXPORTS = [
     "cuhpx_npix", "cuhpx_nrings", "cuhpx_alm_count", "cuhpx_alm_index", "cuhpx_status_string", "cuhpx_ring_info",
-    "cuhpx_workspace_bytes", "cuhpx_workspace_init", "cuhpx_workspace_release", "cuhpx_map2alm", "cuhpx_alm2map",
-    "cuhpx_alm2map_adjoint", "cuhpx_map2alm_adjoint", "cuhpx_spectra_stride", "cuhpx_workspace_spectra",
-    "cuhpx_workspace_mcut", "cuhpx_analysis_fft_stage", "cuhpx_analysis_legendre_stage",
-    "cuhpx_synthesis_legendre_stage", "cuhpx_synthesis_fft_stage", "cuhpx_fma_peak_probe", "cuhpx_workspace_stats",
+    "cuhpx_workspace_bytes", "cuhpx_workspace_init", "cuhpx_workspace_check", "cuhpx_map2alm", "cuhpx_alm2map",
+    "cuhpx_alm2map_adjoint", "cuhpx_map2alm_adjoint", "cuhpx_spectra_stride", "cuhpx_spectra_offset",
+    "cuhpx_plan_mcut", "cuhpx_analysis_fft_stage", "cuhpx_analysis_legendre_stage",
+    "cuhpx_synthesis_legendre_stage", "cuhpx_synthesis_fft_stage", "cuhpx_fma_peak_probe", "cuhpx_plan_stats",
     "cuhpx_map2alm_iter", "cuhpx_reorder", "cuhpx_nest2ring_index", "cuhpx_alm_resize",
 ]
 CUHPX_NEST2RING, CUHPX_RING2NEST = 0, 1
@@ -56,7 +56,7 @@ def _load() -> ctypes.CDLL:
     lib.cuhpx_workspace_bytes.restype = sz
     lib.cuhpx_workspace_bytes.argtypes = [i, i, i, i, i]
     lib.cuhpx_workspace_init.argtypes = [i, i, i, i, i, vp, sz, vp]
-    lib.cuhpx_workspace_release.argtypes = [vp]
+    lib.cuhpx_workspace_check.argtypes = [i, i, i, i, i, vp, sz, vp]
     lib.cuhpx_map2alm.argtypes = [i, i, i, i, i, vp, vp, vp, vp, sz, vp]
     lib.cuhpx_alm2map.argtypes = [i, i, i, i, i, vp, vp, vp, sz, vp]
     lib.cuhpx_alm2map_adjoint.argtypes = [i, i, i, i, i, vp, vp, vp, sz, vp]
@@ -68,15 +68,15 @@ def _load() -> ctypes.CDLL:
     lib.cuhpx_nest2ring_index.argtypes = [i, ctypes.c_longlong]
     lib.cuhpx_spectra_stride.restype = sz
     lib.cuhpx_spectra_stride.argtypes = [i]
-    lib.cuhpx_workspace_spectra.restype = vp
-    lib.cuhpx_workspace_spectra.argtypes = [vp]
-    lib.cuhpx_workspace_mcut.argtypes = [vp, vp]
-    lib.cuhpx_analysis_fft_stage.argtypes = [vp, vp, i, vp, vp]
-    lib.cuhpx_analysis_legendre_stage.argtypes = [vp, i, vp, vp]
-    lib.cuhpx_synthesis_legendre_stage.argtypes = [vp, i, vp, vp]
-    lib.cuhpx_synthesis_fft_stage.argtypes = [vp, vp, i, vp, vp]
+    lib.cuhpx_spectra_offset.restype = sz
+    lib.cuhpx_spectra_offset.argtypes = [i, i, i, i, i]
+    lib.cuhpx_plan_mcut.argtypes = [i, i, i, i, i, vp]
+    lib.cuhpx_analysis_fft_stage.argtypes = [i, i, i, i, i, vp, vp, i, vp, sz, vp]
+    lib.cuhpx_analysis_legendre_stage.argtypes = [i, i, i, i, i, vp, i, vp, sz, vp]
+    lib.cuhpx_synthesis_legendre_stage.argtypes = [i, i, i, i, i, vp, i, vp, sz, vp]
+    lib.cuhpx_synthesis_fft_stage.argtypes = [i, i, i, i, i, vp, vp, i, vp, sz, vp]
     lib.cuhpx_fma_peak_probe.argtypes = [i, i, vp, vp, vp]
-    lib.cuhpx_workspace_stats.argtypes = [vp, vp, i]
+    lib.cuhpx_plan_stats.argtypes = [i, i, i, i, i, vp, i]
     return lib
 
 
@@ -156,8 +156,11 @@ def cuhpx_workspace_init(nside, lmax, mmax, batch, dtype, workspace: torch.Tenso
            "cuhpx_workspace_init")
 
 
-def cuhpx_workspace_release(workspace: torch.Tensor) -> None:
-    _lib.cuhpx_workspace_release(workspace.data_ptr())
+def cuhpx_workspace_check(nside, lmax, mmax, batch, dtype, workspace: torch.Tensor, stream=None) -> None:
+    """Synchronising: raises CuhpxError(CUHPX_EWORKSPACE) unless `workspace` is initialised for these parameters."""
+    _check(_lib.cuhpx_workspace_check(nside, lmax, mmax, batch, dtype, _dev_ptr(workspace),
+                                      workspace.numel() * workspace.element_size(), _stream_ptr(stream)),
+           "cuhpx_workspace_check")
 
 
 def _ws_args(ws: torch.Tensor):
@@ -232,39 +235,47 @@ def ring2nest(hmap: torch.Tensor, nside: int) -> torch.Tensor:
     return out
 
 
-def cuhpx_analysis_fft_stage(d_map, d_ring_weights, use_weights, workspace, stream=None) -> None:
-    _check(_lib.cuhpx_analysis_fft_stage(_dev_ptr(d_map), _dev_ptr(d_ring_weights), int(use_weights),
-                                         _dev_ptr(workspace), _stream_ptr(stream)), "cuhpx_analysis_fft_stage")
+def cuhpx_analysis_fft_stage(params, d_map, d_ring_weights, use_weights, workspace, stream=None) -> None:
+    """params = (nside, lmax, mmax, batch, dtype code), e.g. Transform.params"""
+    p, n = _ws_args(workspace)
+    _check(_lib.cuhpx_analysis_fft_stage(*params, _dev_ptr(d_map), _dev_ptr(d_ring_weights), int(use_weights), p, n,
+                                         _stream_ptr(stream)), "cuhpx_analysis_fft_stage")
 
 
-def cuhpx_analysis_legendre_stage(d_alm, adjoint, workspace, stream=None) -> None:
-    _check(_lib.cuhpx_analysis_legendre_stage(_dev_ptr(d_alm), int(adjoint), _dev_ptr(workspace),
-                                              _stream_ptr(stream)), "cuhpx_analysis_legendre_stage")
+def cuhpx_analysis_legendre_stage(params, d_alm, adjoint, workspace, stream=None) -> None:
+    p, n = _ws_args(workspace)
+    _check(_lib.cuhpx_analysis_legendre_stage(*params, _dev_ptr(d_alm), int(adjoint), p, n, _stream_ptr(stream)),
+           "cuhpx_analysis_legendre_stage")
 
 
-def cuhpx_synthesis_legendre_stage(d_alm, adjoint, workspace, stream=None) -> None:
-    _check(_lib.cuhpx_synthesis_legendre_stage(_dev_ptr(d_alm), int(adjoint), _dev_ptr(workspace),
-                                               _stream_ptr(stream)), "cuhpx_synthesis_legendre_stage")
+def cuhpx_synthesis_legendre_stage(params, d_alm, adjoint, workspace, stream=None) -> None:
+    p, n = _ws_args(workspace)
+    _check(_lib.cuhpx_synthesis_legendre_stage(*params, _dev_ptr(d_alm), int(adjoint), p, n, _stream_ptr(stream)),
+           "cuhpx_synthesis_legendre_stage")
 
 
-def cuhpx_synthesis_fft_stage(d_map, d_ring_weights, use_weights, workspace, stream=None) -> None:
-    _check(_lib.cuhpx_synthesis_fft_stage(_dev_ptr(d_map), _dev_ptr(d_ring_weights), int(use_weights),
-                                          _dev_ptr(workspace), _stream_ptr(stream)), "cuhpx_synthesis_fft_stage")
+def cuhpx_synthesis_fft_stage(params, d_map, d_ring_weights, use_weights, workspace, stream=None) -> None:
+    p, n = _ws_args(workspace)
+    _check(_lib.cuhpx_synthesis_fft_stage(*params, _dev_ptr(d_map), _dev_ptr(d_ring_weights), int(use_weights), p, n,
+                                          _stream_ptr(stream)), "cuhpx_synthesis_fft_stage")
 
 
-def cuhpx_workspace_mcut(workspace: torch.Tensor, nside: int):
+def cuhpx_spectra_offset(params) -> int:
+    return int(_lib.cuhpx_spectra_offset(*params))
+
+
+def cuhpx_plan_mcut(params):
     import numpy as np
 
-    out = np.zeros(4 * nside - 1, dtype=np.int32)
-    _check(_lib.cuhpx_workspace_mcut(_dev_ptr(workspace), out.ctypes.data_as(ctypes.c_void_p)),
-           "cuhpx_workspace_mcut")
+    out = np.zeros(4 * params[0] - 1, dtype=np.int32)
+    _check(_lib.cuhpx_plan_mcut(*params, out.ctypes.data_as(ctypes.c_void_p)), "cuhpx_plan_mcut")
     return out
 
 
-def cuhpx_workspace_stats(workspace: torch.Tensor) -> dict:
-    """Host-side statistics of an initialised workspace (see cuhpx.h)."""
+def cuhpx_plan_stats(params) -> dict:
+    """Host-side statistics of the plan for params (see cuhpx.h)."""
     arr = (ctypes.c_double * 8)()
-    _check(_lib.cuhpx_workspace_stats(_dev_ptr(workspace), arr, 8), "cuhpx_workspace_stats")
+    _check(_lib.cuhpx_plan_stats(*params, arr, 8), "cuhpx_plan_stats")
     keys = ["fft_stage_launches", "legendre_analysis_launches", "legendre_synthesis_launches", "legendre_terms_executed",
             "legendre_terms_full", "spectra_entries", "fft_table_bytes", "workspace_bytes"]
     return dict(zip(keys, [float(v) for v in arr]))
@@ -304,16 +315,30 @@ class Transform:
         if ring_weights is not None:
             self.ring_weights = ring_weights.to(device=self.device, dtype=torch.float64).contiguous()
         with torch.cuda.device(self.device):
-            cuhpx_workspace_init(nside, lmax, mmax, batch, self.code, self.workspace)
+            import time
 
-    def __del__(self):
-        try:
-            cuhpx_workspace_release(self.workspace)
-        except Exception:
-            pass
+            torch.cuda.synchronize()
+            t0 = time.perf_counter()
+            cuhpx_workspace_init(nside, lmax, mmax, batch, self.code, self.workspace)  # returns when the tables are built
+            #: seconds of cuhpx_workspace_init alone (host planning + table kernels; SURVEY 8(a) a0 "first-call time")
+            self.init_seconds = time.perf_counter() - t0
 
     def _args(self):
         return self.nside, self.lmax, self.mmax, self.batch, self.code
+
+    @property
+    def params(self):
+        """(nside, lmax, mmax, batch, dtype code): the scalar arguments every C-ABI call takes"""
+        return self._args()
+
+    def spectra_view(self) -> torch.Tensor:
+        """[batch, nrings, stride] complex view of the ring spectra inside the workspace (stage-level tests)."""
+        off = cuhpx_spectra_offset(self.params)
+        stride = cuhpx_spectra_stride(self.mmax)
+        nr = cuhpx_nrings(self.nside)
+        esz = 16 if self.code == CUHPX_F64 else 8
+        raw = self.workspace.view(torch.uint8)[off:off + self.batch * nr * stride * esz]
+        return raw.view(self.cdtype).view(self.batch, nr, stride)
 
     def map2alm(self, hmap: torch.Tensor, out: torch.Tensor | None = None) -> torch.Tensor:
         assert hmap.shape == (self.batch, self.npix) and hmap.dtype == self.rdtype

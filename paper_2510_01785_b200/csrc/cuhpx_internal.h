@@ -5,21 +5,50 @@
 #include <stddef.h>
 #include <stdint.h>
 
+#include <memory>
 #include <vector>
 
 #include "../../include/cuhpx.h"
 
 namespace cuhpx {
 
+// ------------------------------------------------------------------ workspace header (first 256 bytes of a workspace)
+// Written by cuhpx_workspace_init after every table is in place; every kernel of a transform call checks
+// (magic, key) before it touches a table and returns without side effects other than `bad = 1` if they do not
+// match.  The host keeps nothing per workspace: tables are addressed as workspace base + offset, and the offsets
+// are a pure function of (nside, lmax, mmax, batch, dtype, geometry).
+constexpr unsigned long long WS_MAGIC = 0x6375485058763032ULL;  // "cuHPXv02"
+struct WsHeader {
+    unsigned long long magic;
+    unsigned long long key;  // plan_key(nside, lmax, mmax, batch, dtype, geometry)
+    int nside, lmax, mmax, batch, dtype, geometry;
+    unsigned long long bytes;
+    int bad;  // set by a kernel that found a foreign header
+    int pad;
+};
+static_assert(sizeof(WsHeader) <= 256, "header slot");
+
+inline unsigned long long plan_key(int nside, int lmax, int mmax, int batch, int dtype, int geometry) {
+    unsigned long long h = 0x9E3779B97F4A7C15ULL;
+    const int v[6] = {nside, lmax, mmax, batch, dtype, geometry};
+    for (int i = 0; i < 6; ++i) {
+        h ^= (unsigned long long)(unsigned)v[i] + 0x9E3779B97F4A7C15ULL + (h << 6) + (h >> 2);
+        h *= 0xBF58476D1CE4E5B9ULL;
+    }
+    return h | 1ULL;
+}
+
 // ------------------------------------------------------------------ device-visible plan (POD, passed by value)
-// Ring pairs j = 0 .. npairs-1 (npairs = 2 nside): north ring index j (0-based ring number = j), its mirror
-// is ring nrings-1-j; the equator (j = npairs-1) is its own mirror and is treated as a pair with an empty
-// south member.  SURVEY 8(a) a0.
+// Ring pairs j = 0 .. npairs-1: north ring index j (0-based ring number = j), its mirror is ring nrings-1-j; when
+// nrings is odd the middle ring (j = npairs-1) is its own mirror and is treated as a pair with an empty south
+// member.  SURVEY 8(a) a0.  HEALPix: npairs = 2 nside, nrings = 4 nside - 1.
 struct DevPlan {
     int nside, lmax, mmax, batch;
     int nrings, npairs;
     int mstride;         // complex values per spectra row
     long long npix, nalm;
+    const WsHeader* hdr;     // workspace header (device) and the key this call expects to find there
+    unsigned long long key;
     // per ring pair [npairs]
     const double* y;         // 1 - cos(theta_j)  (formed without cancellation; R3)
     const double* ls_hi;     // log2(sin theta_j), split hi + lo
@@ -42,27 +71,41 @@ struct DevPlan {
     int chunk_pairs;         // ring pairs per chunk
 };
 
-// ------------------------------------------------------------------ host plan
-struct FftDev;  // FFT-stage device tables, defined in ring_fft.cu
-void free_fft_dev(FftDev*);
+// true if the workspace behind P was initialised for the parameters of this call (one 16-byte load per CTA)
+__device__ __forceinline__ bool ws_ok(const DevPlan& P) {
+#ifdef __CUDA_ARCH__
+    const ulonglong2 h = __ldg(reinterpret_cast<const ulonglong2*>(P.hdr));
+    if (h.x == WS_MAGIC && h.y == P.key) return true;
+    if (threadIdx.x == 0) const_cast<WsHeader*>(P.hdr)->bad = 1;
+    return false;
+#else
+    return true;
+#endif
+}
+
+// ------------------------------------------------------------------ host plan: a pure function of the call parameters
+struct FftHost;  // FFT-stage part (ring_fft.cu)
+void free_fft_host(FftHost*);
 
 struct HostPlan {
-    DevPlan d;
+    DevPlan d;  // pointer members hold OFFSETS from the workspace base until resolve() rebases them
     cuhpx_dtype_t dtype;
+    int geometry;
     size_t workspace_bytes;
+    // table offsets inside the workspace
+    size_t off_y, off_lshi, off_lslo, off_ringN, off_start, off_shifted, off_mcut, off_prefhi, off_preflo, off_jmin;
+    size_t off_fft, fft_bytes, off_alpha, off_scale, off_spectra, off_partial;
     std::vector<int> h_ringN, h_mcut, h_jmin, h_shifted;
     std::vector<long long> h_start;
-    // ring lists for the FFT stage, by method (0-based ring numbers over all nrings rings)
-    std::vector<int> rings_direct, rings_pow2, rings_blue;
-    int* d_rings_direct = nullptr;
-    int* d_rings_pow2 = nullptr;
-    int* d_rings_blue = nullptr;
-    FftDev* fft = nullptr;  // owned
-    ~HostPlan() { free_fft_dev(fft); }
+    std::vector<double> h_y, h_lshi, h_lslo, h_prefhi, h_preflo, h_weight;  // h_weight: built-in quadrature weights per ring
+    FftHost* fft = nullptr;  // owned
+    ~HostPlan() { free_fft_host(fft); }
     HostPlan() = default;
     HostPlan(const HostPlan&) = delete;
     HostPlan& operator=(const HostPlan&) = delete;
+    DevPlan resolve(void* ws) const;  // device plan for the workspace at `ws`
 };
+typedef std::shared_ptr<const HostPlan> PlanRef;
 
 inline int ilog2_ceil(long long v) {
     int k = 0;
@@ -73,16 +116,19 @@ inline bool is_pow2(long long v) { return v > 0 && (v & (v - 1)) == 0; }
 
 // ------------------------------------------------------------------ launchers (each returns a cudaError_t)
 cudaError_t launch_legendre_coeff(int lmax, int mmax, double* alpha, double* scale, cudaStream_t st);
-cudaError_t launch_legendre_analysis(const HostPlan& hp, void* d_alm, int adjoint, cudaStream_t st);
-cudaError_t launch_legendre_synthesis(const HostPlan& hp, const void* d_alm, int adjoint, cudaStream_t st);
-cudaError_t launch_fft_analysis(const HostPlan& hp, const void* d_map, const double* d_w, int use_w, cudaStream_t st);
-cudaError_t launch_fft_synthesis(const HostPlan& hp, void* d_map, const double* d_w, int use_w, cudaStream_t st);
+cudaError_t launch_legendre_analysis(const HostPlan& hp, const DevPlan& P, void* d_alm, int adjoint, cudaStream_t st);
+cudaError_t launch_legendre_synthesis(const HostPlan& hp, const DevPlan& P, const void* d_alm, int adjoint, cudaStream_t st);
+cudaError_t launch_fft_analysis(const HostPlan& hp, const DevPlan& P, const void* d_map, const double* d_w, int use_w,
+                                cudaStream_t st);
+cudaError_t launch_fft_synthesis(const HostPlan& hp, const DevPlan& P, void* d_map, const double* d_w, int use_w,
+                                 cudaStream_t st);
 
-// FFT-stage planning: classify rings, size and build tables.  `base` is the device address where the tables may
-// be placed; returns the number of bytes used (when base == nullptr only sizes are computed).
-size_t plan_fft_tables(HostPlan& hp, char* base, bool build, cudaStream_t st, cudaError_t* err);
-// largest supported ring for this dtype (shared-memory bound); used by argument validation
-bool fft_supported(int nside, cuhpx_dtype_t dt);
+// FFT-stage planning (host only): classify the rings, lay the tables out; returns the bytes they take
+size_t fft_plan_host(HostPlan& hp);
+// build the FFT tables inside the workspace (base = workspace + hp.off_fft)
+cudaError_t fft_build_tables(const HostPlan& hp, char* base, cudaStream_t st);
+// largest supported ring for this dtype (register / shared-memory bound); used by argument validation
+bool fft_supported(int max_ring_pixels, cuhpx_dtype_t dt);
 
 // launches per FFT-stage call and bytes of constant tables it reads
 void fft_stage_stats(const HostPlan& hp, int* launches, double* table_bytes);

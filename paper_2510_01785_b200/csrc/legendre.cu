@@ -221,6 +221,7 @@ __global__ void __launch_bounds__(NT, 384 / NT) legendre_analysis_kernel(LegArgs
     static_assert(CHECK_EVERY % LT == 0 && CT % GL == 0 && GL % CHECK_EVERY == 0, "tile sizes");
     static_assert(NV >= 4, "reduction tile");
     const DevPlan& P = a.p;
+    if (!ws_ok(P)) return;
     const int m = blockIdx.x;
     const int ch0 = blockIdx.z * BT;
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
@@ -437,6 +438,7 @@ constexpr int GNC = 2 * GNCH;
 
 __global__ void __launch_bounds__(GK, 3) legendre_analysis_gemm_kernel(LegArgs a) {
     const DevPlan& P = a.p;
+    if (!ws_ok(P)) return;
     const int m = blockIdx.x;
     const int chunk = blockIdx.y;
     const int ch0 = blockIdx.z * GNCH;
@@ -597,6 +599,7 @@ __device__ __forceinline__ int hswz(int x, int ln) { return (x + (ln & 3) + 4 * 
 
 __global__ void __launch_bounds__(GK, 2) legendre_analysis_gemm64_kernel(LegArgs a) {
     const DevPlan& P = a.p;
+    if (!ws_ok(P)) return;
     const int m = blockIdx.x;
     const int ch0 = blockIdx.z * GNCH;
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
@@ -791,6 +794,7 @@ __global__ void __launch_bounds__(GK, 2) legendre_analysis_gemm64_kernel(LegArgs
 // sum the per-chunk partial results: alm[b][idx] = sum_c partial[c][b][idx], c < nchunks(m)
 template <typename T>
 __global__ void combine_partials_kernel(DevPlan P, const T* __restrict__ partial, T* __restrict__ alm) {
+    if (!ws_ok(P)) return;
     const int m = blockIdx.x;
     const int b = blockIdx.y;
     const int nch = (P.npairs - P.jmin[m] + P.chunk_pairs - 1) / P.chunk_pairs;
@@ -809,6 +813,7 @@ template <typename T, int BT, int R, int NT>
 __global__ void __launch_bounds__(NT) legendre_synthesis_kernel(LegArgs a) {
     using T2 = typename Vec2<T>::type;
     const DevPlan& P = a.p;
+    if (!ws_ok(P)) return;
     // grid: x = ring chunk (fastest), y = m: the chunk-CTAs of one order run together and share its a_lm / alpha / s_l
     // rows through L2 instead of each fetching them from DRAM
     const int m = blockIdx.y;
@@ -981,6 +986,7 @@ template <int BT, int R, int NT, int MINB>
 __global__ void __launch_bounds__(NT, MINB) legendre_synthesis_f32x2_kernel(LegArgs a) {
     using T = float;
     const DevPlan& P = a.p;
+    if (!ws_ok(P)) return;
     // grid: x = ring chunk (fastest), y = m: the chunk-CTAs of one order run together and share its a_lm / alpha / s_l
     // rows through L2 instead of each fetching them from DRAM
     const int m = blockIdx.y;
@@ -1163,9 +1169,8 @@ int legendre_chunk_pairs(cuhpx_dtype_t dt, int batch, int lmax, int npairs) {
 }
 
 template <typename T, int BT>
-static cudaError_t run_analysis(const HostPlan& hp, void* d_alm, int adjoint, cudaStream_t st) {
+static cudaError_t run_analysis(const HostPlan& hp, const DevPlan& P, void* d_alm, int adjoint, cudaStream_t st) {
     using C = LegCfg<T, BT>;
-    const DevPlan& P = hp.d;
     LegArgs a;
     a.p = P;
     a.in = nullptr;
@@ -1186,9 +1191,8 @@ static cudaError_t run_analysis(const HostPlan& hp, void* d_alm, int adjoint, cu
 }
 
 template <typename T, int BT>
-static cudaError_t run_synthesis(const HostPlan& hp, const void* d_alm, int adjoint, cudaStream_t st) {
+static cudaError_t run_synthesis(const HostPlan& hp, const DevPlan& P, const void* d_alm, int adjoint, cudaStream_t st) {
     using C = LegCfg<T, BT>;
-    const DevPlan& P = hp.d;
     LegArgs a;
     a.p = P;
     a.in = d_alm;
@@ -1202,8 +1206,7 @@ static cudaError_t run_synthesis(const HostPlan& hp, const void* d_alm, int adjo
 }
 
 template <typename T, int BT, int R, int LT, int NT, int GL, bool SEQ = false>
-static cudaError_t run_analysis_cfg(const HostPlan& hp, void* d_alm, int adjoint, cudaStream_t st) {
-    const DevPlan& P = hp.d;
+static cudaError_t run_analysis_cfg(const HostPlan& hp, const DevPlan& P, void* d_alm, int adjoint, cudaStream_t st) {
     LegArgs a;
     a.p = P;
     a.in = nullptr;
@@ -1223,8 +1226,7 @@ static cudaError_t run_analysis_cfg(const HostPlan& hp, void* d_alm, int adjoint
 }
 
 template <typename T, int BT, int RS, int NTS>
-static cudaError_t run_synthesis_cfg(const HostPlan& hp, const void* d_alm, int adjoint, cudaStream_t st) {
-    const DevPlan& P = hp.d;
+static cudaError_t run_synthesis_cfg(const HostPlan& hp, const DevPlan& P, const void* d_alm, int adjoint, cudaStream_t st) {
     LegArgs a;
     a.p = P;
     a.in = d_alm;
@@ -1237,8 +1239,7 @@ static cudaError_t run_synthesis_cfg(const HostPlan& hp, const void* d_alm, int 
     return cudaGetLastError();
 }
 
-static cudaError_t run_analysis_gemm(const HostPlan& hp, void* d_alm, int adjoint, cudaStream_t st) {
-    const DevPlan& P = hp.d;
+static cudaError_t run_analysis_gemm(const HostPlan& hp, const DevPlan& P, void* d_alm, int adjoint, cudaStream_t st) {
     LegArgs a;
     a.p = P;
     a.in = nullptr;
@@ -1272,17 +1273,16 @@ static cudaError_t run_analysis_gemm(const HostPlan& hp, void* d_alm, int adjoin
 }
 
 // Configurations below are the winners of sweeps on B200 (profiles/r1_legendre_tuning.md).
-cudaError_t launch_legendre_analysis(const HostPlan& hp, void* d_alm, int adjoint, cudaStream_t st) {
+cudaError_t launch_legendre_analysis(const HostPlan& hp, const DevPlan& P, void* d_alm, int adjoint, cudaStream_t st) {
     // in-place accumulation over ring chunks (SEQ): cfg5 88.3 -> 87.0 ms, 3.7 GB of partial writes and 4.3 GB of workspace gone
-    if (hp.dtype == CUHPX_F64) return run_analysis_cfg<double, 1, 8, 8, 128, 64, true>(hp, d_alm, adjoint, st);
-    if (hp.d.batch >= 5) return run_analysis_gemm(hp, d_alm, adjoint, st);
-    if (hp.d.batch >= 4) return run_analysis<float, 4>(hp, d_alm, adjoint, st);
-    return run_analysis<float, 1>(hp, d_alm, adjoint, st);
+    if (hp.dtype == CUHPX_F64) return run_analysis_cfg<double, 1, 8, 8, 128, 64, true>(hp, P, d_alm, adjoint, st);
+    if (P.batch >= 5) return run_analysis_gemm(hp, P, d_alm, adjoint, st);
+    if (P.batch >= 4) return run_analysis<float, 4>(hp, P, d_alm, adjoint, st);
+    return run_analysis<float, 1>(hp, P, d_alm, adjoint, st);
 }
 
 template <int BT, int R, int NT, int MINB>
-static cudaError_t run_synthesis_f32x2(const HostPlan& hp, const void* d_alm, int adjoint, cudaStream_t st) {
-    const DevPlan& P = hp.d;
+static cudaError_t run_synthesis_f32x2(const HostPlan& hp, const DevPlan& P, const void* d_alm, int adjoint, cudaStream_t st) {
     LegArgs a;
     a.p = P;
     a.in = d_alm;
@@ -1295,15 +1295,15 @@ static cudaError_t run_synthesis_f32x2(const HostPlan& hp, const void* d_alm, in
     return cudaGetLastError();
 }
 
-cudaError_t launch_legendre_synthesis(const HostPlan& hp, const void* d_alm, int adjoint, cudaStream_t st) {
-    if (hp.dtype == CUHPX_F64) return run_synthesis_cfg<double, 1, 4, 128>(hp, d_alm, adjoint, st);
-    if (hp.d.batch >= 8) {
+cudaError_t launch_legendre_synthesis(const HostPlan& hp, const DevPlan& P, const void* d_alm, int adjoint, cudaStream_t st) {
+    if (hp.dtype == CUHPX_F64) return run_synthesis_cfg<double, 1, 4, 128>(hp, P, d_alm, adjoint, st);
+    if (P.batch >= 8) {
         // packed-FMA kernels, 8 channels per CTA; short degree ranges want more, smaller CTAs in flight
-        return hp.d.lmax < 512 ? run_synthesis_f32x2<8, 1, 256, 3>(hp, d_alm, adjoint, st)
-                               : run_synthesis_f32x2<8, 2, 128, 3>(hp, d_alm, adjoint, st);
+        return P.lmax < 512 ? run_synthesis_f32x2<8, 1, 256, 3>(hp, P, d_alm, adjoint, st)
+                               : run_synthesis_f32x2<8, 2, 128, 3>(hp, P, d_alm, adjoint, st);
     }
-    if (hp.d.batch >= 4) return run_synthesis<float, 4>(hp, d_alm, adjoint, st);
-    return run_synthesis<float, 1>(hp, d_alm, adjoint, st);
+    if (P.batch >= 4) return run_synthesis<float, 4>(hp, P, d_alm, adjoint, st);
+    return run_synthesis<float, 1>(hp, P, d_alm, adjoint, st);
 }
 
 // ------------------------------------------------------------------ iterative refinement, elementwise steps (Eq. 4)

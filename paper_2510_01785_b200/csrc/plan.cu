@@ -1,10 +1,16 @@
 // Host side of libcuhpx.so: argument validation, HEALPix ring geometry, seed / cut-off
-// tables, workspace carve-up, the workspace registry and the extern "C" entry points of include/cuhpx.h.
+// tables, workspace carve-up and the extern "C" entry points of include/cuhpx.h.
+//
+// The library keeps NO per-workspace state (SURVEY 8(b) "Conventions"): everything a call needs on the host --
+// ring lists, cut-offs, launch shapes, table offsets -- is a pure function of (nside, lmax, mmax, batch, dtype)
+// and is memoised under that key; device tables are addressed as workspace base + offset, so a workspace may be
+// copied, moved or freed by its owner without telling the library.  The first 256 bytes of an initialised
+// workspace hold a header (magic, key) that every kernel checks before it trusts a table.
 #include <cuda_runtime.h>
 #include <math.h>
 #include <string.h>
 
-#include <map>
+#include <list>
 #include <mutex>
 #include <vector>
 
@@ -19,13 +25,12 @@ namespace {
 typedef long double ld;
 const ld PI_LD = 3.14159265358979323846264338327950288419716939937510L;
 
-std::mutex g_mu;
-std::map<void*, HostPlan*> g_plans;
+constexpr int MAX_BATCH = 65535;  // channels index gridDim.y / gridDim.z
 
 bool valid_args(int nside, int lmax, int mmax, int batch, int dtype) {
     if (nside < 1 || nside > (1 << 13) || !is_pow2(nside)) return false;
     if (lmax < 0 || mmax < 0 || mmax > lmax || lmax > 4 * (1 << 13)) return false;
-    if (batch < 1 || batch > (1 << 20)) return false;
+    if (batch < 1 || batch > MAX_BATCH) return false;
     if (dtype != CUHPX_F32 && dtype != CUHPX_F64) return false;
     return true;
 }
@@ -95,48 +100,13 @@ bool pair_active(int lmax, int m, ld pref_m, ld lg2sin, double yj) {
     return false;
 }
 
-struct Layout {
-    size_t off_y, off_lshi, off_lslo, off_ringN, off_start, off_shifted, off_mcut, off_prefhi, off_preflo, off_jmin;
-    size_t off_fft, fft_bytes, off_alpha, off_scale, off_spectra, off_partial, total;
-};
-
-Layout make_layout(HostPlan& hp) {
-    DevPlan& d = hp.d;
-    Layout L;
-    size_t o = 256;  // header
-    auto take = [&](size_t bytes) {
-        size_t r = o;
-        o = align_up(o + bytes);
-        return r;
-    };
-    L.off_y = take(sizeof(double) * d.npairs);
-    L.off_lshi = take(sizeof(double) * d.npairs);
-    L.off_lslo = take(sizeof(double) * d.npairs);
-    L.off_ringN = take(sizeof(int) * d.npairs);
-    L.off_start = take(sizeof(long long) * d.npairs);
-    L.off_shifted = take(sizeof(int) * d.npairs);
-    L.off_mcut = take(sizeof(int) * d.npairs);
-    L.off_prefhi = take(sizeof(double) * (d.mmax + 1));
-    L.off_preflo = take(sizeof(double) * (d.mmax + 1));
-    L.off_jmin = take(sizeof(int) * (d.mmax + 1));
-    L.off_fft = o;
-    cudaError_t err = cudaSuccess;
-    L.fft_bytes = plan_fft_tables(hp, nullptr, false, nullptr, &err);
-    o = align_up(o + L.fft_bytes);
-    L.off_alpha = take(sizeof(double) * (size_t)d.nalm);
-    L.off_scale = take(sizeof(double) * (size_t)d.nalm);
-    const size_t csize = hp.dtype == CUHPX_F64 ? 16 : 8;
-    L.off_spectra = take(csize * (size_t)d.batch * d.nrings * d.mstride);
-    L.off_partial = o;
-    if (d.nchunk_max > 1) take(csize * (size_t)d.nchunk_max * d.batch * d.nalm);
-    L.total = o;
-    return L;
-}
-
-void fill_basic(HostPlan& hp, int nside, int lmax, int mmax, int batch, cuhpx_dtype_t dt) {
-    DevPlan& d = hp.d;
+// Everything the host needs for (nside, lmax, mmax, batch, dtype): geometry, seeds, cut-offs, FFT ring classes, offsets.
+HostPlan* make_plan(int nside, int lmax, int mmax, int batch, cuhpx_dtype_t dt) {
+    HostPlan* hp = new HostPlan;
+    DevPlan& d = hp->d;
     memset(&d, 0, sizeof(d));
-    hp.dtype = dt;
+    hp->dtype = dt;
+    hp->geometry = 0;
     d.nside = nside;
     d.lmax = lmax;
     d.mmax = mmax;
@@ -146,42 +116,166 @@ void fill_basic(HostPlan& hp, int nside, int lmax, int mmax, int batch, cuhpx_dt
     d.mstride = (int)cuhpx_spectra_stride(mmax);
     d.npix = 12LL * nside * nside;
     d.nalm = (long long)cuhpx_alm_count(lmax, mmax);
+    d.key = plan_key(nside, lmax, mmax, batch, (int)dt, 0);
     d.chunk_pairs = legendre_chunk_pairs(dt, batch, lmax, d.npairs);
     d.nchunk_max = (d.npairs + d.chunk_pairs - 1) / d.chunk_pairs;
-    hp.h_ringN.resize(d.npairs);
-    hp.h_start.resize(d.npairs);
-    hp.h_shifted.resize(d.npairs);
+
+    // ---- per-pair and per-m tables (long double on the host, SURVEY 8(a) a0)
+    hp->h_ringN.resize(d.npairs);
+    hp->h_start.resize(d.npairs);
+    hp->h_shifted.resize(d.npairs);
+    hp->h_y.resize(d.npairs);
+    hp->h_lshi.resize(d.npairs);
+    hp->h_lslo.resize(d.npairs);
+    hp->h_prefhi.resize(mmax + 1);
+    hp->h_preflo.resize(mmax + 1);
+    std::vector<ld> lg2sin(d.npairs), pref(mmax + 1);
     for (int j = 0; j < d.npairs; ++j) {
         PairGeom g = pair_geom(nside, j);
-        hp.h_ringN[j] = g.N;
-        hp.h_start[j] = g.start;
-        hp.h_shifted[j] = g.shifted;
+        hp->h_ringN[j] = g.N;
+        hp->h_start[j] = g.start;
+        hp->h_shifted[j] = g.shifted;
+        hp->h_y[j] = (double)g.y;
+        lg2sin[j] = log2l(g.sth);
+        split_hi_lo(lg2sin[j], hp->h_lshi[j], hp->h_lslo[j]);
     }
+    // log2 |lambda_mm| = -0.5 log2(4 pi) + 0.5 sum_{k<=m} log2(1 + 1/(2k)) + m log2 sin(theta)   (Eq. 15 P:195)
+    ld acc = -0.5L * log2l(4.0L * PI_LD);
+    for (int m = 0; m <= mmax; ++m) {
+        if (m > 0) acc += 0.5L * log1pl(1.0L / (2.0L * m)) / logl(2.0L);
+        pref[m] = acc;
+        split_hi_lo(acc, hp->h_prefhi[m], hp->h_preflo[m]);
+    }
+    // ---- jmin[m]: first ring pair that matters at order m (two-pointer: the active set shrinks with m)
+    hp->h_jmin.assign(mmax + 1, 0);
+    int j = 0;
+    for (int m = 0; m <= mmax; ++m) {
+        while (j < d.npairs - 1 && !pair_active(lmax, m, pref[m], lg2sin[j], hp->h_y[j])) ++j;
+        hp->h_jmin[m] = j;
+    }
+    // ---- mcut[j]: last order at which pair j is processed (monotone non-decreasing in j, as the sweep implies)
+    hp->h_mcut.assign(d.npairs, 0);
+    {
+        int m = mmax;
+        for (int jj = d.npairs - 1; jj >= 0; --jj) {
+            while (m > 0 && hp->h_jmin[m] > jj) --m;
+            hp->h_mcut[jj] = m;
+        }
+    }
+
+    // ---- workspace layout
+    size_t o = 256;  // header
+    auto take = [&](size_t bytes) {
+        size_t r = o;
+        o = align_up(o + bytes);
+        return r;
+    };
+    hp->off_y = take(sizeof(double) * d.npairs);
+    hp->off_lshi = take(sizeof(double) * d.npairs);
+    hp->off_lslo = take(sizeof(double) * d.npairs);
+    hp->off_ringN = take(sizeof(int) * d.npairs);
+    hp->off_start = take(sizeof(long long) * d.npairs);
+    hp->off_shifted = take(sizeof(int) * d.npairs);
+    hp->off_mcut = take(sizeof(int) * d.npairs);
+    hp->off_prefhi = take(sizeof(double) * (d.mmax + 1));
+    hp->off_preflo = take(sizeof(double) * (d.mmax + 1));
+    hp->off_jmin = take(sizeof(int) * (d.mmax + 1));
+    hp->off_fft = o;
+    hp->fft_bytes = fft_plan_host(*hp);
+    o = align_up(o + hp->fft_bytes);
+    hp->off_alpha = take(sizeof(double) * (size_t)d.nalm);
+    hp->off_scale = take(sizeof(double) * (size_t)d.nalm);
+    const size_t csize = dt == CUHPX_F64 ? 16 : 8;
+    hp->off_spectra = take(csize * (size_t)d.batch * d.nrings * d.mstride);
+    hp->off_partial = o;
+    if (d.nchunk_max > 1) take(csize * (size_t)d.nchunk_max * d.batch * d.nalm);
+    hp->workspace_bytes = o;
+    return hp;
 }
 
-HostPlan* find_plan(void* ws) {
+// memo of host plans (bounded; entries are immutable and shared, so eviction never invalidates a running call)
+struct PlanKey {
+    int nside, lmax, mmax, batch, dtype;
+    bool operator==(const PlanKey& o) const {
+        return nside == o.nside && lmax == o.lmax && mmax == o.mmax && batch == o.batch && dtype == o.dtype;
+    }
+};
+std::mutex g_mu;
+std::list<std::pair<PlanKey, PlanRef>> g_plans;  // most recently used first
+constexpr size_t MAX_PLANS = 24;
+
+PlanRef get_plan(int nside, int lmax, int mmax, int batch, cuhpx_dtype_t dt) {
+    const PlanKey k{nside, lmax, mmax, batch, (int)dt};
+    {
+        std::lock_guard<std::mutex> lk(g_mu);
+        for (auto it = g_plans.begin(); it != g_plans.end(); ++it)
+            if (it->first == k) {
+                g_plans.splice(g_plans.begin(), g_plans, it);
+                return g_plans.front().second;
+            }
+    }
+    PlanRef p(make_plan(nside, lmax, mmax, batch, dt));  // built outside the lock (may take a while at nside 4096)
     std::lock_guard<std::mutex> lk(g_mu);
-    auto it = g_plans.find(ws);
-    return it == g_plans.end() ? nullptr : it->second;
+    for (auto& e : g_plans)
+        if (e.first == k) return e.second;
+    g_plans.emplace_front(k, p);
+    while (g_plans.size() > MAX_PLANS) g_plans.pop_back();
+    return p;
 }
 
-int check_call(HostPlan** out, int nside, int lmax, int mmax, int batch, cuhpx_dtype_t dt, const void* a,
-               const void* b, void* ws, size_t ws_bytes) {
+bool overlap(const void* a, size_t na, const void* b, size_t nb) {
+    const uintptr_t pa = (uintptr_t)a, pb = (uintptr_t)b;
+    return pa < pb + nb && pb < pa + na;
+}
+
+size_t map_bytes(const HostPlan& hp) { return (size_t)hp.d.batch * (size_t)hp.d.npix * (hp.dtype == CUHPX_F64 ? 8 : 4); }
+size_t alm_bytes(const HostPlan& hp) { return (size_t)hp.d.batch * (size_t)hp.d.nalm * (hp.dtype == CUHPX_F64 ? 16 : 8); }
+
+// Argument checks shared by the operators; a / b are the data buffers with their sizes (either may be null for the
+// stage-level calls, which touch only one user buffer).
+int check_call(PlanRef* out, int nside, int lmax, int mmax, int batch, int dt, const void* a, size_t na, const void* b,
+               size_t nb, const void* ws, size_t ws_bytes) {
     if (!valid_args(nside, lmax, mmax, batch, dt)) return CUHPX_EINVAL;
-    if (!a || !b || !ws) return CUHPX_EINVAL;
+    if ((na && !a) || (nb && !b) || !ws) return CUHPX_EINVAL;
     if (((uintptr_t)a & 15) || ((uintptr_t)b & 15) || ((uintptr_t)ws & 15)) return CUHPX_EINVAL;
-    if (a == b) return CUHPX_EINVAL;
-    HostPlan* hp = find_plan(ws);
-    if (!hp) return CUHPX_EWORKSPACE;
-    const DevPlan& d = hp->d;
-    if (d.nside != nside || d.lmax != lmax || d.mmax != mmax || d.batch != batch || hp->dtype != dt)
-        return CUHPX_EWORKSPACE;
+    // the map may hold up to 4 nside * 4 nside-ish rings of any supported length; unsupported ring lengths were
+    // refused by cuhpx_workspace_bytes / cuhpx_workspace_init already
+    if (!fft_supported(4 * nside, (cuhpx_dtype_t)dt)) return CUHPX_EUNSUPPORTED;
+    PlanRef hp = get_plan(nside, lmax, mmax, batch, (cuhpx_dtype_t)dt);
     if (ws_bytes < hp->workspace_bytes) return CUHPX_EWORKSPACE;
+    const size_t sa = a ? (na == (size_t)-1 ? map_bytes(*hp) : na == (size_t)-2 ? alm_bytes(*hp) : na) : 0;
+    const size_t sb = b ? (nb == (size_t)-1 ? map_bytes(*hp) : nb == (size_t)-2 ? alm_bytes(*hp) : nb) : 0;
+    if (a && b && overlap(a, sa, b, sb)) return CUHPX_EINVAL;
+    if (a && overlap(a, sa, ws, hp->workspace_bytes)) return CUHPX_EINVAL;
+    if (b && overlap(b, sb, ws, hp->workspace_bytes)) return CUHPX_EINVAL;
     *out = hp;
     return CUHPX_OK;
 }
+constexpr size_t MAP = (size_t)-1, ALM = (size_t)-2;  // "size of one map / alm array of this plan"
 
 }  // namespace
+
+DevPlan HostPlan::resolve(void* ws) const {
+    DevPlan P = d;
+    char* base = (char*)ws;
+    P.hdr = (const WsHeader*)base;
+    P.y = (const double*)(base + off_y);
+    P.ls_hi = (const double*)(base + off_lshi);
+    P.ls_lo = (const double*)(base + off_lslo);
+    P.ringN = (const int*)(base + off_ringN);
+    P.start = (const long long*)(base + off_start);
+    P.shifted = (const int*)(base + off_shifted);
+    P.mcut = (const int*)(base + off_mcut);
+    P.pref_hi = (const double*)(base + off_prefhi);
+    P.pref_lo = (const double*)(base + off_preflo);
+    P.jmin = (const int*)(base + off_jmin);
+    P.coef_alpha = (const double*)(base + off_alpha);
+    P.coef_scale = (const double*)(base + off_scale);
+    P.spectra = base + off_spectra;
+    P.partial = d.nchunk_max > 1 ? base + off_partial : nullptr;
+    return P;
+}
+
 }  // namespace cuhpx
 
 using namespace cuhpx;
@@ -210,7 +304,7 @@ size_t cuhpx_spectra_stride(int mmax) { return (size_t)((mmax + 1 + 1) / 2 * 2);
 const char* cuhpx_status_string(int s) {
     switch (s) {
         case CUHPX_OK: return "CUHPX_OK";
-        case CUHPX_EINVAL: return "CUHPX_EINVAL: bad nside/lmax/mmax/batch/dtype or null/misaligned/aliased pointer";
+        case CUHPX_EINVAL: return "CUHPX_EINVAL: bad nside/lmax/mmax/batch/dtype or null/misaligned/overlapping pointer";
         case CUHPX_EWORKSPACE: return "CUHPX_EWORKSPACE: workspace too small, not initialised or for other parameters";
         case CUHPX_EUNSUPPORTED: return "CUHPX_EUNSUPPORTED: request not supported by this build";
         case CUHPX_ECUDA: return "CUHPX_ECUDA: CUDA runtime error (see cudaGetLastError)";
@@ -233,135 +327,81 @@ int cuhpx_ring_info(int nside, int ring, long long* n_pix, long long* first_pix,
 }
 
 size_t cuhpx_workspace_bytes(int nside, int lmax, int mmax, int batch, cuhpx_dtype_t dtype) {
-    if (!valid_args(nside, lmax, mmax, batch, dtype) || !fft_supported(nside, dtype)) return 0;
-    HostPlan hp;
-    fill_basic(hp, nside, lmax, mmax, batch, dtype);
-    return make_layout(hp).total;
+    if (!valid_args(nside, lmax, mmax, batch, dtype) || !fft_supported(4 * nside, dtype)) return 0;
+    return get_plan(nside, lmax, mmax, batch, dtype)->workspace_bytes;
 }
 
 int cuhpx_workspace_init(int nside, int lmax, int mmax, int batch, cuhpx_dtype_t dtype, void* ws, size_t ws_bytes,
                          cuhpx_stream_t stream) {
     if (!valid_args(nside, lmax, mmax, batch, dtype)) return CUHPX_EINVAL;
     if (!ws || ((uintptr_t)ws & 15)) return CUHPX_EINVAL;
-    if (!fft_supported(nside, dtype)) return CUHPX_EUNSUPPORTED;
-    HostPlan* hp = new HostPlan;
-    fill_basic(*hp, nside, lmax, mmax, batch, dtype);
-    Layout L = make_layout(*hp);
-    hp->workspace_bytes = L.total;
-    if (ws_bytes < L.total) {
-        delete hp;
-        return CUHPX_EWORKSPACE;
-    }
-    DevPlan& d = hp->d;
+    if (!fft_supported(4 * nside, dtype)) return CUHPX_EUNSUPPORTED;
+    PlanRef hp = get_plan(nside, lmax, mmax, batch, dtype);
+    if (ws_bytes < hp->workspace_bytes) return CUHPX_EWORKSPACE;
+    const DevPlan& d = hp->d;
     char* base = (char*)ws;
     cudaStream_t st = (cudaStream_t)stream;
-
-    // ---- per-pair and per-m tables (long double on the host, SURVEY 8(a) a0)
-    std::vector<double> y(d.npairs), lshi(d.npairs), lslo(d.npairs), prefhi(mmax + 1), preflo(mmax + 1);
-    std::vector<ld> lg2sin(d.npairs), pref(mmax + 1);
-    for (int j = 0; j < d.npairs; ++j) {
-        PairGeom g = pair_geom(nside, j);
-        y[j] = (double)g.y;
-        lg2sin[j] = log2l(g.sth);
-        split_hi_lo(lg2sin[j], lshi[j], lslo[j]);
-    }
-    // log2 |lambda_mm| = -0.5 log2(4 pi) + 0.5 sum_{k<=m} log2(1 + 1/(2k)) + m log2 sin(theta)   (Eq. 15 P:195)
-    ld acc = -0.5L * log2l(4.0L * PI_LD);
-    for (int m = 0; m <= mmax; ++m) {
-        if (m > 0) acc += 0.5L * log1pl(1.0L / (2.0L * m)) / logl(2.0L);
-        pref[m] = acc;
-        split_hi_lo(acc, prefhi[m], preflo[m]);
-    }
-    // ---- jmin[m]: first ring pair that matters at order m (two-pointer: the active set shrinks with m)
-    hp->h_jmin.assign(mmax + 1, 0);
-    int j = 0;
-    for (int m = 0; m <= mmax; ++m) {
-        while (j < d.npairs - 1 && !pair_active(lmax, m, pref[m], lg2sin[j], y[j])) ++j;
-        hp->h_jmin[m] = j;
-    }
-    // ---- mcut[j]: last order at which pair j is processed
-    hp->h_mcut.assign(d.npairs, 0);
-    {
-        int m = mmax;
-        for (int jj = d.npairs - 1; jj >= 0; --jj) {
-            while (m > 0 && hp->h_jmin[m] > jj) --m;
-            hp->h_mcut[jj] = m;
-        }
-        // make it monotone non-decreasing in j as the sweep implies
-    }
 
     cudaError_t e = cudaSuccess;
     auto up = [&](size_t off, const void* src, size_t bytes) {
         if (e == cudaSuccess) e = cudaMemcpyAsync(base + off, src, bytes, cudaMemcpyHostToDevice, st);
     };
-    up(L.off_y, y.data(), sizeof(double) * d.npairs);
-    up(L.off_lshi, lshi.data(), sizeof(double) * d.npairs);
-    up(L.off_lslo, lslo.data(), sizeof(double) * d.npairs);
-    up(L.off_ringN, hp->h_ringN.data(), sizeof(int) * d.npairs);
-    up(L.off_start, hp->h_start.data(), sizeof(long long) * d.npairs);
-    up(L.off_shifted, hp->h_shifted.data(), sizeof(int) * d.npairs);
-    up(L.off_mcut, hp->h_mcut.data(), sizeof(int) * d.npairs);
-    up(L.off_prefhi, prefhi.data(), sizeof(double) * (mmax + 1));
-    up(L.off_preflo, preflo.data(), sizeof(double) * (mmax + 1));
-    up(L.off_jmin, hp->h_jmin.data(), sizeof(int) * (mmax + 1));
-    // pageable sources: make sure the copies are done before the vectors die
-    if (e == cudaSuccess) e = cudaStreamSynchronize(st);
-
-    d.y = (const double*)(base + L.off_y);
-    d.ls_hi = (const double*)(base + L.off_lshi);
-    d.ls_lo = (const double*)(base + L.off_lslo);
-    d.ringN = (const int*)(base + L.off_ringN);
-    d.start = (const long long*)(base + L.off_start);
-    d.shifted = (const int*)(base + L.off_shifted);
-    d.mcut = (const int*)(base + L.off_mcut);
-    d.pref_hi = (const double*)(base + L.off_prefhi);
-    d.pref_lo = (const double*)(base + L.off_preflo);
-    d.jmin = (const int*)(base + L.off_jmin);
-    d.coef_alpha = (const double*)(base + L.off_alpha);
-    d.coef_scale = (const double*)(base + L.off_scale);
+    // a header that matches nothing while the tables are being (re)built
+    WsHeader hdr;
+    memset(&hdr, 0, sizeof(hdr));
+    up(0, &hdr, sizeof(hdr));
+    if (e == cudaSuccess) e = cudaStreamSynchronize(st);  // hdr is rewritten below; the copy must have read it
+    up(hp->off_y, hp->h_y.data(), sizeof(double) * d.npairs);
+    up(hp->off_lshi, hp->h_lshi.data(), sizeof(double) * d.npairs);
+    up(hp->off_lslo, hp->h_lslo.data(), sizeof(double) * d.npairs);
+    up(hp->off_ringN, hp->h_ringN.data(), sizeof(int) * d.npairs);
+    up(hp->off_start, hp->h_start.data(), sizeof(long long) * d.npairs);
+    up(hp->off_shifted, hp->h_shifted.data(), sizeof(int) * d.npairs);
+    up(hp->off_mcut, hp->h_mcut.data(), sizeof(int) * d.npairs);
+    up(hp->off_prefhi, hp->h_prefhi.data(), sizeof(double) * (mmax + 1));
+    up(hp->off_preflo, hp->h_preflo.data(), sizeof(double) * (mmax + 1));
+    up(hp->off_jmin, hp->h_jmin.data(), sizeof(int) * (mmax + 1));
     if (e == cudaSuccess)
-        e = launch_legendre_coeff(lmax, mmax, (double*)(base + L.off_alpha), (double*)(base + L.off_scale), st);
-    d.spectra = base + L.off_spectra;
-    d.partial = d.nchunk_max > 1 ? base + L.off_partial : nullptr;
+        e = launch_legendre_coeff(lmax, mmax, (double*)(base + hp->off_alpha), (double*)(base + hp->off_scale), st);
+    if (e == cudaSuccess) e = fft_build_tables(*hp, base + hp->off_fft, st);
+    hdr.magic = WS_MAGIC;
+    hdr.key = d.key;
+    hdr.nside = nside;
+    hdr.lmax = lmax;
+    hdr.mmax = mmax;
+    hdr.batch = batch;
+    hdr.dtype = (int)dtype;
+    hdr.geometry = hp->geometry;
+    hdr.bytes = hp->workspace_bytes;
+    up(0, &hdr, sizeof(hdr));
+    // the sources above are pageable host memory owned by the (shared, immutable) plan or by this frame
+    if (e == cudaSuccess) e = cudaStreamSynchronize(st);
+    return e == cudaSuccess ? CUHPX_OK : CUHPX_ECUDA;
+}
 
-    if (e == cudaSuccess) {
-        cudaError_t e2 = cudaSuccess;
-        plan_fft_tables(*hp, base + L.off_fft, true, st, &e2);
-        e = e2;
-    }
-    if (e != cudaSuccess) {
-        delete hp;
-        return CUHPX_ECUDA;
-    }
-    {
-        std::lock_guard<std::mutex> lk(g_mu);
-        auto it = g_plans.find(ws);
-        if (it != g_plans.end()) {
-            delete it->second;
-            g_plans.erase(it);
-        }
-        g_plans[ws] = hp;
-    }
+int cuhpx_workspace_check(int nside, int lmax, int mmax, int batch, cuhpx_dtype_t dtype, const void* ws, size_t ws_bytes,
+                          cuhpx_stream_t stream) {
+    if (!valid_args(nside, lmax, mmax, batch, dtype)) return CUHPX_EINVAL;
+    if (!ws || ((uintptr_t)ws & 15)) return CUHPX_EINVAL;
+    if (!fft_supported(4 * nside, dtype)) return CUHPX_EUNSUPPORTED;
+    PlanRef hp = get_plan(nside, lmax, mmax, batch, dtype);
+    if (ws_bytes < hp->workspace_bytes) return CUHPX_EWORKSPACE;
+    WsHeader hdr;
+    if (cudaMemcpyAsync(&hdr, ws, sizeof(hdr), cudaMemcpyDeviceToHost, (cudaStream_t)stream) != cudaSuccess) return CUHPX_ECUDA;
+    if (cudaStreamSynchronize((cudaStream_t)stream) != cudaSuccess) return CUHPX_ECUDA;
+    if (hdr.magic != WS_MAGIC || hdr.key != hp->d.key || hdr.bytes != hp->workspace_bytes || hdr.bad) return CUHPX_EWORKSPACE;
     return CUHPX_OK;
 }
 
-int cuhpx_workspace_release(void* ws) {
-    std::lock_guard<std::mutex> lk(g_mu);
-    auto it = g_plans.find(ws);
-    if (it == g_plans.end()) return CUHPX_EWORKSPACE;
-    delete it->second;
-    g_plans.erase(it);
-    return CUHPX_OK;
+size_t cuhpx_spectra_offset(int nside, int lmax, int mmax, int batch, cuhpx_dtype_t dtype) {
+    if (!valid_args(nside, lmax, mmax, batch, dtype) || !fft_supported(4 * nside, dtype)) return 0;
+    return get_plan(nside, lmax, mmax, batch, dtype)->off_spectra;
 }
 
-void* cuhpx_workspace_spectra(void* ws) {
-    HostPlan* hp = find_plan(ws);
-    return hp ? hp->d.spectra : nullptr;
-}
-
-int cuhpx_workspace_mcut(void* ws, int* h_mcut) {
-    HostPlan* hp = find_plan(ws);
-    if (!hp || !h_mcut) return CUHPX_EWORKSPACE;
+int cuhpx_plan_mcut(int nside, int lmax, int mmax, int batch, cuhpx_dtype_t dtype, int* h_mcut) {
+    if (!valid_args(nside, lmax, mmax, batch, dtype) || !h_mcut) return CUHPX_EINVAL;
+    if (!fft_supported(4 * nside, dtype)) return CUHPX_EUNSUPPORTED;
+    PlanRef hp = get_plan(nside, lmax, mmax, batch, dtype);
     const DevPlan& d = hp->d;
     for (int r = 0; r < d.nrings; ++r) {
         const int j = r < d.nrings - 1 - r ? r : d.nrings - 1 - r;
@@ -370,9 +410,10 @@ int cuhpx_workspace_mcut(void* ws, int* h_mcut) {
     return CUHPX_OK;
 }
 
-int cuhpx_workspace_stats(void* ws, double* out, int count) {
-    HostPlan* hp = find_plan(ws);
-    if (!hp || !out || count < 1) return CUHPX_EWORKSPACE;
+int cuhpx_plan_stats(int nside, int lmax, int mmax, int batch, cuhpx_dtype_t dtype, double* out, int count) {
+    if (!valid_args(nside, lmax, mmax, batch, dtype) || !out || count < 1) return CUHPX_EINVAL;
+    if (!fft_supported(4 * nside, dtype)) return CUHPX_EUNSUPPORTED;
+    PlanRef hp = get_plan(nside, lmax, mmax, batch, dtype);
     const DevPlan& d = hp->d;
     double st[8] = {0};
     int fl = 0;
@@ -395,108 +436,125 @@ int cuhpx_workspace_stats(void* ws, double* out, int count) {
         if ((expr) != cudaSuccess) return CUHPX_ECUDA; \
     } while (0)
 
-int cuhpx_analysis_fft_stage(const void* d_map, const double* d_w, int use_w, void* ws, cuhpx_stream_t stream) {
-    HostPlan* hp = find_plan(ws);
-    if (!hp) return CUHPX_EWORKSPACE;
-    if (!d_map) return CUHPX_EINVAL;
-    CUDA_OR_FAIL(launch_fft_analysis(*hp, d_map, d_w, use_w, (cudaStream_t)stream));
+int cuhpx_analysis_fft_stage(int nside, int lmax, int mmax, int batch, cuhpx_dtype_t dt, const void* d_map,
+                             const double* d_w, int use_w, void* ws, size_t ws_bytes, cuhpx_stream_t stream) {
+    PlanRef hp;
+    int rc = check_call(&hp, nside, lmax, mmax, batch, dt, d_map, MAP, nullptr, 0, ws, ws_bytes);
+    if (rc) return rc;
+    if (d_w && ((uintptr_t)d_w & 7)) return CUHPX_EINVAL;
+    CUDA_OR_FAIL(launch_fft_analysis(*hp, hp->resolve(ws), d_map, d_w, use_w, (cudaStream_t)stream));
     return CUHPX_OK;
 }
 
-int cuhpx_analysis_legendre_stage(void* d_alm, int adjoint, void* ws, cuhpx_stream_t stream) {
-    HostPlan* hp = find_plan(ws);
-    if (!hp) return CUHPX_EWORKSPACE;
-    if (!d_alm) return CUHPX_EINVAL;
-    CUDA_OR_FAIL(launch_legendre_analysis(*hp, d_alm, adjoint, (cudaStream_t)stream));
+int cuhpx_analysis_legendre_stage(int nside, int lmax, int mmax, int batch, cuhpx_dtype_t dt, void* d_alm, int adjoint,
+                                  void* ws, size_t ws_bytes, cuhpx_stream_t stream) {
+    PlanRef hp;
+    int rc = check_call(&hp, nside, lmax, mmax, batch, dt, d_alm, ALM, nullptr, 0, ws, ws_bytes);
+    if (rc) return rc;
+    CUDA_OR_FAIL(launch_legendre_analysis(*hp, hp->resolve(ws), d_alm, adjoint, (cudaStream_t)stream));
     return CUHPX_OK;
 }
 
-int cuhpx_synthesis_legendre_stage(const void* d_alm, int adjoint, void* ws, cuhpx_stream_t stream) {
-    HostPlan* hp = find_plan(ws);
-    if (!hp) return CUHPX_EWORKSPACE;
-    if (!d_alm) return CUHPX_EINVAL;
-    CUDA_OR_FAIL(launch_legendre_synthesis(*hp, d_alm, adjoint, (cudaStream_t)stream));
+int cuhpx_synthesis_legendre_stage(int nside, int lmax, int mmax, int batch, cuhpx_dtype_t dt, const void* d_alm,
+                                   int adjoint, void* ws, size_t ws_bytes, cuhpx_stream_t stream) {
+    PlanRef hp;
+    int rc = check_call(&hp, nside, lmax, mmax, batch, dt, d_alm, ALM, nullptr, 0, ws, ws_bytes);
+    if (rc) return rc;
+    CUDA_OR_FAIL(launch_legendre_synthesis(*hp, hp->resolve(ws), d_alm, adjoint, (cudaStream_t)stream));
     return CUHPX_OK;
 }
 
-int cuhpx_synthesis_fft_stage(void* d_map, const double* d_w, int use_w, void* ws, cuhpx_stream_t stream) {
-    HostPlan* hp = find_plan(ws);
-    if (!hp) return CUHPX_EWORKSPACE;
-    if (!d_map) return CUHPX_EINVAL;
-    CUDA_OR_FAIL(launch_fft_synthesis(*hp, d_map, d_w, use_w, (cudaStream_t)stream));
+int cuhpx_synthesis_fft_stage(int nside, int lmax, int mmax, int batch, cuhpx_dtype_t dt, void* d_map, const double* d_w,
+                              int use_w, void* ws, size_t ws_bytes, cuhpx_stream_t stream) {
+    PlanRef hp;
+    int rc = check_call(&hp, nside, lmax, mmax, batch, dt, d_map, MAP, nullptr, 0, ws, ws_bytes);
+    if (rc) return rc;
+    if (d_w && ((uintptr_t)d_w & 7)) return CUHPX_EINVAL;
+    CUDA_OR_FAIL(launch_fft_synthesis(*hp, hp->resolve(ws), d_map, d_w, use_w, (cudaStream_t)stream));
     return CUHPX_OK;
 }
 
 int cuhpx_map2alm(int nside, int lmax, int mmax, int batch, cuhpx_dtype_t dt, const void* d_map, void* d_alm,
                   const double* d_w, void* ws, size_t ws_bytes, cuhpx_stream_t stream) {
-    HostPlan* hp = nullptr;
-    int rc = check_call(&hp, nside, lmax, mmax, batch, dt, d_map, d_alm, ws, ws_bytes);
+    PlanRef hp;
+    int rc = check_call(&hp, nside, lmax, mmax, batch, dt, d_map, MAP, d_alm, ALM, ws, ws_bytes);
     if (rc) return rc;
     if (d_w && ((uintptr_t)d_w & 7)) return CUHPX_EINVAL;
     cudaStream_t st = (cudaStream_t)stream;
-    CUDA_OR_FAIL(launch_fft_analysis(*hp, d_map, d_w, 1, st));
-    CUDA_OR_FAIL(launch_legendre_analysis(*hp, d_alm, 0, st));
+    const DevPlan P = hp->resolve(ws);
+    CUDA_OR_FAIL(launch_fft_analysis(*hp, P, d_map, d_w, 1, st));
+    CUDA_OR_FAIL(launch_legendre_analysis(*hp, P, d_alm, 0, st));
     return CUHPX_OK;
 }
 
 int cuhpx_alm2map_adjoint(int nside, int lmax, int mmax, int batch, cuhpx_dtype_t dt, const void* d_gmap,
                           void* d_galm, void* ws, size_t ws_bytes, cuhpx_stream_t stream) {
-    HostPlan* hp = nullptr;
-    int rc = check_call(&hp, nside, lmax, mmax, batch, dt, d_gmap, d_galm, ws, ws_bytes);
+    PlanRef hp;
+    int rc = check_call(&hp, nside, lmax, mmax, batch, dt, d_gmap, MAP, d_galm, ALM, ws, ws_bytes);
     if (rc) return rc;
     cudaStream_t st = (cudaStream_t)stream;
-    CUDA_OR_FAIL(launch_fft_analysis(*hp, d_gmap, nullptr, 0, st));
-    CUDA_OR_FAIL(launch_legendre_analysis(*hp, d_galm, 1, st));
+    const DevPlan P = hp->resolve(ws);
+    CUDA_OR_FAIL(launch_fft_analysis(*hp, P, d_gmap, nullptr, 0, st));
+    CUDA_OR_FAIL(launch_legendre_analysis(*hp, P, d_galm, 1, st));
     return CUHPX_OK;
 }
 
 int cuhpx_alm2map(int nside, int lmax, int mmax, int batch, cuhpx_dtype_t dt, const void* d_alm, void* d_map,
                   void* ws, size_t ws_bytes, cuhpx_stream_t stream) {
-    HostPlan* hp = nullptr;
-    int rc = check_call(&hp, nside, lmax, mmax, batch, dt, d_alm, d_map, ws, ws_bytes);
+    PlanRef hp;
+    int rc = check_call(&hp, nside, lmax, mmax, batch, dt, d_alm, ALM, d_map, MAP, ws, ws_bytes);
     if (rc) return rc;
     cudaStream_t st = (cudaStream_t)stream;
-    CUDA_OR_FAIL(launch_legendre_synthesis(*hp, d_alm, 0, st));
-    CUDA_OR_FAIL(launch_fft_synthesis(*hp, d_map, nullptr, 0, st));
+    const DevPlan P = hp->resolve(ws);
+    CUDA_OR_FAIL(launch_legendre_synthesis(*hp, P, d_alm, 0, st));
+    CUDA_OR_FAIL(launch_fft_synthesis(*hp, P, d_map, nullptr, 0, st));
     return CUHPX_OK;
 }
 
 int cuhpx_map2alm_adjoint(int nside, int lmax, int mmax, int batch, cuhpx_dtype_t dt, const void* d_galm,
                           void* d_gmap, const double* d_w, void* ws, size_t ws_bytes, cuhpx_stream_t stream) {
-    HostPlan* hp = nullptr;
-    int rc = check_call(&hp, nside, lmax, mmax, batch, dt, d_galm, d_gmap, ws, ws_bytes);
+    PlanRef hp;
+    int rc = check_call(&hp, nside, lmax, mmax, batch, dt, d_galm, ALM, d_gmap, MAP, ws, ws_bytes);
     if (rc) return rc;
     if (d_w && ((uintptr_t)d_w & 7)) return CUHPX_EINVAL;
     cudaStream_t st = (cudaStream_t)stream;
-    CUDA_OR_FAIL(launch_legendre_synthesis(*hp, d_galm, 1, st));
-    CUDA_OR_FAIL(launch_fft_synthesis(*hp, d_gmap, d_w, 1, st));
+    const DevPlan P = hp->resolve(ws);
+    CUDA_OR_FAIL(launch_legendre_synthesis(*hp, P, d_galm, 1, st));
+    CUDA_OR_FAIL(launch_fft_synthesis(*hp, P, d_gmap, d_w, 1, st));
     return CUHPX_OK;
 }
 
 int cuhpx_map2alm_iter(int nside, int lmax, int mmax, int batch, cuhpx_dtype_t dt, const void* d_map, void* d_alm,
                        const double* d_w, int n_iter, void* d_scratch_map, void* d_scratch_alm, void* ws,
                        size_t ws_bytes, cuhpx_stream_t stream) {
-    HostPlan* hp = nullptr;
-    int rc = check_call(&hp, nside, lmax, mmax, batch, dt, d_map, d_alm, ws, ws_bytes);
+    PlanRef hp;
+    int rc = check_call(&hp, nside, lmax, mmax, batch, dt, d_map, MAP, d_alm, ALM, ws, ws_bytes);
     if (rc) return rc;
     if (d_w && ((uintptr_t)d_w & 7)) return CUHPX_EINVAL;
     if (n_iter < 0) return CUHPX_EINVAL;
-    if (n_iter > 0 && (!d_scratch_map || !d_scratch_alm || ((uintptr_t)d_scratch_map & 15) || ((uintptr_t)d_scratch_alm & 15) ||
-                       d_scratch_map == d_map || d_scratch_alm == d_alm))
-        return CUHPX_EINVAL;
+    if (n_iter > 0) {
+        PlanRef h2;
+        if ((rc = check_call(&h2, nside, lmax, mmax, batch, dt, d_scratch_map, MAP, d_scratch_alm, ALM, ws, ws_bytes))) return rc;
+        if (overlap(d_scratch_map, map_bytes(*hp), d_map, map_bytes(*hp)) ||
+            overlap(d_scratch_alm, alm_bytes(*hp), d_alm, alm_bytes(*hp)) ||
+            overlap(d_scratch_map, map_bytes(*hp), d_alm, alm_bytes(*hp)) ||
+            overlap(d_scratch_alm, alm_bytes(*hp), d_map, map_bytes(*hp)))
+            return CUHPX_EINVAL;
+    }
     cudaStream_t st = (cudaStream_t)stream;
+    const DevPlan P = hp->resolve(ws);
     // a^(0) = A f
-    CUDA_OR_FAIL(launch_fft_analysis(*hp, d_map, d_w, 1, st));
-    CUDA_OR_FAIL(launch_legendre_analysis(*hp, d_alm, 0, st));
-    const size_t nmap = (size_t)hp->d.batch * (size_t)hp->d.npix, nalm2 = 2 * (size_t)hp->d.batch * (size_t)hp->d.nalm;
+    CUDA_OR_FAIL(launch_fft_analysis(*hp, P, d_map, d_w, 1, st));
+    CUDA_OR_FAIL(launch_legendre_analysis(*hp, P, d_alm, 0, st));
+    const size_t nmap = (size_t)P.batch * (size_t)P.npix, nalm2 = 2 * (size_t)P.batch * (size_t)P.nalm;
     for (int k = 0; k < n_iter; ++k) {
         // r = f - S a
-        CUDA_OR_FAIL(launch_legendre_synthesis(*hp, d_alm, 0, st));
-        CUDA_OR_FAIL(launch_fft_synthesis(*hp, d_scratch_map, nullptr, 0, st));
+        CUDA_OR_FAIL(launch_legendre_synthesis(*hp, P, d_alm, 0, st));
+        CUDA_OR_FAIL(launch_fft_synthesis(*hp, P, d_scratch_map, nullptr, 0, st));
         CUDA_OR_FAIL(launch_residual(dt, d_map, d_scratch_map, nmap, st));
         // a += A r
-        CUDA_OR_FAIL(launch_fft_analysis(*hp, d_scratch_map, d_w, 1, st));
-        CUDA_OR_FAIL(launch_legendre_analysis(*hp, d_scratch_alm, 0, st));
+        CUDA_OR_FAIL(launch_fft_analysis(*hp, P, d_scratch_map, d_w, 1, st));
+        CUDA_OR_FAIL(launch_legendre_analysis(*hp, P, d_scratch_alm, 0, st));
         CUDA_OR_FAIL(launch_accumulate(dt, d_scratch_alm, d_alm, nalm2, st));
     }
     return CUHPX_OK;
@@ -504,9 +562,12 @@ int cuhpx_map2alm_iter(int nside, int lmax, int mmax, int batch, cuhpx_dtype_t d
 
 int cuhpx_reorder(int nside, int batch, cuhpx_dtype_t dt, int direction, const void* d_in, void* d_out,
                   cuhpx_stream_t stream) {
-    if (nside < 1 || !is_pow2(nside) || nside > (1 << 13) || batch < 1 || (dt != CUHPX_F32 && dt != CUHPX_F64)) return CUHPX_EINVAL;
+    if (nside < 1 || !is_pow2(nside) || nside > (1 << 13) || batch < 1 || batch > MAX_BATCH || (dt != CUHPX_F32 && dt != CUHPX_F64))
+        return CUHPX_EINVAL;
     if (direction != CUHPX_NEST2RING && direction != CUHPX_RING2NEST) return CUHPX_EINVAL;
-    if (!d_in || !d_out || d_in == d_out || ((uintptr_t)d_in & 15) || ((uintptr_t)d_out & 15)) return CUHPX_EINVAL;
+    if (!d_in || !d_out || ((uintptr_t)d_in & 15) || ((uintptr_t)d_out & 15)) return CUHPX_EINVAL;
+    const size_t nb = (size_t)batch * 12 * nside * nside * (dt == CUHPX_F64 ? 8 : 4);
+    if (overlap(d_in, nb, d_out, nb)) return CUHPX_EINVAL;
     CUDA_OR_FAIL(launch_reorder(nside, batch, dt, direction == CUHPX_NEST2RING, d_in, d_out, (cudaStream_t)stream));
     return CUHPX_OK;
 }
@@ -514,8 +575,11 @@ int cuhpx_reorder(int nside, int batch, cuhpx_dtype_t dt, int direction, const v
 int cuhpx_alm_resize(int lmax_in, int mmax_in, int lmax_out, int mmax_out, int batch, cuhpx_dtype_t dt,
                      const void* d_in, void* d_out, cuhpx_stream_t stream) {
     if (lmax_in < 0 || mmax_in < 0 || mmax_in > lmax_in || lmax_out < 0 || mmax_out < 0 || mmax_out > lmax_out) return CUHPX_EINVAL;
-    if (batch < 1 || (dt != CUHPX_F32 && dt != CUHPX_F64)) return CUHPX_EINVAL;
-    if (!d_in || !d_out || d_in == d_out || ((uintptr_t)d_in & 15) || ((uintptr_t)d_out & 15)) return CUHPX_EINVAL;
+    if (batch < 1 || batch > MAX_BATCH || (dt != CUHPX_F32 && dt != CUHPX_F64)) return CUHPX_EINVAL;
+    if (!d_in || !d_out || ((uintptr_t)d_in & 15) || ((uintptr_t)d_out & 15)) return CUHPX_EINVAL;
+    const size_t cs = dt == CUHPX_F64 ? 16 : 8;
+    if (overlap(d_in, batch * cuhpx_alm_count(lmax_in, mmax_in) * cs, d_out, batch * cuhpx_alm_count(lmax_out, mmax_out) * cs))
+        return CUHPX_EINVAL;
     CUDA_OR_FAIL(launch_alm_resize(lmax_in, mmax_in, lmax_out, mmax_out, batch, dt, d_in, d_out, (cudaStream_t)stream));
     return CUHPX_OK;
 }

@@ -17,6 +17,8 @@
 #include <string.h>
 
 #include <algorithm>
+#include <mutex>
+#include <vector>
 
 #include "block_fft.cuh"
 #include "cuhpx_internal.h"
@@ -111,6 +113,7 @@ template <typename T>
 __global__ void __launch_bounds__(FFT_THREADS) ring_direct_analysis_kernel(DevPlan P, const RingInfo* __restrict__ info,
                                                                           const T* __restrict__ map,
                                                                           const double* __restrict__ w, int use_w) {
+    if (!ws_ok(P)) return;
     using T2 = typename V2<T>::type;
     extern __shared__ __align__(16) unsigned char smem_raw[];
     const int ch = blockIdx.y;
@@ -152,6 +155,7 @@ template <typename T>
 __global__ void __launch_bounds__(FFT_THREADS) ring_direct_synthesis_kernel(DevPlan P, const RingInfo* __restrict__ info,
                                                                            T* __restrict__ map,
                                                                            const double* __restrict__ w, int use_w) {
+    if (!ws_ok(P)) return;
     using T2 = typename V2<T>::type;
     extern __shared__ __align__(16) unsigned char smem_raw[];
     const int ch = blockIdx.y;
@@ -204,6 +208,7 @@ template <typename T, int CB>
 __global__ void __launch_bounds__(DIRECT_CB_THREADS) ring_direct_analysis_cb_kernel(DevPlan P, const RingInfo* __restrict__ info,
                                                                                    const T* __restrict__ map,
                                                                                    const double* __restrict__ w, int use_w) {
+    if (!ws_ok(P)) return;
     using T2 = typename V2<T>::type;
     extern __shared__ __align__(16) unsigned char smem_raw[];
     const int ch0 = blockIdx.y * CB;
@@ -269,6 +274,7 @@ template <typename T, int CB>
 __global__ void __launch_bounds__(DIRECT_CB_THREADS) ring_direct_synthesis_cb_kernel(DevPlan P, const RingInfo* __restrict__ info,
                                                                                     T* __restrict__ map,
                                                                                     const double* __restrict__ w, int use_w) {
+    if (!ws_ok(P)) return;
     using T2 = typename V2<T>::type;
     extern __shared__ __align__(16) unsigned char smem_raw[];
     const int ch0 = blockIdx.y * CB;
@@ -461,6 +467,7 @@ __global__ void __launch_bounds__(FftPlan<LOGN>::NT, MinBlocks<T, LOGN>::value) 
                                                                                const T* __restrict__ map,
                                                                                const double* __restrict__ w, int use_w,
                                                                                FftTables tabs) {
+    if (!ws_ok(P)) return;
     using F = BlockFFT<T, LOGN, LOGN + 2>;
     using T2 = typename V2<T>::type;
     constexpr int n = F::N, N = 2 * n, Q = 2 * N, E = F::E, NT = F::NT;
@@ -503,6 +510,7 @@ __global__ void __launch_bounds__(FftPlan<LOGN>::NT, MinBlocks<T, LOGN>::value) 
                                                                                 T* __restrict__ map,
                                                                                 const double* __restrict__ w, int use_w,
                                                                                 FftTables tabs) {
+    if (!ws_ok(P)) return;
     using F = BlockFFT<T, LOGN, LOGN + 2>;
     using T2 = typename V2<T>::type;
     constexpr int n = F::N, N = 2 * n, Q = 2 * N, E = F::E, NT = F::NT;
@@ -582,6 +590,7 @@ __global__ void __launch_bounds__(FftPlan<LOGM>::NT, MinBlocks<T, LOGM>::blue) r
                                                                                const T* __restrict__ map,
                                                                                const double* __restrict__ w, int use_w,
                                                                                FftTables tabs) {
+    if (!ws_ok(P)) return;
     using F = BlockFFT<T, LOGM>;
     using T2 = typename V2<T>::type;
     using SM = BlueSmem<T, LOGM>;
@@ -710,6 +719,7 @@ __global__ void __launch_bounds__(FftPlan<LOGM>::NT, MinBlocks<T, LOGM>::blue) r
                                                                                 T* __restrict__ map,
                                                                                 const double* __restrict__ w, int use_w,
                                                                                 FftTables tabs) {
+    if (!ws_ok(P)) return;
     using F = BlockFFT<T, LOGM>;
     using T2 = typename V2<T>::type;
     using SM = BlueSmem<T, LOGM>;
@@ -864,7 +874,7 @@ __global__ void twiddle_table_kernel(typename V2<T>::type* tw, int twlen) {
     }
 }
 
-// ------------------------------------------------------------------ planning
+// ------------------------------------------------------------------ planning (host only: a pure function of the call parameters)
 static int blue_logm(int i) {  // M = 2^LOGM >= 2 i - 1, at least 2^MIN_LOG
     int l = ilog2_ceil(2LL * i - 1);
     return l < MIN_LOG ? MIN_LOG : l;
@@ -878,103 +888,113 @@ template <int LOG> static size_t filter_smem_bytes() {
     return Xchg<double>::bytes(1 << LOG) + sizeof(double2) * (size_t)roots_len(1 << LOG);
 }
 
-bool fft_supported(int nside, cuhpx_dtype_t dt) {
+bool fft_supported(int max_ring_pixels, cuhpx_dtype_t dt) {
     (void)dt;
-    return nside <= 4096;  // belt: n = 2 nside <= 2^13; caps: M <= 2^13 (fp64 needs 209 KB of the SM's 227 KB)
+    return max_ring_pixels <= 16384;  // belt: n = N / 2 <= 2^13; caps: M <= 2^13 (fp64 needs 209 KB of the SM's 227 KB)
 }
 
-struct RingFftLists {
+// Host part of the FFT-stage plan: ring classes and the layout of the tables inside the workspace (offsets relative to
+// the FFT region, HostPlan::off_fft):
+//   [work items: direct | pow2[7..13] | blue[7..13]] [blue_i[7..13]] [filt_offset: nside x i64]
+//   [twiddle T2[twlen]] [twiddle double2[twlen] (set-up only, kept)] [filters]
+struct FftHost {
     std::vector<RingInfo> direct;
     std::vector<RingInfo> pow2[MAX_LOG + 1];
     std::vector<RingInfo> blue[MAX_LOG + 1];
     std::vector<int> blue_i[MAX_LOG + 1];  // distinct i per LOGM
+    std::vector<long long> filt_off;       // [nside] offset (complex units) of the filter of cap ring i, -1 if none
+    size_t off_direct, off_pow2[MAX_LOG + 1], off_blue[MAX_LOG + 1], off_blue_i[MAX_LOG + 1];
+    size_t off_filt_offset, off_tw, off_tw64, off_filt, total;
+    long long filt_total;
+    int twlen;
+    int max_mcut_direct;
+    int side_from;  // Bluestein classes with LOG <= side_from go to the side stream (with the direct kernel)
 };
+void free_fft_host(FftHost* f) { delete f; }
 
-static void classify(const HostPlan& hp, RingFftLists& L) {
+size_t fft_plan_host(HostPlan& hp) {
     const DevPlan& d = hp.d;
+    FftHost* F = new FftHost;
+    free_fft_host(hp.fft);
+    hp.fft = F;
     for (int r = 0; r < d.nrings; ++r) {
         const int j = std::min(r, d.nrings - 1 - r);
         RingInfo R;
         R.N = hp.h_ringN[j];
         R.start = (r > j) ? d.npix - R.N - hp.h_start[j] : hp.h_start[j];
-        R.mcut = hp.h_mcut.empty() ? 0 : hp.h_mcut[j];  // sizing pass: cut-offs not computed yet
+        R.mcut = hp.h_mcut[j];
         R.shifted = hp.h_shifted[j];
         R.r = r;
         R.pad0 = R.pad1 = 0;
         const int N = R.N;
-        if (N == 4 * d.nside && ilog2_ceil(N) - 1 >= MIN_LOG) L.pow2[ilog2_ceil(N) - 1].push_back(R);  // belt rings (N = 4 nside = 2^k)
-        else if (N <= DIRECT_MAX_N) L.direct.push_back(R);
+        if (N == 4 * d.nside && ilog2_ceil(N) - 1 >= MIN_LOG) F->pow2[ilog2_ceil(N) - 1].push_back(R);  // belt rings (N = 4 nside = 2^k)
+        else if (N <= DIRECT_MAX_N) F->direct.push_back(R);
         else {  // cap rings, chirp-z for every i (the few i = 2^k among them are not worth launches of their own)
             const int i = N / 4, lm = blue_logm(i);
-            L.blue[lm].push_back(R);
-            if (r == j) L.blue_i[lm].push_back(i);
+            F->blue[lm].push_back(R);
+            if (r == j) F->blue_i[lm].push_back(i);
         }
     }
     // longest rings first inside a class: the tail of a launch is then made of its cheapest items
     for (int l = MIN_LOG; l <= MAX_LOG; ++l)
-        std::stable_sort(L.blue[l].begin(), L.blue[l].end(), [](const RingInfo& a, const RingInfo& b) { return a.N > b.N; });
-}
+        std::stable_sort(F->blue[l].begin(), F->blue[l].end(), [](const RingInfo& a, const RingInfo& b) { return a.N > b.N; });
 
-// Device layout of the FFT tables inside the workspace (all offsets relative to `base`):
-//   [work items: direct | pow2[8..13] | blue[8..13]] [blue_i[8..13]] [filt_offset: nside x i64]
-//   [twiddle T2[twlen]] [twiddle double2[twlen] (set-up only, kept)] [filters]
-struct FftLayout {
-    size_t off_direct, off_pow2[MAX_LOG + 1], off_blue[MAX_LOG + 1], off_blue_i[MAX_LOG + 1];
-    size_t off_filt_offset, off_tw, off_tw64, off_filt, total;
-    long long filt_total;
-};
-
-static FftLayout fft_layout(const HostPlan& hp, const RingFftLists& L, std::vector<long long>& filt_off) {
-    const DevPlan& d = hp.d;
     const size_t csize = hp.dtype == CUHPX_F64 ? 16 : 8;
-    FftLayout Y;
     size_t o = 0;
     auto take = [&](size_t bytes) {
         size_t r = o;
         o = (o + bytes + 255) / 256 * 256;
         return r;
     };
-    Y.off_direct = take(sizeof(RingInfo) * L.direct.size());
+    F->off_direct = take(sizeof(RingInfo) * F->direct.size());
+    for (int l = 0; l <= MAX_LOG; ++l) F->off_pow2[l] = F->off_blue[l] = F->off_blue_i[l] = 0;
     for (int l = MIN_LOG; l <= MAX_LOG; ++l) {
-        Y.off_pow2[l] = take(sizeof(RingInfo) * L.pow2[l].size());
-        Y.off_blue[l] = take(sizeof(RingInfo) * L.blue[l].size());
-        Y.off_blue_i[l] = take(sizeof(int) * L.blue_i[l].size());
+        F->off_pow2[l] = take(sizeof(RingInfo) * F->pow2[l].size());
+        F->off_blue[l] = take(sizeof(RingInfo) * F->blue[l].size());
+        F->off_blue_i[l] = take(sizeof(int) * F->blue_i[l].size());
     }
-    Y.off_filt_offset = take(sizeof(long long) * d.nside);
-    const int twlen = 8 * d.nside < 2048 ? 2048 : 8 * d.nside;
-    Y.off_tw = take(csize * twlen);
-    Y.off_tw64 = take(16 * (size_t)twlen);
-    filt_off.assign(d.nside, -1);
+    F->off_filt_offset = take(sizeof(long long) * d.nside);
+    F->twlen = 8 * d.nside < 2048 ? 2048 : 8 * d.nside;
+    F->off_tw = take(csize * F->twlen);
+    F->off_tw64 = take(16 * (size_t)F->twlen);
+    F->filt_off.assign(d.nside, -1);
     long long fo = 0;
     for (int l = MIN_LOG; l <= MAX_LOG; ++l)
-        for (int i : L.blue_i[l]) {
-            filt_off[i] = fo;
+        for (int i : F->blue_i[l]) {
+            F->filt_off[i] = fo;
             fo += 1LL << l;
         }
-    Y.filt_total = fo;
-    Y.off_filt = take(csize * (size_t)fo);
-    Y.total = o;
-    return Y;
+    F->filt_total = fo;
+    F->off_filt = take(csize * (size_t)fo);
+    F->total = o;
+    F->max_mcut_direct = 0;
+    for (const RingInfo& R : F->direct) F->max_mcut_direct = std::max(F->max_mcut_direct, R.mcut);
+    int lmax_blue = -1;
+    for (int l = MIN_LOG; l <= MAX_LOG; ++l)
+        if (!F->blue[l].empty()) lmax_blue = l;
+    F->side_from = lmax_blue - 2;
+    return F->total;
 }
 
-struct FftDev {  // device pointers resolved from the layout (kept per plan in a side table)
-    const RingInfo* direct;
-    const RingInfo* pow2[MAX_LOG + 1];
-    const RingInfo* blue[MAX_LOG + 1];
-    int n_direct, n_pow2[MAX_LOG + 1], n_blue[MAX_LOG + 1];
-    // prefetch distance per launch: CTAs resident on the whole GPU, [analysis 0 / synthesis 1][pow2 0 / blue 1][LOG]
-    int pf[2][2][MAX_LOG + 1];
-    int max_mcut_direct;
-    FftTables tabs;
-    // The short-ring classes run on a side stream beside the long-ring kernels (fork / join with events), so
-    // their launch latencies and partial waves hide under the kernels that carry the bytes.
-    cudaStream_t side;
-    cudaEvent_t ev_fork, ev_join;
-    int side_from;  // Bluestein classes with LOG <= side_from go to the side stream (with the direct kernel)
+// ------------------------------------------------------------------ per-device lazily created launch resources
+// Kernel attributes (dynamic shared memory), L2-prefetch distances (CTAs resident on the whole GPU) and the side
+// stream on which the short-ring classes run beside the long-ring kernels (fork / join with events, so their launch
+// latencies and partial waves hide under the kernels that carry the bytes).  None of it belongs to a workspace.
+struct DevRes {
+    bool ready = false;
+    cudaError_t err = cudaSuccess;
+    // [dtype f32 0 / f64 1][analysis 0 / synthesis 1][pow2 0 / blue 1][LOG]
+    int pf[2][2][2][MAX_LOG + 1];
+    cudaStream_t side = nullptr;
+    cudaEvent_t ev_fork = nullptr, ev_join = nullptr;
+    std::mutex mu;  // the (record, wait) pairs on the shared events must not interleave between host threads
 };
+static DevRes g_dev[64];
+static std::mutex g_dev_mu;
 
-template <typename T, int LOG> static cudaError_t set_smem_attrs(FftDev& D, int sms) {
+template <typename T, int LOG> static cudaError_t set_smem_attrs(DevRes& D, int sms) {
     cudaError_t e;
+    constexpr int TI = sizeof(T) == 8 ? 1 : 0;
     const size_t sp = fft_smem_bytes<T, LOG>(false), sb = fft_smem_bytes<T, LOG>(true);
     if ((e = cudaFuncSetAttribute(ring_pow2_analysis_kernel<T, LOG>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sp))) return e;
     if ((e = cudaFuncSetAttribute(ring_pow2_synthesis_kernel<T, LOG>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sp))) return e;
@@ -985,221 +1005,222 @@ template <typename T, int LOG> static cudaError_t set_smem_attrs(FftDev& D, int 
     int occ = 0;
     constexpr int NT = FftPlan<LOG>::NT;
     if ((e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, ring_pow2_analysis_kernel<T, LOG>, NT, sp))) return e;
-    D.pf[0][0][LOG] = occ * sms;
+    D.pf[TI][0][0][LOG] = occ * sms;
     if ((e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, ring_pow2_synthesis_kernel<T, LOG>, NT, sp))) return e;
-    D.pf[1][0][LOG] = occ * sms;
+    D.pf[TI][1][0][LOG] = occ * sms;
     if ((e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, ring_blue_analysis_kernel<T, LOG>, NT, sb))) return e;
-    D.pf[0][1][LOG] = occ * sms;
+    D.pf[TI][0][1][LOG] = occ * sms;
     if ((e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, ring_blue_synthesis_kernel<T, LOG>, NT, sb))) return e;
-    D.pf[1][1][LOG] = occ * sms;
+    D.pf[TI][1][1][LOG] = occ * sms;
     return cudaSuccess;
 }
 
-template <typename T, int LOG>
-static cudaError_t build_filters(const RingFftLists& L, const FftLayout& Y, char* base, cudaStream_t st, int twlen) {
-    if (L.blue_i[LOG].empty()) return cudaSuccess;
-    using T2 = typename V2<T>::type;
-    blue_filter_kernel<T, LOG><<<(unsigned)L.blue_i[LOG].size(), FftPlan<LOG>::NT, filter_smem_bytes<LOG>(), st>>>(
-        (const int*)(base + Y.off_blue_i[LOG]), (const long long*)(base + Y.off_filt_offset), (T2*)(base + Y.off_filt),
-        (const double2*)(base + Y.off_tw64), twlen);
-    return cudaGetLastError();
-}
-
-template <typename T> static cudaError_t build_tables_t(FftDev& D, const RingFftLists& L, const FftLayout& Y, char* base,
-                                                        cudaStream_t st, int twlen) {
-    using T2 = typename V2<T>::type;
+template <typename T> static cudaError_t set_all_attrs(DevRes& D, int sms) {
     cudaError_t e;
-    int dev = 0, sms = 0;
-    if ((e = cudaGetDevice(&dev)) != cudaSuccess) return e;
-    if ((e = cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev)) != cudaSuccess) return e;
 #define CUHPX_ATTR(LOG) if ((e = set_smem_attrs<T, LOG>(D, sms)) != cudaSuccess) return e;
     CUHPX_ATTR(7) CUHPX_ATTR(8) CUHPX_ATTR(9) CUHPX_ATTR(10) CUHPX_ATTR(11) CUHPX_ATTR(12) CUHPX_ATTR(13)
 #undef CUHPX_ATTR
-    twiddle_table_kernel<T><<<(twlen + 255) / 256, 256, 0, st>>>((T2*)(base + Y.off_tw), twlen);
-    twiddle_table_kernel<double><<<(twlen + 255) / 256, 256, 0, st>>>((double2*)(base + Y.off_tw64), twlen);
+    // direct synthesis kernel: [twiddles N][G: mcut + 1]; the largest the SM can hold (launches check their own need)
+    return cudaFuncSetAttribute(ring_direct_synthesis_kernel<T>, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024);
+}
+
+static DevRes* dev_res(cudaError_t* err) {
+    int dev = 0;
+    if ((*err = cudaGetDevice(&dev)) != cudaSuccess) return nullptr;
+    if (dev < 0 || dev >= 64) {
+        *err = cudaErrorInvalidDevice;
+        return nullptr;
+    }
+    DevRes& D = g_dev[dev];
+    std::lock_guard<std::mutex> lk(g_dev_mu);
+    if (!D.ready) {
+        int sms = 0;
+        cudaError_t e = cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+        memset(D.pf, 0, sizeof(D.pf));
+        if (e == cudaSuccess) e = set_all_attrs<float>(D, sms);
+        if (e == cudaSuccess) e = set_all_attrs<double>(D, sms);
+        if (e == cudaSuccess) e = cudaStreamCreateWithFlags(&D.side, cudaStreamNonBlocking);
+        if (e == cudaSuccess) e = cudaEventCreateWithFlags(&D.ev_fork, cudaEventDisableTiming);
+        if (e == cudaSuccess) e = cudaEventCreateWithFlags(&D.ev_join, cudaEventDisableTiming);
+        D.err = e;
+        D.ready = true;
+    }
+    *err = D.err;
+    return D.err == cudaSuccess ? &D : nullptr;
+}
+
+// ------------------------------------------------------------------ table building (cuhpx_workspace_init)
+template <typename T, int LOG>
+static cudaError_t build_filters(const FftHost& F, char* base, cudaStream_t st) {
+    if (F.blue_i[LOG].empty()) return cudaSuccess;
+    using T2 = typename V2<T>::type;
+    blue_filter_kernel<T, LOG><<<(unsigned)F.blue_i[LOG].size(), FftPlan<LOG>::NT, filter_smem_bytes<LOG>(), st>>>(
+        (const int*)(base + F.off_blue_i[LOG]), (const long long*)(base + F.off_filt_offset), (T2*)(base + F.off_filt),
+        (const double2*)(base + F.off_tw64), F.twlen);
+    return cudaGetLastError();
+}
+
+template <typename T> static cudaError_t build_tables_t(const FftHost& F, char* base, cudaStream_t st) {
+    using T2 = typename V2<T>::type;
+    cudaError_t e;
+    twiddle_table_kernel<T><<<(F.twlen + 255) / 256, 256, 0, st>>>((T2*)(base + F.off_tw), F.twlen);
+    twiddle_table_kernel<double><<<(F.twlen + 255) / 256, 256, 0, st>>>((double2*)(base + F.off_tw64), F.twlen);
     if ((e = cudaGetLastError()) != cudaSuccess) return e;
-#define CUHPX_FILT(LOG) if ((e = build_filters<T, LOG>(L, Y, base, st, twlen)) != cudaSuccess) return e;
+#define CUHPX_FILT(LOG) if ((e = build_filters<T, LOG>(F, base, st)) != cudaSuccess) return e;
     CUHPX_FILT(7) CUHPX_FILT(8) CUHPX_FILT(9) CUHPX_FILT(10) CUHPX_FILT(11) CUHPX_FILT(12) CUHPX_FILT(13)
 #undef CUHPX_FILT
     return cudaSuccess;
 }
 
-size_t plan_fft_tables(HostPlan& hp, char* base, bool build, cudaStream_t st, cudaError_t* err) {
-    RingFftLists L;
-    classify(hp, L);
-    std::vector<long long> filt_off;
-    const FftLayout Y = fft_layout(hp, L, filt_off);
-    if (!build) return Y.total;
-    const DevPlan& d = hp.d;
-    const int twlen = 8 * d.nside < 2048 ? 2048 : 8 * d.nside;
+cudaError_t fft_build_tables(const HostPlan& hp, char* base, cudaStream_t st) {
+    if (!hp.fft) return cudaErrorInvalidValue;
+    const FftHost& F = *hp.fft;
     cudaError_t e = cudaSuccess;
+    if (!dev_res(&e)) return e;  // kernel attributes of this device are in place before the first (possibly captured) call
+    const size_t csz = hp.dtype == CUHPX_F64 ? 16 : 8;
+    if ((DIRECT_MAX_N + F.max_mcut_direct + 1) * csz > 200 * 1024) return cudaErrorInvalidConfiguration;
     auto up = [&](size_t off, const void* src, size_t bytes) {
         if (e == cudaSuccess && bytes) e = cudaMemcpyAsync(base + off, src, bytes, cudaMemcpyHostToDevice, st);
     };
-    up(Y.off_direct, L.direct.data(), sizeof(RingInfo) * L.direct.size());
+    up(F.off_direct, F.direct.data(), sizeof(RingInfo) * F.direct.size());
     for (int l = MIN_LOG; l <= MAX_LOG; ++l) {
-        up(Y.off_pow2[l], L.pow2[l].data(), sizeof(RingInfo) * L.pow2[l].size());
-        up(Y.off_blue[l], L.blue[l].data(), sizeof(RingInfo) * L.blue[l].size());
-        up(Y.off_blue_i[l], L.blue_i[l].data(), sizeof(int) * L.blue_i[l].size());
+        up(F.off_pow2[l], F.pow2[l].data(), sizeof(RingInfo) * F.pow2[l].size());
+        up(F.off_blue[l], F.blue[l].data(), sizeof(RingInfo) * F.blue[l].size());
+        up(F.off_blue_i[l], F.blue_i[l].data(), sizeof(int) * F.blue_i[l].size());
     }
-    up(Y.off_filt_offset, filt_off.data(), sizeof(long long) * d.nside);
-    if (e == cudaSuccess) e = cudaStreamSynchronize(st);  // pageable sources
-    FftDev D;
-    memset(&D, 0, sizeof(D));
-    if (e == cudaSuccess)
-        e = hp.dtype == CUHPX_F64 ? build_tables_t<double>(D, L, Y, base, st, twlen)
-                                  : build_tables_t<float>(D, L, Y, base, st, twlen);
-    D.direct = (const RingInfo*)(base + Y.off_direct);
-    D.n_direct = (int)L.direct.size();
-    for (int l = 0; l <= MAX_LOG; ++l) {
-        D.pow2[l] = l >= MIN_LOG ? (const RingInfo*)(base + Y.off_pow2[l]) : nullptr;
-        D.blue[l] = l >= MIN_LOG ? (const RingInfo*)(base + Y.off_blue[l]) : nullptr;
-        D.n_pow2[l] = l >= MIN_LOG ? (int)L.pow2[l].size() : 0;
-        D.n_blue[l] = l >= MIN_LOG ? (int)L.blue[l].size() : 0;
-    }
-    D.tabs.tw = base + Y.off_tw;
-    D.tabs.twlen = twlen;
-    D.tabs.filt = base + Y.off_filt;
-    D.tabs.filt_offset = (const long long*)(base + Y.off_filt_offset);
-    D.tabs.pf = 0;
-    D.max_mcut_direct = 0;
-    for (const RingInfo& R : L.direct) D.max_mcut_direct = std::max(D.max_mcut_direct, R.mcut);
-    const size_t csz = hp.dtype == CUHPX_F64 ? 16 : 8;
-    if (e == cudaSuccess && (DIRECT_MAX_N + D.max_mcut_direct + 1) * csz > 200 * 1024) e = cudaErrorInvalidConfiguration;
-    if (e == cudaSuccess) {
-        const int want = (int)((DIRECT_MAX_N + D.max_mcut_direct + 1) * csz);
-        e = hp.dtype == CUHPX_F64
-                ? cudaFuncSetAttribute(ring_direct_synthesis_kernel<double>, cudaFuncAttributeMaxDynamicSharedMemorySize, std::max(want, 48 * 1024))
-                : cudaFuncSetAttribute(ring_direct_synthesis_kernel<float>, cudaFuncAttributeMaxDynamicSharedMemorySize, std::max(want, 48 * 1024));
-    }
-    D.side_from = -1;
-    {
-        int lmax_blue = -1;
-        for (int l = MIN_LOG; l <= MAX_LOG; ++l)
-            if (D.n_blue[l]) lmax_blue = l;
-        D.side_from = lmax_blue - 2;
-    }
-    if (e == cudaSuccess) e = cudaStreamCreateWithFlags(&D.side, cudaStreamNonBlocking);
-    if (e == cudaSuccess) e = cudaEventCreateWithFlags(&D.ev_fork, cudaEventDisableTiming);
-    if (e == cudaSuccess) e = cudaEventCreateWithFlags(&D.ev_join, cudaEventDisableTiming);
-    free_fft_dev(hp.fft);
-    hp.fft = new FftDev(D);
-    hp.rings_direct.clear();
-    for (const RingInfo& R : L.direct) hp.rings_direct.push_back(R.r);
-    *err = e;
-    return Y.total;
-}
-
-void free_fft_dev(FftDev* f) {
-    if (!f) return;
-    if (f->ev_fork) cudaEventDestroy(f->ev_fork);
-    if (f->ev_join) cudaEventDestroy(f->ev_join);
-    if (f->side) cudaStreamDestroy(f->side);
-    delete f;
+    up(F.off_filt_offset, F.filt_off.data(), sizeof(long long) * hp.d.nside);
+    if (e != cudaSuccess) return e;
+    return hp.dtype == CUHPX_F64 ? build_tables_t<double>(F, base, st) : build_tables_t<float>(F, base, st);
 }
 
 void fft_stage_stats(const HostPlan& hp, int* launches, double* table_bytes) {
     *launches = 0;
     *table_bytes = 0;
     if (!hp.fft) return;
-    const FftDev& D = *hp.fft;
+    const FftHost& F = *hp.fft;
     const double csz = hp.dtype == CUHPX_F64 ? 16 : 8;
-    if (D.n_direct) ++*launches;
+    if (!F.direct.empty()) ++*launches;
     for (int l = MIN_LOG; l <= MAX_LOG; ++l) {
-        if (D.n_pow2[l]) ++*launches;
-        if (D.n_blue[l]) {
+        if (!F.pow2[l].empty()) ++*launches;
+        if (!F.blue[l].empty()) {
             ++*launches;
-            *table_bytes += 0.5 * D.n_blue[l] * (double)(1 << l) * csz;  // one filter per ring size i, shared N/S
+            *table_bytes += 0.5 * F.blue[l].size() * (double)(1 << l) * csz;  // one filter per ring size i, shared N/S
         }
     }
-    *table_bytes += D.tabs.twlen * csz;
+    *table_bytes += F.twlen * csz;
 }
 
 // ------------------------------------------------------------------ launchers
+struct FftCall {  // what one stage call resolves from (plan, workspace, device)
+    const FftHost* F;
+    const char* base;  // FFT region of the workspace
+    const DevRes* D;
+    FftTables tabs;
+    int ti;  // 0 fp32, 1 fp64
+};
+
 // Bluestein classes LOG <= side_from and the direct kernel go to the side stream
 template <typename T, bool ANALYSIS, int LOG>
-static void launch_class(const DevPlan& P, const FftDev& D, T* map, const double* w, int use_w, cudaStream_t main_st,
+static void launch_class(const DevPlan& P, const FftCall& C, T* map, const double* w, int use_w, cudaStream_t main_st,
                          cudaStream_t side_st) {
-    FftTables tabs = D.tabs;
+    const FftHost& F = *C.F;
+    FftTables tabs = C.tabs;
     constexpr int A = ANALYSIS ? 0 : 1;
-    if (D.n_pow2[LOG]) {
-        tabs.pf = D.pf[A][0][LOG];
+    if (!F.pow2[LOG].empty()) {
+        tabs.pf = C.D->pf[C.ti][A][0][LOG];
+        const RingInfo* items = (const RingInfo*)(C.base + F.off_pow2[LOG]);
+        const dim3 grid((unsigned)F.pow2[LOG].size(), P.batch);
         if (ANALYSIS)
-            ring_pow2_analysis_kernel<T, LOG><<<dim3(D.n_pow2[LOG], P.batch), FftPlan<LOG>::NT, fft_smem_bytes<T, LOG>(false), main_st>>>(
-                P, D.pow2[LOG], map, w, use_w, tabs);
+            ring_pow2_analysis_kernel<T, LOG><<<grid, FftPlan<LOG>::NT, fft_smem_bytes<T, LOG>(false), main_st>>>(P, items, map, w, use_w, tabs);
         else
-            ring_pow2_synthesis_kernel<T, LOG><<<dim3(D.n_pow2[LOG], P.batch), FftPlan<LOG>::NT, fft_smem_bytes<T, LOG>(false), main_st>>>(
-                P, D.pow2[LOG], map, w, use_w, tabs);
+            ring_pow2_synthesis_kernel<T, LOG><<<grid, FftPlan<LOG>::NT, fft_smem_bytes<T, LOG>(false), main_st>>>(P, items, map, w, use_w, tabs);
     }
-    if (D.n_blue[LOG]) {
-        tabs.pf = D.pf[A][1][LOG];
-        cudaStream_t st = LOG <= D.side_from ? side_st : main_st;
+    if (!F.blue[LOG].empty()) {
+        tabs.pf = C.D->pf[C.ti][A][1][LOG];
+        cudaStream_t st = LOG <= F.side_from ? side_st : main_st;
+        const RingInfo* items = (const RingInfo*)(C.base + F.off_blue[LOG]);
+        const dim3 grid((unsigned)F.blue[LOG].size(), P.batch);
         if (ANALYSIS)
-            ring_blue_analysis_kernel<T, LOG><<<dim3(D.n_blue[LOG], P.batch), FftPlan<LOG>::NT, fft_smem_bytes<T, LOG>(true), st>>>(
-                P, D.blue[LOG], map, w, use_w, tabs);
+            ring_blue_analysis_kernel<T, LOG><<<grid, FftPlan<LOG>::NT, fft_smem_bytes<T, LOG>(true), st>>>(P, items, map, w, use_w, tabs);
         else
-            ring_blue_synthesis_kernel<T, LOG><<<dim3(D.n_blue[LOG], P.batch), FftPlan<LOG>::NT, fft_smem_bytes<T, LOG>(true), st>>>(
-                P, D.blue[LOG], map, w, use_w, tabs);
+            ring_blue_synthesis_kernel<T, LOG><<<grid, FftPlan<LOG>::NT, fft_smem_bytes<T, LOG>(true), st>>>(P, items, map, w, use_w, tabs);
     }
 }
 
 template <typename T, bool ANALYSIS>
-static cudaError_t run_fft_stage(const HostPlan& hp, T* map, const double* d_w, int use_w, cudaStream_t st) {
-    const DevPlan& P = hp.d;
+static cudaError_t run_fft_stage(const HostPlan& hp, const DevPlan& P, T* map, const double* d_w, int use_w, cudaStream_t st) {
     if (!hp.fft) return cudaErrorInvalidValue;
-    const FftDev& D = *hp.fft;
-    bool side_work = D.n_direct > 0, main_work = false;
+    cudaError_t e = cudaSuccess;
+    DevRes* D = dev_res(&e);
+    if (!D) return e;
+    const FftHost& F = *hp.fft;
+    FftCall C;
+    C.F = &F;
+    C.base = reinterpret_cast<const char*>(P.hdr) + hp.off_fft;
+    C.D = D;
+    C.ti = sizeof(T) == 8 ? 1 : 0;
+    C.tabs.tw = C.base + F.off_tw;
+    C.tabs.twlen = F.twlen;
+    C.tabs.filt = C.base + F.off_filt;
+    C.tabs.filt_offset = (const long long*)(C.base + F.off_filt_offset);
+    C.tabs.pf = 0;
+    bool side_work = !F.direct.empty(), main_work = false;
     for (int l = MIN_LOG; l <= MAX_LOG; ++l) {
-        if (D.n_blue[l] && l <= D.side_from) side_work = true;
-        if (D.n_pow2[l] || (D.n_blue[l] && l > D.side_from)) main_work = true;
+        if (!F.blue[l].empty() && l <= F.side_from) side_work = true;
+        if (!F.pow2[l].empty() || (!F.blue[l].empty() && l > F.side_from)) main_work = true;
     }
     const bool fork = side_work && main_work;
-    cudaStream_t side = fork ? D.side : st;
-    cudaError_t e;
+    cudaStream_t side = fork ? D->side : st;
+    std::unique_lock<std::mutex> lk(D->mu, std::defer_lock);
     if (fork) {
-        if ((e = cudaEventRecord(D.ev_fork, st)) != cudaSuccess) return e;
-        if ((e = cudaStreamWaitEvent(side, D.ev_fork, 0)) != cudaSuccess) return e;
+        lk.lock();
+        if ((e = cudaEventRecord(D->ev_fork, st)) != cudaSuccess) return e;
+        if ((e = cudaStreamWaitEvent(side, D->ev_fork, 0)) != cudaSuccess) return e;
     }
     // largest rings first: they dominate the run time
-    launch_class<T, ANALYSIS, 13>(P, D, map, d_w, use_w, st, side);
-    launch_class<T, ANALYSIS, 12>(P, D, map, d_w, use_w, st, side);
-    launch_class<T, ANALYSIS, 11>(P, D, map, d_w, use_w, st, side);
-    launch_class<T, ANALYSIS, 10>(P, D, map, d_w, use_w, st, side);
-    launch_class<T, ANALYSIS, 9>(P, D, map, d_w, use_w, st, side);
-    launch_class<T, ANALYSIS, 8>(P, D, map, d_w, use_w, st, side);
-    launch_class<T, ANALYSIS, 7>(P, D, map, d_w, use_w, st, side);
-    if (D.n_direct) {
+    launch_class<T, ANALYSIS, 13>(P, C, map, d_w, use_w, st, side);
+    launch_class<T, ANALYSIS, 12>(P, C, map, d_w, use_w, st, side);
+    launch_class<T, ANALYSIS, 11>(P, C, map, d_w, use_w, st, side);
+    launch_class<T, ANALYSIS, 10>(P, C, map, d_w, use_w, st, side);
+    launch_class<T, ANALYSIS, 9>(P, C, map, d_w, use_w, st, side);
+    launch_class<T, ANALYSIS, 8>(P, C, map, d_w, use_w, st, side);
+    launch_class<T, ANALYSIS, 7>(P, C, map, d_w, use_w, st, side);
+    if (!F.direct.empty()) {
         constexpr int CB = 8;
+        const RingInfo* items = (const RingInfo*)(C.base + F.off_direct);
+        const unsigned nd = (unsigned)F.direct.size();
         const size_t cb_ana = (size_t)DIRECT_MAX_N * (2 + CB) * sizeof(T);
-        const size_t cb_syn = ((size_t)DIRECT_MAX_N + (size_t)(D.max_mcut_direct + 1) * CB) * 2 * sizeof(T);
+        const size_t cb_syn = ((size_t)DIRECT_MAX_N + (size_t)(F.max_mcut_direct + 1) * CB) * 2 * sizeof(T);
         if (P.batch >= 4 && cb_syn <= 48 * 1024) {  // channel-blocked direct sums
-            const dim3 grid(D.n_direct, (P.batch + CB - 1) / CB);
-            if (ANALYSIS) ring_direct_analysis_cb_kernel<T, CB><<<grid, DIRECT_CB_THREADS, cb_ana, side>>>(P, D.direct, map, d_w, use_w);
-            else ring_direct_synthesis_cb_kernel<T, CB><<<grid, DIRECT_CB_THREADS, cb_syn, side>>>(P, D.direct, map, d_w, use_w);
+            const dim3 grid(nd, (P.batch + CB - 1) / CB);
+            if (ANALYSIS) ring_direct_analysis_cb_kernel<T, CB><<<grid, DIRECT_CB_THREADS, cb_ana, side>>>(P, items, map, d_w, use_w);
+            else ring_direct_synthesis_cb_kernel<T, CB><<<grid, DIRECT_CB_THREADS, cb_syn, side>>>(P, items, map, d_w, use_w);
         } else if (ANALYSIS)
-            ring_direct_analysis_kernel<T><<<dim3(D.n_direct, P.batch), FFT_THREADS, (size_t)DIRECT_MAX_N * 3 * sizeof(T), side>>>(
-                P, D.direct, map, d_w, use_w);
+            ring_direct_analysis_kernel<T><<<dim3(nd, P.batch), FFT_THREADS, (size_t)DIRECT_MAX_N * 3 * sizeof(T), side>>>(
+                P, items, map, d_w, use_w);
         else
-            ring_direct_synthesis_kernel<T><<<dim3(D.n_direct, P.batch), FFT_THREADS,
-                                              ((size_t)DIRECT_MAX_N + D.max_mcut_direct + 1) * 2 * sizeof(T), side>>>(P, D.direct, map, d_w, use_w);
+            ring_direct_synthesis_kernel<T><<<dim3(nd, P.batch), FFT_THREADS,
+                                              ((size_t)DIRECT_MAX_N + F.max_mcut_direct + 1) * 2 * sizeof(T), side>>>(P, items, map, d_w, use_w);
     }
     if ((e = cudaGetLastError()) != cudaSuccess) return e;
     if (fork) {
-        if ((e = cudaEventRecord(D.ev_join, side)) != cudaSuccess) return e;
-        if ((e = cudaStreamWaitEvent(st, D.ev_join, 0)) != cudaSuccess) return e;
+        if ((e = cudaEventRecord(D->ev_join, side)) != cudaSuccess) return e;
+        if ((e = cudaStreamWaitEvent(st, D->ev_join, 0)) != cudaSuccess) return e;
     }
     return cudaSuccess;
 }
 
-cudaError_t launch_fft_analysis(const HostPlan& hp, const void* d_map, const double* d_w, int use_w, cudaStream_t st) {
+cudaError_t launch_fft_analysis(const HostPlan& hp, const DevPlan& P, const void* d_map, const double* d_w, int use_w,
+                                cudaStream_t st) {
     // analysis kernels only read the map; one launcher template serves both directions
-    return hp.dtype == CUHPX_F64 ? run_fft_stage<double, true>(hp, (double*)const_cast<void*>(d_map), d_w, use_w, st)
-                                 : run_fft_stage<float, true>(hp, (float*)const_cast<void*>(d_map), d_w, use_w, st);
+    return hp.dtype == CUHPX_F64 ? run_fft_stage<double, true>(hp, P, (double*)const_cast<void*>(d_map), d_w, use_w, st)
+                                 : run_fft_stage<float, true>(hp, P, (float*)const_cast<void*>(d_map), d_w, use_w, st);
 }
 
-cudaError_t launch_fft_synthesis(const HostPlan& hp, void* d_map, const double* d_w, int use_w, cudaStream_t st) {
-    return hp.dtype == CUHPX_F64 ? run_fft_stage<double, false>(hp, (double*)d_map, d_w, use_w, st)
-                                 : run_fft_stage<float, false>(hp, (float*)d_map, d_w, use_w, st);
+cudaError_t launch_fft_synthesis(const HostPlan& hp, const DevPlan& P, void* d_map, const double* d_w, int use_w,
+                                 cudaStream_t st) {
+    return hp.dtype == CUHPX_F64 ? run_fft_stage<double, false>(hp, P, (double*)d_map, d_w, use_w, st)
+                                 : run_fft_stage<float, false>(hp, P, (float*)d_map, d_w, use_w, st);
 }
 
 }  // namespace cuhpx

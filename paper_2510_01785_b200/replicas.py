@@ -22,12 +22,21 @@ def rank_seed(seed: int, rank: int) -> int:
     return int(seed) + 1000 * int(rank)
 
 
-def channel_shard(batch: int, rank: int, world_size: int):
-    """Contiguous slice [lo, hi) of the `batch` independent channels that `rank` owns when one batched call is
-    split over ranks (sizes differ by at most one; empty when there are more ranks than channels)."""
-    base, extra = divmod(int(batch), int(world_size))
-    lo = rank * base + min(rank, extra)
-    return lo, lo + base + (1 if rank < extra else 0)
+def spawn_ranks(nproc: int, argv, env=None) -> int:
+    """Launch `nproc` ranks of the script `argv` (one per GPU of this node) the way the driver does -- torchrun with a
+    loop-back rendezvous on a free port -- and return its exit code.  bench.py calls this when it is started plainly
+    with --gpus N > 1 (no WORLD_SIZE in the environment), so that `python bench.py --gpus N` really runs N ranks."""
+    import os
+    import socket
+    import subprocess
+    import sys
+
+    with socket.socket() as s:
+        s.bind(("127.0.0.1", 0))
+        port = s.getsockname()[1]
+    cmd = [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", f"--nproc-per-node={int(nproc)}",
+           "--master-addr", "127.0.0.1", "--master-port", str(port)] + list(argv)
+    return subprocess.run(cmd, env=dict(os.environ if env is None else env)).returncode
 
 
 def reduce_timing(ms: float, units: float, device=None):

@@ -69,12 +69,18 @@ def test_workspace_bytes_and_argument_validation():
     assert lib.cuhpx_workspace_init(4, 4, 4, 1, 1, None, 1 << 20, None) == B.CUHPX_EINVAL
     assert lib.cuhpx_workspace_init(4, 4, 4, 1, 1, 8, 1 << 20, None) == B.CUHPX_EINVAL  # misaligned
     assert lib.cuhpx_workspace_init(4, 4, 4, 1, 1, 256, 16, None) == B.CUHPX_EWORKSPACE  # too small
-    # unknown workspace -> EWORKSPACE; bad scalars / null / aliased pointers -> EINVAL
-    assert lib.cuhpx_map2alm(4, 4, 4, 1, 1, 256, 512, None, 1024, 1 << 20, None) == B.CUHPX_EWORKSPACE
+    # workspace too small -> EWORKSPACE; bad scalars / null / overlapping pointers -> EINVAL
+    assert lib.cuhpx_map2alm(4, 4, 4, 1, 1, 256, 1 << 21, None, 1 << 22, 64, None) == B.CUHPX_EWORKSPACE
     assert lib.cuhpx_map2alm(5, 4, 4, 1, 1, 256, 512, None, 1024, 1 << 20, None) == B.CUHPX_EINVAL
     assert lib.cuhpx_alm2map(4, 4, 4, 1, 1, None, 512, 1024, 1 << 20, None) == B.CUHPX_EINVAL
-    assert lib.cuhpx_alm2map(4, 4, 4, 1, 1, 512, 512, 1024, 1 << 20, None) == B.CUHPX_EINVAL
+    assert lib.cuhpx_alm2map(4, 4, 4, 1, 1, 512, 512, 1 << 22, 1 << 20, None) == B.CUHPX_EINVAL
+    assert lib.cuhpx_alm2map(4, 4, 4, 1, 1, 512, 512 + 16, 1 << 22, 1 << 20, None) == B.CUHPX_EINVAL  # partial overlap
+    assert lib.cuhpx_alm2map(4, 4, 4, 1, 1, 512, 1 << 22, 1 << 22, 1 << 20, None) == B.CUHPX_EINVAL  # output inside workspace
     assert lib.cuhpx_alm2map_adjoint(4, 4, 4, 1, 1, 256, 520, 1024, 1 << 20, None) == B.CUHPX_EINVAL
     assert lib.cuhpx_map2alm_adjoint(4, 4, 4, 1, 2, 256, 512, None, 1024, 1 << 20, None) == B.CUHPX_EINVAL
-    assert lib.cuhpx_analysis_fft_stage(256, None, 0, 1024, None) == B.CUHPX_EWORKSPACE
-    assert lib.cuhpx_workspace_release(1024) == B.CUHPX_EWORKSPACE
+    assert lib.cuhpx_analysis_fft_stage(4, 4, 4, 1, 1, 256, None, 0, 1 << 22, 64, None) == B.CUHPX_EWORKSPACE
+    assert lib.cuhpx_workspace_bytes(4, 4, 4, 65536, 1) == 0  # channels index a grid dimension
+    assert B.cuhpx_spectra_offset((4, 4, 4, 1, 1)) > 0 and B.cuhpx_spectra_offset((3, 4, 4, 1, 1)) == 0
+    assert len(B.cuhpx_plan_mcut((4, 8, 8, 1, 1))) == 15
+    st = B.cuhpx_plan_stats((32, 64, 64, 1, 1))
+    assert st["legendre_terms_full"] == 2145 * 64 and 0 < st["legendre_terms_executed"] <= st["legendre_terms_full"]

@@ -174,6 +174,9 @@ def test_map2alm_iter_matches_oracle(nside, lmax, batch, dtype, n_iter, weighted
     # channel group; packed-FMA synthesis with two channel groups, the second ragged (both CTA shapes)
     (32, 64, 64, 5, "f64"), (256, 300, 300, 6, "f32"), (256, 600, 450, 6, "f32"), (64, 128, 128, 11, "f32"),
     (128, 520, 520, 9, "f32"),
+    # fp32 with few channels at sizes where the exponent-scaled seeds matter (sc < 0 on polar rings) and the
+    # analysis walks several ring chunks: legendre_analysis_kernel<float, 1 / 4>, legendre_synthesis_kernel<float, 1 / 4>
+    (256, 600, 600, 1, "f32"), (512, 700, 700, 4, "f32"),
 ])
 def test_small_and_ragged_cases(nside, lmax, mmax, batch, dtype):
     """mmax < lmax, lmax far above 2 nside (every polar ring aliases), batch not a multiple of the channel
@@ -189,16 +192,11 @@ def test_fft_stage_alone_matches_ring_dft():
     nside, lmax = 16, 40
     T = make_transform(nside, lmax, lmax, 2, "f64")
     fmap = synth.gaussian_map(55, nside, 2)
-    B.cuhpx_analysis_fft_stage(to_dev(fmap, "f64"), None, 0, T.workspace)
+    B.cuhpx_analysis_fft_stage(T.params, to_dev(fmap, "f64"), None, 0, T.workspace)
     torch.cuda.synchronize()
-    mcut = B.cuhpx_workspace_mcut(T.workspace, nside)
-    stride = B.cuhpx_spectra_stride(lmax)
+    mcut = B.cuhpx_plan_mcut(T.params)
     nrings = 4 * nside - 1
-    nbytes = 2 * nrings * stride * 16
-    ptr = B.lib().cuhpx_workspace_spectra(T.workspace.data_ptr())
-    off = (ptr - T.workspace.data_ptr()) // 8
-    spec = T.workspace[off: off + nbytes // 8].view(torch.float64).cpu().numpy().view(np.complex128)
-    spec = spec.reshape(2, nrings, stride)
+    spec = T.spectra_view().cpu().numpy()
     for ring in range(1, nrings + 1):
         n, start = oracle.ring_geometry(nside, ring)[:2]
         assert mcut[ring - 1] >= min(lmax, 2)  # low orders are needed on every ring
@@ -234,27 +232,37 @@ def test_stream_ordering_and_error_codes():
         got = T.map2alm(fmap)
     s.synchronize()
     assert torch.equal(ref, got)
-    # a workspace initialised for other parameters is refused
-    alm = torch.empty(1, T.nalm, dtype=torch.complex128, device="cuda")
+    # A workspace initialised for other parameters: the library keeps no per-workspace state, so the host cannot
+    # know; every kernel checks the header, the call leaves the output untouched and marks the workspace, and
+    # cuhpx_workspace_check (synchronising) reports it.  Overlapping buffers are refused on the host.
+    B.cuhpx_workspace_check(*T.params, T.workspace)
+    big = torch.empty(B.cuhpx_workspace_bytes(nside, lmax + 8, lmax + 8, 1, B.CUHPX_F64) // 8 + 64, dtype=torch.int64, device="cuda")
+    big[: T.workspace.numel()] = T.workspace  # a moved copy of an initialised workspace works as is
+    got2 = torch.empty_like(ref)
+    B.cuhpx_map2alm(*T.params, fmap, got2, None, big[: T.workspace.numel()])
+    assert torch.equal(ref, got2)
+    nalm2 = B.cuhpx_alm_count(lmax + 8, lmax + 8)
+    alm = torch.full((1, nalm2), 7.0 + 1.0j, dtype=torch.complex128, device="cuda")
+    B.cuhpx_map2alm(nside, lmax + 8, lmax + 8, 1, B.CUHPX_F64, fmap, alm, None, big)  # header says (lmax, lmax)
+    torch.cuda.synchronize()
+    assert torch.all(alm == 7.0 + 1.0j), "a kernel trusted a workspace built for other parameters"
     with pytest.raises(B.CuhpxError) as ei:
-        B.cuhpx_map2alm(nside, lmax, lmax - 1, 1, B.CUHPX_F64, fmap, alm, None, T.workspace)
+        B.cuhpx_workspace_check(nside, lmax + 8, lmax + 8, 1, B.CUHPX_F64, big)
     assert ei.value.status == B.CUHPX_EWORKSPACE
-    with pytest.raises(B.CuhpxError) as ei:
-        B.cuhpx_map2alm(nside, lmax, lmax, 1, B.CUHPX_F32, fmap, alm, None, T.workspace)
+    with pytest.raises(B.CuhpxError) as ei:  # too small for the parameters of the call
+        B.cuhpx_map2alm(nside, lmax + 8, lmax + 8, 1, B.CUHPX_F64, fmap, alm, None, T.workspace)
     assert ei.value.status == B.CUHPX_EWORKSPACE
+    both = torch.empty(T.npix + 2 * T.nalm, dtype=torch.float64, device="cuda")
+    with pytest.raises(B.CuhpxError) as ei:  # partial overlap of input and output
+        B.cuhpx_map2alm(*T.params, both[: T.npix].view(1, -1), both[T.npix - 2: T.npix - 2 + 2 * T.nalm].view(torch.complex128).view(1, -1),
+                        None, T.workspace)
+    assert ei.value.status == B.CUHPX_EINVAL
 
 
 # ----------------------------------------------------------------------------- FFT stage at full ring sizes
 
 def _spectra_view(B, T, batch, nside, mmax, dtype):
-    stride = B.cuhpx_spectra_stride(mmax)
-    nrings = 4 * nside - 1
-    esz = 16 if dtype == "f64" else 8
-    ptr = B.lib().cuhpx_workspace_spectra(T.workspace.data_ptr())
-    off = ptr - T.workspace.data_ptr()
-    raw = T.workspace.view(torch.uint8)[off: off + batch * nrings * stride * esz]
-    v = raw.view(torch.complex128 if dtype == "f64" else torch.complex64)
-    return v.view(batch, nrings, stride)
+    return T.spectra_view()
 
 
 def _class_rings(nside):
@@ -273,7 +281,7 @@ def test_fft_stages_every_size_class(nside, lmax, dtype):
     kernel family (direct / pow2 / chirp-z) and every block-FFT size (2^8 .. 2^13), incl. the m > N/2 fold."""
     B = _binding()
     T = make_transform(nside, lmax, lmax, 1, dtype)
-    mcut = B.cuhpx_workspace_mcut(T.workspace, nside)
+    mcut = B.cuhpx_plan_mcut(T.params)
     rings = _class_rings(nside)
     npix = 12 * nside * nside
     fmap = np.zeros(npix)
@@ -281,7 +289,7 @@ def test_fft_stages_every_size_class(nside, lmax, dtype):
         n, start = oracle.ring_geometry(nside, r)[:2]
         fmap[start:start + n] = synth.normal(900 + nside, r, n)
     fmap_r = rounded(fmap, dtype)
-    B.cuhpx_analysis_fft_stage(to_dev(fmap[None], dtype), None, 0, T.workspace)
+    B.cuhpx_analysis_fft_stage(T.params, to_dev(fmap[None], dtype), None, 0, T.workspace)
     torch.cuda.synchronize()
     spec = _spectra_view(B, T, 1, nside, lmax, dtype)
     tol = 1e-12 if dtype == "f64" else 3e-6
@@ -303,7 +311,7 @@ def test_fft_stages_every_size_class(nside, lmax, dtype):
         Gs[r] = G
         spec[0, r - 1, : mc + 1] = torch.from_numpy(G).to(spec.dtype).cuda()
     out = torch.empty(1, npix, dtype=torch.float64 if dtype == "f64" else torch.float32, device="cuda")
-    B.cuhpx_synthesis_fft_stage(out, None, 0, T.workspace)
+    B.cuhpx_synthesis_fft_stage(T.params, out, None, 0, T.workspace)
     torch.cuda.synchronize()
     out = out.cpu().numpy().astype(np.float64)[0]
     for r in rings:
@@ -378,6 +386,30 @@ def test_cfg4_nside1024_fp32_batch8():
 
 
 @pytest.mark.slow
+@pytest.mark.parametrize("batch", [1, 3])
+def test_nside1024_fp32_few_channels(batch):
+    """A single fp32 map (and three) at nside 1024, lmax = mmax = 2047: the default user configuration runs the
+    few-channel fp32 kernels (multi-chunk analysis, exponent-scaled seeds), which configs[3] (batch 8) never reaches.
+    Oracle: seeded subset on the first and last channel."""
+    nside, lmax = 1024, 2047
+    T = make_transform(nside, lmax, lmax, batch, "f32")
+    alm = synth.powerlaw_alm(414, lmax, lmax, batch)
+    rings = _subset_rings(414, nside, 20)
+    sl, sm = _subset_lm(414, lmax, lmax, 24, 6)
+    sl_idx = [oracle.alm_index(lmax, l, m) for l, m in zip(sl, sm)]
+    slices = _ring_slices(nside, rings)
+    got_map = T.alm2map(to_dev(alm, "f32", True)).cpu().numpy()
+    galm = T.map2alm(torch.from_numpy(got_map).cuda()).cpu().numpy().astype(np.complex128)
+    for c in sorted({0, batch - 1}):
+        ref = oracle.alm2map_rings(nside, lmax, lmax, rounded(alm[c], "f32", True), rings)
+        got = np.concatenate([got_map[c].astype(np.float64)[s] for s in slices])
+        assert err32(got, ref) <= TOL32
+        ref = oracle.map2alm_subset(nside, lmax, lmax, got_map[c].astype(np.float64), sl, sm)
+        assert err32(galm[c][sl_idx], ref) <= TOL32
+        assert np.abs(galm[c][sl_idx] - ref).max() <= 2e-5 * np.abs(ref).max()
+
+
+@pytest.mark.slow
 def test_cfg5_nside4096_fp64():
     """configs[4]: nside 4096, lmax = mmax = 8191, fp64: alm -> alm2map -> map2alm.  Oracle checked on a seeded
     subset of 512+ (l, m) and 64+ rings; the analysis is checked on the GPU's own map so both
@@ -394,22 +426,22 @@ def test_cfg5_nside4096_fp64():
     got_map = dmap.cpu().numpy()[0]
     ref = oracle.alm2map_rings(nside, lmax, lmax, alm[0], rings)
     got = np.concatenate([got_map[s] for s in slices])
-    e_syn = np.abs(got - ref).max() / np.abs(got_map).max()
+    e_syn = np.abs(got - ref).max() / np.abs(ref).max()  # oracle-side maximum (of the sampled rings)
     assert e_syn <= TOL64, f"alm2map {e_syn:.3e}"
     galm = T.map2alm(dmap).cpu().numpy()[0]
     ref = oracle.map2alm_subset(nside, lmax, lmax, got_map, sl, sm)
-    e_ana = np.abs(galm[sl_idx] - ref).max() / np.abs(galm).max()
+    e_ana = np.abs(galm[sl_idx] - ref).max() / np.abs(ref).max()  # the sample holds (0, 0), the largest coefficient
     assert e_ana <= TOL64, f"map2alm {e_ana:.3e}"
     assert np.all(galm[: lmax + 1].imag == 0.0)
     # adjoints on the same subset
     gst = T.alm2map_adjoint(dmap).cpu().numpy()[0]
     ref = oracle.alm2map_adjoint_subset(nside, lmax, lmax, got_map, sl, sm)
-    e_st = np.abs(gst[sl_idx] - ref).max() / np.abs(gst).max()
+    e_st = np.abs(gst[sl_idx] - ref).max() / np.abs(ref).max()
     assert e_st <= TOL64, f"alm2map_adjoint {e_st:.3e}"
     gat = T.map2alm_adjoint(to_dev(alm, "f64", True)).cpu().numpy()[0]
     ref = oracle.map2alm_adjoint_rings(nside, lmax, lmax, alm[0], rings)
     got = np.concatenate([gat[s] for s in slices])
-    e_at = np.abs(got - ref).max() / np.abs(gat).max()
+    e_at = np.abs(got - ref).max() / np.abs(ref).max()
     assert e_at <= TOL64, f"map2alm_adjoint {e_at:.3e}"
     print("cfg5", e_syn, e_ana, e_st, e_at)
 
@@ -432,3 +464,33 @@ def test_results_are_bitwise_repeatable(nside, lmax, batch, dtype):
         assert torch.equal(T.alm2map_adjoint(fmap), ref["st"])
         assert torch.equal(T.alm2map(alm), ref["s"])
         assert torch.equal(T.map2alm_adjoint(alm), ref["at"])
+
+
+@pytest.mark.parametrize("nside,lmax,batch,dtype", [(64, 128, 1, "f64"), (128, 255, 8, "f32"), (512, 1023, 1, "f64"),
+                                                    (256, 511, 2, "f32")])
+def test_cuda_graph_capture_replay(nside, lmax, batch, dtype):
+    """include/cuhpx.h promises that the transform calls never synchronise and can be captured in a CUDA graph
+    (the FFT stage forks part of its work onto a library stream and joins it back: exactly what breaks under capture
+    if done wrong).  Capture map2alm + alm2map once, replay on three fresh inputs, compare with eager bit for bit."""
+    B = _binding()
+    T = make_transform(nside, lmax, lmax, batch, dtype)
+    ins = [(to_dev(synth.gaussian_map(40 + k, nside, batch), dtype), to_dev(synth.powerlaw_alm(50 + k, lmax, lmax, batch), dtype, True))
+           for k in range(3)]
+    s_map, s_alm = ins[0][0].clone(), ins[0][1].clone()
+    o_alm = torch.zeros_like(s_alm)
+    o_map = torch.zeros_like(s_map)
+    T.map2alm(s_map)  # warm: nothing is created lazily inside the capture
+    torch.cuda.synchronize()
+    g = torch.cuda.CUDAGraph()
+    with torch.cuda.graph(g):
+        B.cuhpx_map2alm(*T.params, s_map, o_alm, None, T.workspace)
+        B.cuhpx_alm2map(*T.params, s_alm, o_map, T.workspace)
+    for fmap, alm in ins:
+        s_map.copy_(fmap)
+        s_alm.copy_(alm)
+        o_alm.zero_()
+        o_map.zero_()
+        g.replay()
+        torch.cuda.synchronize()
+        assert torch.equal(o_alm, T.map2alm(fmap)) and torch.equal(o_map, T.alm2map(alm))
+    B.cuhpx_workspace_check(*T.params, T.workspace)
