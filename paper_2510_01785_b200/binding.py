@@ -307,7 +307,11 @@ class Transform:
         self.device = torch.device(device)
         self.npix = cuhpx_npix(nside)
         self.nalm = cuhpx_alm_count(lmax, mmax)
-        nbytes = cuhpx_workspace_bytes(nside, lmax, mmax, batch, self.code)
+        import time
+
+        t0 = time.perf_counter()
+        nbytes = cuhpx_workspace_bytes(nside, lmax, mmax, batch, self.code)  # first call for these parameters: host planning
+        plan_seconds = time.perf_counter() - t0
         if nbytes == 0:
             raise CuhpxError(CUHPX_EINVAL, "cuhpx_workspace_bytes")
         self.workspace = torch.empty((nbytes + 7) // 8, dtype=torch.int64, device=self.device)
@@ -315,13 +319,12 @@ class Transform:
         if ring_weights is not None:
             self.ring_weights = ring_weights.to(device=self.device, dtype=torch.float64).contiguous()
         with torch.cuda.device(self.device):
-            import time
-
             torch.cuda.synchronize()
             t0 = time.perf_counter()
             cuhpx_workspace_init(nside, lmax, mmax, batch, self.code, self.workspace)  # returns when the tables are built
-            #: seconds of cuhpx_workspace_init alone (host planning + table kernels; SURVEY 8(a) a0 "first-call time")
-            self.init_seconds = time.perf_counter() - t0
+            #: seconds of the table set-up alone (SURVEY 8(a) a0 "first-call time"): host planning (ring classes, cut-offs;
+            #: memoised per parameter set, so ~0 from the second Transform on) + cuhpx_workspace_init (uploads, table kernels)
+            self.init_seconds = plan_seconds + (time.perf_counter() - t0)
 
     def _args(self):
         return self.nside, self.lmax, self.mmax, self.batch, self.code

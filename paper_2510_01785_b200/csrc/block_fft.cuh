@@ -208,15 +208,24 @@ template <int R> __device__ __forceinline__ constexpr int brev_r(int x) {
 }
 
 // Multiply register r (holding butterfly output q = bitrev_R(r)) by w^q, w = exp(-2 pi i t / Q) (conjugated if
-// CONJ).  w^(2^k) come from the root table, the other powers are running products (<= 3 multiplies from a table
-// value).  q t < Q for every q < R.
+// CONJ).  fp32: w^(2^k) come from the root table, the other powers are running products (<= 3 multiplies from a
+// table value).  fp64: only w comes from the table, w^2, w^4, w^8 by squaring (3 flops and no shared-memory access
+// instead of 2 LDS.128 + 4 flops; the fp64 kernels are bound by the shared-memory pipe, and <= 3 squarings cost
+// ~1e-15 of phase accuracy).  q t < Q for every q < R.
 template <int R, bool CONJ, typename T>
 __device__ __forceinline__ void apply_twiddles(const Roots<T>& rt, int t, T* re, T* im) {
-    T w1r = 0, w1i = 0, cr = 1, ci = 0;
+    T w1r = 0, w1i = 0, cr = 1, ci = 0, pr = 1, pi = 0;  // (pr, pi): the last power of two
 #pragma unroll
     for (int q = 1; q < R; ++q) {
-        if ((q & (q - 1)) == 0) {  // power of two: table value
-            rt.template get<(CONJ ? +1 : -1)>(q * t, cr, ci);
+        if ((q & (q - 1)) == 0) {  // power of two
+            if (q == 1 || sizeof(T) == 4) {
+                rt.template get<(CONJ ? +1 : -1)>(q * t, cr, ci);
+            } else {
+                cr = pr * pr - pi * pi;
+                ci = 2 * pr * pi;
+            }
+            pr = cr;
+            pi = ci;
             if (q == 1) {
                 w1r = cr;
                 w1i = ci;
@@ -233,14 +242,25 @@ __device__ __forceinline__ void apply_twiddles(const Roots<T>& rt, int t, T* re,
     }
 }
 
-// LOGQ: log2 of the order of the root table handed to forward / inverse (LOGQ >= LOGN)
-template <typename T, int LOGN, int LOGQ = LOGN> struct BlockFFT {
+// LOGQ: log2 of the order of the root table handed to forward / inverse (LOGQ >= LOGN).
+// GROUPS > 1: the CTA holds GROUPS independent teams of NT threads, each running its own FFT on its own exchange
+// buffer; `tid` is the index inside the team and the passes meet at the team's named barrier (1 + team) instead of
+// the CTA barrier, so one team's exchange overlaps the other's butterflies.
+template <typename T, int LOGN, int LOGQ = LOGN, int GROUPS = 1> struct BlockFFT {
     using P = FftPlan<LOGN>;
     using T2 = typename V2<T>::type;
     static constexpr int N = 1 << LOGN, NT = P::NT, E = N / NT, NP = P::NP;
     static constexpr int RLAST = PassRadix<LOGN, NP - 1>::value;
     static constexpr int R0 = P::R0;
     static constexpr size_t SMEM_BYTES = Xchg<T>::bytes(N);
+
+    static __device__ __forceinline__ void team_sync() {
+        if constexpr (GROUPS == 1) {
+            __syncthreads();
+        } else {
+            asm volatile("bar.sync %0, %1;" ::"r"(1 + (int)(threadIdx.x / NT)), "n"(NT) : "memory");
+        }
+    }
 
     // position of register e = c R + rho in pass S
     template <int S> static __device__ __forceinline__ int pos(int tid, int c, int rho) {
@@ -299,7 +319,7 @@ template <typename T, int LOGN, int LOGQ = LOGN> struct BlockFFT {
         if constexpr (S < NP) {
             constexpr int R = PassRadix<LOGN, S>::value, L = PassLen<LOGN, S>::value, LR = L / R;
             if constexpr (S > 0) {
-                __syncthreads();
+                team_sync();
                 load<S>(re, im, x, tid);
             }
 #pragma unroll
@@ -320,7 +340,7 @@ template <typename T, int LOGN, int LOGQ = LOGN> struct BlockFFT {
         if constexpr (S >= 0) {
             constexpr int R = PassRadix<LOGN, S>::value, L = PassLen<LOGN, S>::value, LR = L / R;
             if constexpr (S < NP - 1) {
-                __syncthreads();
+                team_sync();
                 load<S>(re, im, x, tid);
             }
 #pragma unroll
@@ -347,7 +367,7 @@ template <typename T, int LOGN, int LOGQ = LOGN> struct BlockFFT {
     // write the forward result to shared memory in natural frequency order (call after forward; syncs first,
     // because other threads may still be reading the exchange buffer; caller syncs before reading)
     static __device__ __forceinline__ void store_natural(const T (&re)[E], const T (&im)[E], const Xchg<T>& x, int tid) {
-        __syncthreads();
+        team_sync();
 #pragma unroll
         for (int e = 0; e < E; ++e) x.st(freq_index(tid, e), re[e], im[e]);
     }

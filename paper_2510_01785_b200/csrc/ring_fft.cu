@@ -452,6 +452,36 @@ __device__ __forceinline__ typename V2<T>::type analysis_unpack(T z1r, T z1i, T 
     return o;
 }
 
+// Hermitian unpack of TWO outputs at once: the bins k and n - k (n = N / 2, 0 <= k <= n / 2) of the packed analysis FFT
+// share E = (Z[k] + conj Z[n-k]) / 2 and O = -i (Z[k] - conj Z[n-k]) / 2, and W_N^(n-k) = -conj(W_N^k):
+//   X[k] = E + W_N^k O,   X[n-k] = conj(E - W_N^k O);   twists: omega^k and omega^(n-k) = -i conj(omega^k).
+// One root look-up and ~29 flops for two outputs (the one-at-a-time unpack: two look-ups and ~30 flops per output).
+// z1 = Z[k], z2 = Z[(n - k) mod n]; (pc, ps) = omega^k = exp(-i pi k / N); h = weight / 2.  Valid for k = 0 (f2 = X[n],
+// the Nyquist bin) and k = n / 2 (f1 = f2).
+template <typename T>
+__device__ __forceinline__ void analysis_unpack_pair(T z1r, T z1i, T z2r, T z2i, T pc, T ps, int shifted, T h,
+                                                     typename V2<T>::type& f1, typename V2<T>::type& f2) {
+    const T er = z1r + z2r, ei = z1i - z2i;      // 2 E
+    const T orr = z1i + z2i, oi = z2r - z1r;     // 2 O = -i (z1 - conj z2)
+    const T wc = pc * pc - ps * ps, ws = 2 * pc * ps;  // W_N^k = omega^(2 k)
+    const T tr = wc * orr - ws * oi, ti = wc * oi + ws * orr;
+    const T x1r = er + tr, x1i = ei + ti;        // 2 X[k]
+    const T x2r = er - tr, x2i = ei - ti;        // 2 conj X[n-k]
+    if (shifted) {
+        const T hc = h * pc, hs = h * ps;
+        f1.x = x1r * hc - x1i * hs;
+        f1.y = x1r * hs + x1i * hc;
+        const T ur = x2r * hc - x2i * hs, ui = x2r * hs + x2i * hc;  // h omega^k (2 conj X[n-k])
+        f2.x = -ui;  // -i conj(u)
+        f2.y = -ur;
+    } else {
+        f1.x = h * x1r;
+        f1.y = h * x1i;
+        f2.x = h * x2r;
+        f2.y = -h * x2i;
+    }
+}
+
 // Resident CTAs per SM the register allocation aims for: 16 points per thread are 64 (fp64) / 32 (fp32) data
 // registers, so fp64 kernels get 128 registers per thread and fp32 pow2 kernels 64.
 template <typename T, int LOG> struct MinBlocks {
@@ -493,8 +523,21 @@ __global__ void __launch_bounds__(FftPlan<LOGN>::NT, MinBlocks<T, LOGN>::value) 
     F::store_natural(re, im, xs, tid);
     __syncthreads();
     T2* dst = reinterpret_cast<T2*>(P.spectra) + ((size_t)ch * P.nrings + R.r) * P.mstride;
-#pragma unroll 4
-    for (int m = tid; m <= R.mcut; m += NT) {
+    const T h = (T)0.5 * wt;
+    const int mcut = R.mcut;
+#pragma unroll 2
+    for (int k = tid; k <= n / 2; k += NT) {  // orders k and n - k together
+        if (k > mcut) break;
+        T z1r, z1i, z2r, z2i, pc, ps;
+        xs.ld(k, z1r, z1i);
+        xs.ld((n - k) & (n - 1), z2r, z2i);
+        rt.template get<-1>(k, pc, ps);
+        T2 f1, f2;
+        analysis_unpack_pair<T>(z1r, z1i, z2r, z2i, pc, ps, R.shifted, h, f1, f2);
+        dst[k] = f1;
+        if (n - k <= mcut && 2 * k != n) dst[n - k] = f2;
+    }
+    for (int m = n + 1 + tid; m <= mcut; m += NT) {  // aliased orders (lmax beyond the ring's Nyquist frequency)
         const int k = m & (N - 1);
         const bool cj = k > n;
         const int kk = cj ? N - k : k;
@@ -541,6 +584,132 @@ __global__ void __launch_bounds__(FftPlan<LOGN>::NT, MinBlocks<T, LOGN>::value) 
         o.x = wt * a;
         o.y = -wt * b;
         dst[t] = o;
+    }
+}
+
+// ------------------------------------------------------------------ long power-of-two rings in halves
+// A packed FFT of n = 2 H points whose registers fill a whole SM (fp64, N = 16384: 8192 complex = half of the register
+// file, one 512-thread CTA per SM, load / passes / store never overlap) is split with one radix-2 step:
+//
+// analysis: work item = (ring, parity p of the output bin).  Z[2 k' + p] = FFT_H(y_p)[k'],
+//   y_p[j] = (z[j] + (-1)^p z[j + H]) W_n^(p j), formed while loading; the Hermitian partners k and n - k have the same
+//   parity, so the unpack stays inside the item.  256 threads, two items resident per SM: one loads or stores while
+//   the other computes.  Both items of a ring read the whole ring (the second read comes from L2) and write every
+//   other 16-byte bin of the spectra row (the halves of a 32-byte sector meet in L2, microseconds apart).
+// synthesis: one CTA of two teams of NT threads; team g transforms the inputs of parity g, Y[2 k' + g] (decimation in
+//   time: D[t] = A[t] + W_n^t B[t], D[t + H] = A[t] - W_n^t B[t]); the teams meet only at their own named barriers
+//   during the passes, then all threads combine and store whole sectors of the map.
+template <typename T, int LOGH>
+__global__ void __launch_bounds__(FftPlan<LOGH>::NT, 2) ring_pow2_half_analysis_kernel(DevPlan P, const RingInfo* __restrict__ info,
+                                                                                      const T* __restrict__ map,
+                                                                                      const double* __restrict__ w, int use_w,
+                                                                                      FftTables tabs) {
+    if (!ws_ok(P)) return;
+    using F = BlockFFT<T, LOGH, LOGH + 3>;
+    using T2 = typename V2<T>::type;
+    constexpr int H = F::N, n = 2 * H, N = 2 * n, Q = 2 * N, E = F::E, NT = F::NT;
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    const Xchg<T> xs(smem_raw, H);
+    T2* rbase = reinterpret_cast<T2*>(smem_raw + Xchg<T>::bytes(H));
+    const int tid = threadIdx.x;
+    const int ch = blockIdx.y;
+    const int par = blockIdx.x & 1;
+    const RingInfo R = load_info(info, blockIdx.x >> 1);
+    const T2* src = reinterpret_cast<const T2*>(map + (size_t)ch * P.npix + R.start);
+    T re[E], im[E];
+#pragma unroll
+    for (int e = 0; e < E; ++e) {
+        const int j = F::index0(tid, e);
+        const T2 a = src[j], b = src[j + H];
+        re[e] = par ? a.x - b.x : a.x + b.x;
+        im[e] = par ? a.y - b.y : a.y + b.y;
+    }
+    fill_roots_pow2<T>(rbase, Q, reinterpret_cast<const T2*>(tabs.tw), tabs.twlen, tid, NT);
+    const T wt = (T)ring_weight(P, R, w, use_w);
+    __syncthreads();
+    const Roots<T> rt(rbase);
+    if (par) {
+        // times W_n^j = omega^(4 j), j = index0(tid, 0) + d_e with d_e a compile-time offset: one look-up per thread,
+        // the d_e factors are warp-uniform (broadcast) table entries
+        T w0c, w0s;
+        rt.template get<-1>(4 * F::index0(tid, 0), w0c, w0s);
+#pragma unroll
+        for (int e = 0; e < E; ++e) {
+            const int d = F::index0(0, e) - F::index0(0, 0);
+            T cc, cs;
+            rt.template get<-1>(4 * d, cc, cs);
+            const T wc = w0c * cc - w0s * cs, ws = w0c * cs + w0s * cc;
+            const T a = re[e], b = im[e];
+            re[e] = a * wc - b * ws;
+            im[e] = a * ws + b * wc;
+        }
+    }
+    F::forward(re, im, xs, rt, tid);
+    F::store_natural(re, im, xs, tid);
+    __syncthreads();
+    // bins k = 2 k' + par; partner n - k = 2 k'' + par with k'' = (H - k' - par) mod H
+    T2* dst = reinterpret_cast<T2*>(P.spectra) + ((size_t)ch * P.nrings + R.r) * P.mstride;
+    const T h = (T)0.5 * wt;
+    const int mcut = R.mcut;
+    const int npairs = par ? H / 2 : H / 2 + 1;
+#pragma unroll 2
+    for (int kp = tid; kp < npairs; kp += NT) {
+        const int k = 2 * kp + par;
+        if (k > mcut) break;
+        T z1r, z1i, z2r, z2i, pc, ps;
+        xs.ld(kp, z1r, z1i);
+        xs.ld((H - kp - par) & (H - 1), z2r, z2i);
+        rt.template get<-1>(k, pc, ps);
+        T2 f1, f2;
+        analysis_unpack_pair<T>(z1r, z1i, z2r, z2i, pc, ps, R.shifted, h, f1, f2);
+        dst[k] = f1;
+        if (n - k <= mcut && 2 * k != n) dst[n - k] = f2;
+    }
+}
+
+template <typename T, int LOGH>
+__global__ void __launch_bounds__(2 * FftPlan<LOGH>::NT, 1) ring_pow2_teams_synthesis_kernel(DevPlan P, const RingInfo* __restrict__ info,
+                                                                                            T* __restrict__ map,
+                                                                                            const double* __restrict__ w, int use_w,
+                                                                                            FftTables tabs) {
+    if (!ws_ok(P)) return;
+    using F = BlockFFT<T, LOGH, LOGH + 3, 2>;
+    using T2 = typename V2<T>::type;
+    constexpr int H = F::N, n = 2 * H, N = 2 * n, Q = 2 * N, E = F::E, NT = F::NT;
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    const int tid = threadIdx.x, team = tid / NT, tt = tid % NT;
+    const Xchg<T> xa(smem_raw, H), xb(smem_raw + Xchg<T>::bytes(H), H);
+    const Xchg<T>& xs = team ? xb : xa;
+    T2* rbase = reinterpret_cast<T2*>(smem_raw + 2 * Xchg<T>::bytes(H));
+    const int ch = blockIdx.y;
+    const RingInfo R = begin_item<T, false>(P, info, map, tabs.pf);
+    fill_roots_pow2<T>(rbase, Q, reinterpret_cast<const T2*>(tabs.tw), tabs.twlen, tid, 2 * NT);
+    const T wt = (T)ring_weight(P, R, w, use_w);
+    __syncthreads();
+    const Roots<T> rt(rbase);
+    const T2* G = reinterpret_cast<const T2*>(P.spectra) + ((size_t)ch * P.nrings + R.r) * P.mstride;
+    T re[E], im[E];
+#pragma unroll
+    for (int e = 0; e < E; ++e)
+        synth_packed_input<T, true>(G, 2 * F::index0(tt, e) + team, N, R.mcut, R.shifted, rt, re[e], im[e]);
+    F::forward(re, im, xs, rt, tt);
+    F::store_natural(re, im, xs, tt);
+    __syncthreads();
+    T2* dst = reinterpret_cast<T2*>(map + (size_t)ch * P.npix + R.start);
+#pragma unroll 2
+    for (int t = tid; t < H; t += 2 * NT) {
+        T ar, ai, br, bi, c, s;
+        xa.ld(t, ar, ai);
+        xb.ld(t, br, bi);
+        rt.template get<-1>(4 * t, c, s);  // W_n^t
+        const T pr = br * c - bi * s, pi = br * s + bi * c;
+        T2 o;
+        o.x = wt * (ar + pr);
+        o.y = -wt * (ai + pi);
+        dst[t] = o;
+        o.x = wt * (ar - pr);
+        o.y = -wt * (ai - pi);
+        dst[t + H] = o;
     }
 }
 
@@ -675,8 +844,31 @@ __global__ void __launch_bounds__(FftPlan<LOGM>::NT, MinBlocks<T, LOGM>::blue) r
     // Z[q] = Ze[q mod i] + W_n^q Zo[q mod i], q < n = 2 i.  twist = omega^m, W_N^kk = omega^(2 kk),
     // W_n^q = omega^(4 q); without aliasing (m <= n, the common case) kk = m and one root per output suffices.
     T2* dst = reinterpret_cast<T2*>(P.spectra) + ((size_t)ch * P.nrings + R.r) * P.mstride;
+    const int mcut = R.mcut;
+    const T h = (T)0.5 * wt;
+    // orders kk and n - kk together (they share E / O, see analysis_unpack_pair); W_n^(n - kk) = conj(W_n^kk)
 #pragma unroll 2
-    for (int m = tid; m <= R.mcut; m += NT) {
+    for (int kk = tid; kk <= i; kk += NT) {
+        if (kk > mcut) break;
+        T pc, ps;  // omega^kk
+        rt.template get<-1>(kk, pc, ps);
+        const T w2c = pc * pc - ps * ps, w2s = 2 * pc * ps;        // W_N^kk
+        const T w4c = w2c * w2c - w2s * w2s, w4s = 2 * w2c * w2s;  // W_n^kk (= -1 at kk = i)
+        const int a1 = kk == i ? 0 : kk, a2 = (kk == 0 || kk == i) ? 0 : i - kk;
+        const T c2 = (kk == 0) ? (T)1 : w4c, s2 = (kk == 0) ? (T)0 : -w4s;
+        const T2 ze1 = Ze[a1], ze2 = Ze[a2];
+        T o1r, o1i, o2r, o2i;
+        xs.ld(a1, o1r, o1i);
+        xs.ld(a2, o2r, o2i);
+        const T z1r = ze1.x + (o1r * w4c - o1i * w4s), z1i = ze1.y + (o1r * w4s + o1i * w4c);
+        const T z2r = ze2.x + (o2r * c2 - o2i * s2), z2i = ze2.y + (o2r * s2 + o2i * c2);
+        T2 f1, f2;
+        analysis_unpack_pair<T>(z1r, z1i, z2r, z2i, pc, ps, R.shifted, h, f1, f2);
+        dst[kk] = f1;
+        if (n - kk <= mcut && kk != i) dst[n - kk] = f2;
+    }
+    // aliased orders m > n (lmax beyond the ring's Nyquist frequency): one at a time
+    for (int m = n + 1 + tid; m <= mcut; m += NT) {
         const int k = m < N ? m : m % N;
         const bool cj = k > n;
         const int kk = cj ? N - k : k;
@@ -884,6 +1076,11 @@ template <typename T, int LOG> static size_t fft_smem_bytes(bool blue) {
     if (blue) return BlueSmem<T, LOG>::total;
     return Xchg<T>::bytes(1 << LOG) + sizeof(T) * 2 * (size_t)roots_len(4 << LOG);
 }
+constexpr int HALVES_LOG = 13;  // packed-FFT size class whose fp64 rings are processed in halves
+// exchange buffer(s) of H = 2^LOGH points + root table of order Q = 8 H
+template <typename T, int LOGH> static size_t half_smem_bytes(int teams) {
+    return teams * Xchg<T>::bytes(1 << LOGH) + sizeof(T) * 2 * (size_t)roots_len(8 << LOGH);
+}
 template <int LOG> static size_t filter_smem_bytes() {
     return Xchg<double>::bytes(1 << LOG) + sizeof(double2) * (size_t)roots_len(1 << LOG);
 }
@@ -908,6 +1105,7 @@ struct FftHost {
     long long filt_total;
     int twlen;
     int max_mcut_direct;
+    int pow2_max_mcut;  // largest order wanted on a belt ring
     int side_from;  // Bluestein classes with LOG <= side_from go to the side stream (with the direct kernel)
 };
 void free_fft_host(FftHost* f) { delete f; }
@@ -968,6 +1166,9 @@ size_t fft_plan_host(HostPlan& hp) {
     F->off_filt = take(csize * (size_t)fo);
     F->total = o;
     F->max_mcut_direct = 0;
+    F->pow2_max_mcut = 0;
+    for (int l = MIN_LOG; l <= MAX_LOG; ++l)
+        for (const RingInfo& R : F->pow2[l]) F->pow2_max_mcut = std::max(F->pow2_max_mcut, R.mcut);
     for (const RingInfo& R : F->direct) F->max_mcut_direct = std::max(F->max_mcut_direct, R.mcut);
     int lmax_blue = -1;
     for (int l = MIN_LOG; l <= MAX_LOG; ++l)
@@ -1020,6 +1221,12 @@ template <typename T> static cudaError_t set_all_attrs(DevRes& D, int sms) {
 #define CUHPX_ATTR(LOG) if ((e = set_smem_attrs<T, LOG>(D, sms)) != cudaSuccess) return e;
     CUHPX_ATTR(7) CUHPX_ATTR(8) CUHPX_ATTR(9) CUHPX_ATTR(10) CUHPX_ATTR(11) CUHPX_ATTR(12) CUHPX_ATTR(13)
 #undef CUHPX_ATTR
+    if constexpr (sizeof(T) == 8) {
+        if ((e = cudaFuncSetAttribute(ring_pow2_half_analysis_kernel<T, HALVES_LOG - 1>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                      (int)half_smem_bytes<T, HALVES_LOG - 1>(1)))) return e;
+        if ((e = cudaFuncSetAttribute(ring_pow2_teams_synthesis_kernel<T, HALVES_LOG - 1>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                      (int)half_smem_bytes<T, HALVES_LOG - 1>(2)))) return e;
+    }
     // direct synthesis kernel: [twiddles N][G: mcut + 1]; the largest the SM can hold (launches check their own need)
     return cudaFuncSetAttribute(ring_direct_synthesis_kernel<T>, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024);
 }
@@ -1129,8 +1336,24 @@ static void launch_class(const DevPlan& P, const FftCall& C, T* map, const doubl
     if (!F.pow2[LOG].empty()) {
         tabs.pf = C.D->pf[C.ti][A][0][LOG];
         const RingInfo* items = (const RingInfo*)(C.base + F.off_pow2[LOG]);
-        const dim3 grid((unsigned)F.pow2[LOG].size(), P.batch);
-        if (ANALYSIS)
+        const unsigned ni = (unsigned)F.pow2[LOG].size();
+        const dim3 grid(ni, P.batch);
+        bool done = false;
+        if constexpr (LOG == HALVES_LOG && sizeof(T) == 8) {
+            // fp64 rings of 2^14 pixels: half-ring work items / two teams per CTA (unless orders beyond the ring's
+            // Nyquist frequency are wanted: those need both halves of the spectrum in one place)
+            if (F.pow2_max_mcut <= (2 << LOG) / 2) {
+                if (ANALYSIS)
+                    ring_pow2_half_analysis_kernel<T, LOG - 1><<<dim3(2 * ni, P.batch), FftPlan<LOG - 1>::NT, half_smem_bytes<T, LOG - 1>(1), main_st>>>(
+                        P, items, map, w, use_w, tabs);
+                else
+                    ring_pow2_teams_synthesis_kernel<T, LOG - 1><<<grid, 2 * FftPlan<LOG - 1>::NT, half_smem_bytes<T, LOG - 1>(2), main_st>>>(
+                        P, items, map, w, use_w, tabs);
+                done = true;
+            }
+        }
+        if (done) {
+        } else if (ANALYSIS)
             ring_pow2_analysis_kernel<T, LOG><<<grid, FftPlan<LOG>::NT, fft_smem_bytes<T, LOG>(false), main_st>>>(P, items, map, w, use_w, tabs);
         else
             ring_pow2_synthesis_kernel<T, LOG><<<grid, FftPlan<LOG>::NT, fft_smem_bytes<T, LOG>(false), main_st>>>(P, items, map, w, use_w, tabs);
