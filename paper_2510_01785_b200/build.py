@@ -11,8 +11,9 @@ import sys
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libcuhpx.so")
-SOURCES = ["plan.cu", "legendre.cu", "ring_fft.cu", "reorder.cu"]
+SOURCES = ["plan.cu", "legendre.cu", "legendre_tc.cu", "ring_fft.cu", "reorder.cu"]
 HEADERS = [os.path.join(CSRC, "cuhpx_internal.h"), os.path.join(CSRC, "block_fft.cuh"),
+           os.path.join(CSRC, "legendre_common.cuh"), os.path.join(CSRC, "tc_common.cuh"),
            os.path.join(HERE, "..", "include", "cuhpx.h")]
 NVCC_FLAGS = [
     "-O3", "-std=c++17", "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo",

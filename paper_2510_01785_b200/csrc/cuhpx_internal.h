@@ -67,6 +67,10 @@ struct DevPlan {
     // scratch
     void* spectra;           // [batch][nrings][mstride] complex<T>
     void* partial;           // [nchunk_max][batch][nalm] complex<T> (analysis partial sums), or null
+    // tensor-core Legendre kernels (fp32, batch >= 8; legendre_tc.cu): operand images built per call
+    const long long* tc_prefix;  // [mmax + 2] stages of 32 degrees before order m
+    void* tc_images;             // [channel group][stage] images (alpha + B-operand tiles), or null
+    int tc_nb;                   // channels per group (0: tensor-core path not planned)
     int nchunk_max;          // ring-pair chunks per m in the Legendre analysis grid
     int chunk_pairs;         // ring pairs per chunk
 };
@@ -94,7 +98,8 @@ struct HostPlan {
     size_t workspace_bytes;
     // table offsets inside the workspace
     size_t off_y, off_lshi, off_lslo, off_ringN, off_start, off_shifted, off_mcut, off_prefhi, off_preflo, off_jmin;
-    size_t off_fft, fft_bytes, off_alpha, off_scale, off_spectra, off_partial;
+    size_t off_fft, fft_bytes, off_alpha, off_scale, off_spectra, off_partial, off_tcprefix, off_tcimages;
+    std::vector<long long> h_tcprefix;
     std::vector<int> h_ringN, h_mcut, h_jmin, h_shifted;
     std::vector<long long> h_start;
     std::vector<double> h_y, h_lshi, h_lslo, h_prefhi, h_preflo, h_weight;  // h_weight: built-in quadrature weights per ring
@@ -115,6 +120,9 @@ inline int ilog2_ceil(long long v) {
 inline bool is_pow2(long long v) { return v > 0 && (v & (v - 1)) == 0; }
 
 // ------------------------------------------------------------------ launchers (each returns a cudaError_t)
+// tensor-core Legendre path: channels per group for this (dtype, batch) or 0, and bytes of one stage image
+int legendre_tc_group(cuhpx_dtype_t dt, int batch);
+size_t legendre_tc_image_bytes(int nb);
 cudaError_t launch_legendre_coeff(int lmax, int mmax, double* alpha, double* scale, cudaStream_t st);
 cudaError_t launch_legendre_analysis(const HostPlan& hp, const DevPlan& P, void* d_alm, int adjoint, cudaStream_t st);
 cudaError_t launch_legendre_synthesis(const HostPlan& hp, const DevPlan& P, const void* d_alm, int adjoint, cudaStream_t st);

@@ -12,58 +12,13 @@
 #include <math.h>
 
 #include "cuhpx_internal.h"
+#include "legendre_common.cuh"
 
 namespace cuhpx {
 
 constexpr int LEG_THREADS = 256;
 constexpr int LEG_WARPS = LEG_THREADS / 32;
 constexpr int CT = 64;  // recurrence-coefficient tile (l values per __syncthreads)
-
-template <typename T> struct Vec2;
-template <> struct Vec2<float> { using type = float2; };
-template <> struct Vec2<double> { using type = double2; };
-
-// Exponent windows of the scaled recurrence.  true lambda = val * 2^(K * sc), sc <= 0.  A ring is "inactive"
-// while sc < 0; then |true lambda| < 2^(THR + 56 - K): 2^-200 (fp64) / 2^-44 (fp32 outputs), i.e. it cannot
-// change the result.  56 = log2 of the largest growth over the 8 steps between two checks.
-template <typename T> struct ScaleCfg;
-template <> struct ScaleCfg<double> { static constexpr int THR = 256, K = 512; };
-template <> struct ScaleCfg<float> { static constexpr int THR = 60, K = 160; };
-__host__ __device__ constexpr double pow2c(int e) {
-    double v = 1.0;
-    for (int i = 0; i < (e < 0 ? -e : e); ++i) v = e < 0 ? v * 0.5 : v * 2.0;
-    return v;
-}
-constexpr int CHECK_EVERY = 8;  // l steps between rescale checks (must divide CT and be a multiple of LT)
-
-// log2|lambda_mm(theta_j)| = pref[m] + m log2 sin(theta_j), evaluated in double-double so that the seed is
-// good to ~1e-16 relative even when the exponent is in the thousands.
-template <typename T>
-__device__ __forceinline__ void lambda_seed(int m, double pref_hi, double pref_lo, double ls_hi, double ls_lo,
-                                            double& val, int& sc) {
-    const double dm = (double)m;
-    const double p = dm * ls_hi;
-    const double pe = fma(dm, ls_hi, -p);
-    const double s = p + pref_hi;
-    const double bb = s - p;
-    const double se = (p - (s - bb)) + (pref_hi - bb);
-    const double lo = pe + se + fma(dm, ls_lo, pref_lo);
-    const double n = rint(s + lo);
-    const double f = (s - n) + lo;
-    const double mant = exp2(f);
-    int ni = (int)fmax(n, -2.0e9);
-    sc = 0;
-    constexpr int THR = ScaleCfg<T>::THR, K = ScaleCfg<T>::K;
-    if (ni < THR - K) {
-        // floor((ni - THR) / K) + 1, written for negative numerators
-        const int num = ni - THR;
-        const int fl = -((-num + K - 1) / K);
-        sc = fl + 1;
-        ni -= K * sc;
-    }
-    val = scalbn(mant, ni);
-    if (m & 1) val = -val;
-}
 
 // ------------------------------------------------------------------ recurrence coefficients (built once per plan)
 // Eq. 16 reads lambda_l = A_l x lambda_{l-1} + B_l lambda_{l-2}, A_l = sqrt((4l^2-1)/(l^2-m^2)),
@@ -139,13 +94,6 @@ cudaError_t launch_legendre_coeff(int lmax, int mmax, double* alpha, double* sca
     return cudaGetLastError();
 }
 
-struct LegArgs {
-    DevPlan p;
-    const void* in;  // analysis: unused (spectra from plan); synthesis: alm
-    void* out;       // analysis: alm or partial; synthesis: unused
-    int adjoint;
-    int to_partial;  // analysis: write [chunk][batch][nalm] partial sums
-};
 
 // sum NV per-thread values across the 32 lanes; afterwards lane L holds, in v[0 .. Q-1], the totals of the
 // values with index Q * (L >> SH) + q, Q = max(NV / 32, 1), SH = max(5 - log2 NV, 0).
@@ -1298,6 +1246,9 @@ static cudaError_t run_synthesis_f32x2(const HostPlan& hp, const DevPlan& P, con
 cudaError_t launch_legendre_synthesis(const HostPlan& hp, const DevPlan& P, const void* d_alm, int adjoint, cudaStream_t st) {
     if (hp.dtype == CUHPX_F64) return run_synthesis_cfg<double, 1, 4, 128>(hp, P, d_alm, adjoint, st);
     if (P.batch >= 8) {
+        // tensor-core kernel (legendre_tc.cu): lambda goes to tensor memory, the contraction to tcgen05.mma
+        const cudaError_t e = launch_legendre_synthesis_tc(hp, P, d_alm, adjoint, st);
+        if (e != cudaErrorNotSupported) return e;
         // packed-FMA kernels, 8 channels per CTA; short degree ranges want more, smaller CTAs in flight
         return P.lmax < 512 ? run_synthesis_f32x2<8, 1, 256, 3>(hp, P, d_alm, adjoint, st)
                                : run_synthesis_f32x2<8, 2, 128, 3>(hp, P, d_alm, adjoint, st);

@@ -189,6 +189,16 @@ HostPlan* make_plan(int nside, int lmax, int mmax, int batch, cuhpx_dtype_t dt) 
     hp->off_spectra = take(csize * (size_t)d.batch * d.nrings * d.mstride);
     hp->off_partial = o;
     if (d.nchunk_max > 1) take(csize * (size_t)d.nchunk_max * d.batch * d.nalm);
+    // tensor-core Legendre path: per-call operand images (stages of 32 degrees, see legendre_tc.cu)
+    d.tc_nb = legendre_tc_group(dt, batch);
+    hp->off_tcprefix = hp->off_tcimages = 0;
+    if (d.tc_nb > 0) {
+        hp->h_tcprefix.assign(mmax + 2, 0);
+        for (int m = 0; m <= mmax; ++m) hp->h_tcprefix[m + 1] = hp->h_tcprefix[m] + (lmax - m + 1 + 31) / 32;
+        hp->off_tcprefix = take(sizeof(long long) * (mmax + 2));
+        const size_t groups = (size_t)(batch + d.tc_nb - 1) / d.tc_nb;
+        hp->off_tcimages = take(groups * (size_t)hp->h_tcprefix[mmax + 1] * legendre_tc_image_bytes(d.tc_nb));
+    }
     hp->workspace_bytes = o;
     return hp;
 }
@@ -273,6 +283,8 @@ DevPlan HostPlan::resolve(void* ws) const {
     P.coef_scale = (const double*)(base + off_scale);
     P.spectra = base + off_spectra;
     P.partial = d.nchunk_max > 1 ? base + off_partial : nullptr;
+    P.tc_prefix = d.tc_nb > 0 ? (const long long*)(base + off_tcprefix) : nullptr;
+    P.tc_images = d.tc_nb > 0 ? base + off_tcimages : nullptr;
     return P;
 }
 
@@ -361,6 +373,7 @@ int cuhpx_workspace_init(int nside, int lmax, int mmax, int batch, cuhpx_dtype_t
     up(hp->off_prefhi, hp->h_prefhi.data(), sizeof(double) * (mmax + 1));
     up(hp->off_preflo, hp->h_preflo.data(), sizeof(double) * (mmax + 1));
     up(hp->off_jmin, hp->h_jmin.data(), sizeof(int) * (mmax + 1));
+    if (d.tc_nb > 0) up(hp->off_tcprefix, hp->h_tcprefix.data(), sizeof(long long) * (mmax + 2));
     if (e == cudaSuccess)
         e = launch_legendre_coeff(lmax, mmax, (double*)(base + hp->off_alpha), (double*)(base + hp->off_scale), st);
     if (e == cudaSuccess) e = fft_build_tables(*hp, base + hp->off_fft, st);
@@ -421,7 +434,7 @@ int cuhpx_plan_stats(int nside, int lmax, int mmax, int batch, cuhpx_dtype_t dty
     fft_stage_stats(*hp, &fl, &tb);
     st[0] = fl;
     st[1] = d.nchunk_max > 1 ? 2 : 1;
-    st[2] = 1;
+    st[2] = d.tc_nb > 0 ? 2 : 1;  // tensor-core synthesis: operand images + main kernel
     for (int m = 0; m <= d.mmax; ++m) st[3] += (double)(d.lmax - m + 1) * (double)(d.npairs - hp->h_jmin[m]);
     st[4] = (double)d.nalm * (double)d.npairs;
     for (int r = 0; r < d.nrings; ++r) st[5] += hp->h_mcut[r < d.nrings - 1 - r ? r : d.nrings - 1 - r] + 1;
