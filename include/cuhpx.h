@@ -115,6 +115,22 @@ int cuhpx_map2alm_iter(int nside, int lmax, int mmax, int batch, cuhpx_dtype_t d
                        const double* d_ring_weights, int n_iter, void* d_scratch_map, void* d_scratch_alm,
                        void* d_workspace, size_t workspace_bytes, cuhpx_stream_t stream);
 
+/* ---- ring quadrature weights ("cuHPX adopts ring weights as the default"; the paper
+ * takes the values from the HEALPix data distribution, which is not available here -- DESIGN.md reading R11).
+ * Writes 4 nside - 1 doubles w_i (rings north to south, including the 4 pi / Npix factor, i.e. directly usable as
+ * d_ring_weights of cuhpx_map2alm / cuhpx_map2alm_iter / cuhpx_map2alm_adjoint) such that the m = 0 quadrature of Eq. 26
+ * is exact:  sum_i w_i N_i lambda_l0(theta_i) = sqrt(4 pi) delta_l0  for every l <= lmax_w  (so a_l0 of a zonal map
+ * band-limited to lmax_w / 2 is recovered to rounding), choosing among all such weights the one closest to equal weights,
+ * min sum_i N_i (w_i - 4 pi / Npix)^2; the result is north/south symmetric.  lmax_w <= 0 selects the default 3 nside;
+ * lmax_w > 3 nside is CUHPX_EINVAL (the Gram matrix of the zonal harmonics on the rings degenerates beyond).
+ * Solved on the device with the m = 0 Legendre stages of the transform itself (conjugate gradients, ~50 iterations);
+ * d_workspace: caller-owned DEVICE scratch of cuhpx_ring_weights_workspace_bytes() bytes, overwritten.  SYNCHRONISES
+ * `stream` (table building + one read-back of the final residual); returns CUHPX_EUNSUPPORTED if the constraints are
+ * not met to 1e-11. */
+size_t cuhpx_ring_weights_workspace_bytes(int nside, int lmax_w);
+int cuhpx_ring_weights(int nside, int lmax_w, double* d_weights, void* d_workspace, size_t workspace_bytes,
+                       cuhpx_stream_t stream);
+
 /* ---- layout reordering NESTED <-> RING (paper section III-B, via (x, y, f) P:118-123)
  * NESTED: index = f nside^2 + Z-order (Morton) interleave of (x, y) inside base face f (x on the even bits), P:109;
  * RING: as everywhere else in this header.  d_in / d_out: [batch][npix] elements of `dtype` (moved as bits,

@@ -24,7 +24,7 @@ EXPORTS = [
     "cuhpx_alm2map_adjoint", "cuhpx_map2alm_adjoint", "cuhpx_spectra_stride", "cuhpx_spectra_offset",
     "cuhpx_plan_mcut", "cuhpx_analysis_fft_stage", "cuhpx_analysis_legendre_stage",
     "cuhpx_synthesis_legendre_stage", "cuhpx_synthesis_fft_stage", "cuhpx_fma_peak_probe", "cuhpx_plan_stats",
-    "cuhpx_map2alm_iter", "cuhpx_reorder", "cuhpx_nest2ring_index", "cuhpx_alm_resize",
+    "cuhpx_map2alm_iter", "cuhpx_ring_weights_workspace_bytes", "cuhpx_ring_weights", "cuhpx_reorder", "cuhpx_nest2ring_index", "cuhpx_alm_resize",
 ]
 CUHPX_NEST2RING, CUHPX_RING2NEST = 0, 1
 
@@ -63,6 +63,9 @@ def _load() -> ctypes.CDLL:
     lib.cuhpx_map2alm_adjoint.argtypes = [i, i, i, i, i, vp, vp, vp, vp, sz, vp]
     lib.cuhpx_map2alm_iter.argtypes = [i, i, i, i, i, vp, vp, vp, i, vp, vp, vp, sz, vp]
     lib.cuhpx_reorder.argtypes = [i, i, i, i, vp, vp, vp]
+    lib.cuhpx_ring_weights_workspace_bytes.argtypes = [i, i]
+    lib.cuhpx_ring_weights_workspace_bytes.restype = sz
+    lib.cuhpx_ring_weights.argtypes = [i, i, vp, vp, sz, vp]
     lib.cuhpx_alm_resize.argtypes = [i, i, i, i, i, i, vp, vp, vp]
     lib.cuhpx_nest2ring_index.restype = ctypes.c_longlong
     lib.cuhpx_nest2ring_index.argtypes = [i, ctypes.c_longlong]
@@ -198,6 +201,27 @@ def cuhpx_map2alm_adjoint(nside, lmax, mmax, batch, dtype, d_galm, d_gmap, d_rin
     p, n = _ws_args(workspace)
     _check(_lib.cuhpx_map2alm_adjoint(nside, lmax, mmax, batch, dtype, _dev_ptr(d_galm), _dev_ptr(d_gmap),
                                       _dev_ptr(d_ring_weights), p, n, _stream_ptr(stream)), "cuhpx_map2alm_adjoint")
+
+
+def cuhpx_ring_weights_workspace_bytes(nside: int, lmax_w: int = 0) -> int:
+    return int(_lib.cuhpx_ring_weights_workspace_bytes(nside, lmax_w))
+
+
+def cuhpx_ring_weights(nside, lmax_w, d_weights, workspace, stream=None) -> None:
+    p, n = _ws_args(workspace)
+    _check(_lib.cuhpx_ring_weights(nside, lmax_w, _dev_ptr(d_weights), p, n, _stream_ptr(stream)), "cuhpx_ring_weights")
+
+
+def ring_weights(nside: int, lmax_w: int = 0, device="cuda") -> torch.Tensor:
+    """Ring quadrature weights [4 nside - 1] (fp64, device) exact for the m = 0 modes up to lmax_w (default 3 nside)."""
+    nbytes = cuhpx_ring_weights_workspace_bytes(nside, lmax_w)
+    if nbytes == 0:
+        raise CuhpxError(1, "cuhpx_ring_weights_workspace_bytes")
+    ws = torch.empty(nbytes, dtype=torch.uint8, device=device)
+    w = torch.empty(4 * nside - 1, dtype=torch.float64, device=device)
+    with torch.cuda.device(w.device):
+        cuhpx_ring_weights(nside, lmax_w, w, ws)
+    return w
 
 
 def cuhpx_reorder(nside, batch, dtype, direction, d_in, d_out, stream=None) -> None:

@@ -151,6 +151,10 @@ long long nest_to_ring_index(int nside, long long ipnest);
 cudaError_t launch_alm_resize(int lmax_in, int mmax_in, int lmax_out, int mmax_out, int batch, cuhpx_dtype_t dt,
                               const void* in, void* out, cudaStream_t st);
 
+// ring quadrature weights (ring_weights.cu): scratch layout [transform workspace][CG vectors]; the solve synchronises
+size_t ring_weights_scratch_bytes(size_t transform_ws_bytes, int lmax_w);
+cudaError_t ring_weights_solve(const HostPlan& hp, const DevPlan& P, char* vec_base, double* d_w, double* h_resid, cudaStream_t st);
+
 cudaError_t fma_peak_probe(cuhpx_dtype_t dt, int iters, float* ms, double* count, cudaStream_t st);
 
 }  // namespace cuhpx

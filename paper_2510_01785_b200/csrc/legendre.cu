@@ -10,6 +10,7 @@
 // registers.  cos(theta) enters as x p = p - y p with y = 1 - cos(theta) (R3).
 #include <cuda_runtime.h>
 #include <math.h>
+#include <stdlib.h>
 
 #include "cuhpx_internal.h"
 #include "legendre_common.cuh"
@@ -157,8 +158,8 @@ __device__ __forceinline__ void warp_reduce_split(T (&v)[NV], int lane) {
 }
 
 // SEQ: one CTA walks the ring chunks of its order m and accumulates a_lm in place (no partial arrays / combine kernel)
-template <typename T, int BT, int R, int LT, int NT, int GL = GROUP_L, bool SEQ = false>
-__global__ void __launch_bounds__(NT, 384 / NT) legendre_analysis_kernel(LegArgs a) {
+template <typename T, int BT, int R, int LT, int NT, int GL = GROUP_L, bool SEQ = false, int MINB = 384 / NT>
+__global__ void __launch_bounds__(NT, MINB) legendre_analysis_kernel(LegArgs a) {
     using T2 = typename Vec2<T>::type;
     constexpr int NW = NT / 32;
     constexpr int NV = LT * BT * 2;
@@ -240,13 +241,23 @@ __global__ void __launch_bounds__(NT, 384 / NT) legendre_analysis_kernel(LegArgs
     bool warp_active = __any_sync(0xffffffffu, nact > 0);
     // alpha of the steps that produce degrees l = m + t0 + 1 + i; the next tile is fetched into a register while
     // the current one is consumed, so no global-load latency sits between two tiles
-    double nextA = (tid < CT && 1 + tid < nl) ? P.coef_alpha[abase + m + 1 + tid] : 0.0;
+    constexpr int APT = (CT + NT - 1) / NT;  // alpha values a thread carries (CTAs may be narrower than the tile)
+    double nextA[APT];
+#pragma unroll
+    for (int q = 0; q < APT; ++q) {
+        const int i = tid + q * NT;
+        nextA[q] = (i < CT && 1 + i < nl) ? P.coef_alpha[abase + m + 1 + i] : 0.0;
+    }
     constexpr int NOUT = (TPG * NV + NT - 1) / NT;  // output elements per thread and group (cross-warp sums)
     for (int t0 = 0; t0 < nl; t0 += CT) {
         const int cb = (t0 / CT) & 1;
-        if (tid < CT) {
-            sA[cb][tid] = nextA;
-            nextA = (t0 + CT + 1 + tid < nl) ? P.coef_alpha[abase + m + t0 + CT + 1 + tid] : 0.0;
+#pragma unroll
+        for (int q = 0; q < APT; ++q) {
+            const int i = tid + q * NT;
+            if (i < CT) {
+                sA[cb][i] = nextA[q];
+                nextA[q] = (t0 + CT + 1 + i < nl) ? P.coef_alpha[abase + m + t0 + CT + 1 + i] : 0.0;
+            }
         }
         __syncthreads();
         const int tend = min(CT, nl - t0);
@@ -1100,7 +1111,7 @@ __global__ void __launch_bounds__(NT, MINB) legendre_synthesis_f32x2_kernel(LegA
 // R (ring pairs per thread) and LT (l values per reduction tile) per instantiation.
 template <typename T, int BT> struct LegCfg;
 // analysis: NT threads x R ring pairs = one chunk; synthesis: LEG_THREADS x RS
-template <> struct LegCfg<double, 1> { static constexpr int NT = 128, R = 8, LT = 8, RS = 4, NTS = 256; };
+template <> struct LegCfg<double, 1> { static constexpr int NT = 64, R = 7, LT = 8, RS = 4, NTS = 256; };
 template <> struct LegCfg<float, 1> { static constexpr int NT = 128, R = 8, LT = 8, RS = 4, NTS = 256; };
 template <> struct LegCfg<float, 4> { static constexpr int NT = 128, R = 4, LT = 4, RS = 2, NTS = 256; };
 
@@ -1153,7 +1164,7 @@ static cudaError_t run_synthesis(const HostPlan& hp, const DevPlan& P, const voi
     return cudaGetLastError();
 }
 
-template <typename T, int BT, int R, int LT, int NT, int GL, bool SEQ = false>
+template <typename T, int BT, int R, int LT, int NT, int GL, bool SEQ = false, int MINB = 384 / NT>
 static cudaError_t run_analysis_cfg(const HostPlan& hp, const DevPlan& P, void* d_alm, int adjoint, cudaStream_t st) {
     LegArgs a;
     a.p = P;
@@ -1162,7 +1173,7 @@ static cudaError_t run_analysis_cfg(const HostPlan& hp, const DevPlan& P, void* 
     a.to_partial = !SEQ && P.nchunk_max > 1;
     a.out = a.to_partial ? P.partial : d_alm;
     dim3 grid(P.mmax + 1, SEQ ? 1 : P.nchunk_max, (P.batch + BT - 1) / BT);
-    legendre_analysis_kernel<T, BT, R, LT, NT, GL, SEQ><<<grid, NT, 0, st>>>(a);
+    legendre_analysis_kernel<T, BT, R, LT, NT, GL, SEQ, MINB><<<grid, NT, 0, st>>>(a);
     cudaError_t e = cudaGetLastError();
     if (e != cudaSuccess) return e;
     if (a.to_partial) {
@@ -1223,7 +1234,9 @@ static cudaError_t run_analysis_gemm(const HostPlan& hp, const DevPlan& P, void*
 // Configurations below are the winners of sweeps on B200 (profiles/r1_legendre_tuning.md).
 cudaError_t launch_legendre_analysis(const HostPlan& hp, const DevPlan& P, void* d_alm, int adjoint, cudaStream_t st) {
     // in-place accumulation over ring chunks (SEQ): cfg5 88.3 -> 87.0 ms, 3.7 GB of partial writes and 4.3 GB of workspace gone
-    if (hp.dtype == CUHPX_F64) return run_analysis_cfg<double, 1, 8, 8, 128, 64, true>(hp, P, d_alm, adjoint, st);
+    // fp64: 2-warp CTAs of 7 ring pairs per thread (r2 sweep over NT 32..128, R 5..8, resident CTAs: 80.9 ms at nside 4096
+    // against 87.0 ms for the r1 shape 128 x 8; a software-pipelined butterfly was tried and was slower, 86-91 ms)
+    if (hp.dtype == CUHPX_F64) return run_analysis_cfg<double, 1, 7, 8, 64, 64, true>(hp, P, d_alm, adjoint, st);
     if (P.batch >= 5) return run_analysis_gemm(hp, P, d_alm, adjoint, st);
     if (P.batch >= 4) return run_analysis<float, 4>(hp, P, d_alm, adjoint, st);
     return run_analysis<float, 1>(hp, P, d_alm, adjoint, st);

@@ -573,6 +573,32 @@ int cuhpx_map2alm_iter(int nside, int lmax, int mmax, int batch, cuhpx_dtype_t d
     return CUHPX_OK;
 }
 
+static int ring_weights_lmax(int nside, int lmax_w) { return lmax_w > 0 ? lmax_w : 3 * nside; }
+
+size_t cuhpx_ring_weights_workspace_bytes(int nside, int lmax_w) {
+    const int lw = ring_weights_lmax(nside, lmax_w);
+    if (!valid_args(nside, lw, 0, 1, CUHPX_F64) || lw > 3 * nside || !fft_supported(4 * nside, CUHPX_F64)) return 0;
+    return ring_weights_scratch_bytes(get_plan(nside, lw, 0, 1, CUHPX_F64)->workspace_bytes, lw);
+}
+
+int cuhpx_ring_weights(int nside, int lmax_w, double* d_weights, void* ws, size_t ws_bytes, cuhpx_stream_t stream) {
+    const int lw = ring_weights_lmax(nside, lmax_w);
+    if (!valid_args(nside, lw, 0, 1, CUHPX_F64) || lw > 3 * nside) return CUHPX_EINVAL;
+    if (!d_weights || !ws || ((uintptr_t)d_weights & 7) || ((uintptr_t)ws & 15)) return CUHPX_EINVAL;
+    if (!fft_supported(4 * nside, CUHPX_F64)) return CUHPX_EUNSUPPORTED;
+    PlanRef hp = get_plan(nside, lw, 0, 1, CUHPX_F64);
+    const size_t need = ring_weights_scratch_bytes(hp->workspace_bytes, lw);
+    if (ws_bytes < need) return CUHPX_EWORKSPACE;
+    if (overlap(d_weights, sizeof(double) * (size_t)hp->d.nrings, ws, need)) return CUHPX_EINVAL;
+    const int rc = cuhpx_workspace_init(nside, lw, 0, 1, CUHPX_F64, ws, hp->workspace_bytes, stream);
+    if (rc != CUHPX_OK) return rc;
+    double resid = 0.0;
+    char* vec = (char*)ws + (hp->workspace_bytes + 255) / 256 * 256;
+    CUDA_OR_FAIL(ring_weights_solve(*hp, hp->resolve(ws), vec, d_weights, &resid, (cudaStream_t)stream));
+    // the constraints hold to rounding when the conjugate gradients have converged (they do for lmax_w <= 3 nside)
+    return resid <= 1e-11 ? CUHPX_OK : CUHPX_EUNSUPPORTED;
+}
+
 int cuhpx_reorder(int nside, int batch, cuhpx_dtype_t dt, int direction, const void* d_in, void* d_out,
                   cuhpx_stream_t stream) {
     if (nside < 1 || !is_pow2(nside) || nside > (1 << 13) || batch < 1 || batch > MAX_BATCH || (dt != CUHPX_F32 && dt != CUHPX_F64))
