@@ -59,6 +59,9 @@ extern "C" {
 
 typedef enum { CUHPX_F32 = 0, CUHPX_F64 = 1 } cuhpx_dtype_t;
 
+/* ring grids the two stages can run on (cuhpx_grid_* calls below; the calls without "grid" are HEALPix) */
+typedef enum { CUHPX_GRID_HEALPIX = 0, CUHPX_GRID_GAUSS_LEGENDRE = 1, CUHPX_GRID_EQUIANGULAR = 2 } cuhpx_grid_t;
+
 typedef enum {
     CUHPX_OK = 0,
     CUHPX_EINVAL = 1,       /* bad nside / lmax / mmax / batch / dtype, null or misaligned pointer */
@@ -149,6 +152,35 @@ long long cuhpx_nest2ring_index(int nside, long long ipnest);
  * cuhpx_map2alm (nside_a) -> cuhpx_alm_resize -> cuhpx_alm2map (nside_b). */
 int cuhpx_alm_resize(int lmax_in, int mmax_in, int lmax_out, int mmax_out, int batch, cuhpx_dtype_t dtype,
                      const void* d_alm_in, void* d_alm_out, cuhpx_stream_t stream);
+
+/* ---- the same transforms on iso-latitude grids (the two-stage structure "generalizes to
+ * ... Legendre-Gauss or Lobatto grids", used there for regridding through torch-harmonics).  A grid is nlat rings, north
+ * to south, of nlon equally spaced pixels each, the first at phi = 0; map layout [batch][nlat * nlon], ring-major.
+ *   CUHPX_GRID_GAUSS_LEGENDRE: cos(theta_k) = the nlat roots of P_nlat, per-pixel weight w_k^GL 2 pi / nlon: analysis is
+ *       exact for band limit lmax <= nlat - 1, mmax <= (nlon - 1) / 2, so map2alm(alm2map(a)) = a to rounding
+ *   CUHPX_GRID_EQUIANGULAR:    theta_k = pi (k + 1/2) / nlat with Fejer's first-rule weights (exact for zonal
+ *       polynomials of degree <= nlat - 1, i.e. a round trip is exact for lmax <= (nlat - 1) / 2)
+ *   CUHPX_GRID_HEALPIX:        nlat = nside, nlon ignored: identical to the calls above
+ * nlon must be a power of two, 4 <= nlon <= 16384; 1 <= nlat <= 16384.  d_ring_weights: nlat doubles or NULL = the grid's
+ * own quadrature weights.  Every other convention (alm layout, ownership, workspace header, asynchrony, error codes,
+ * adjoint inner products) is that of the HEALPix calls; the kernels are the same, only the ring table differs. */
+size_t cuhpx_grid_npix(int grid, int nlat, int nlon);
+/* cos(theta) and the per-pixel quadrature weight of ring 1 .. nlat (host only; not for CUHPX_GRID_HEALPIX: cuhpx_ring_info) */
+int cuhpx_grid_ring_info(int grid, int nlat, int nlon, int ring, double* cos_theta, double* weight);
+size_t cuhpx_grid_workspace_bytes(int grid, int nlat, int nlon, int lmax, int mmax, int batch, cuhpx_dtype_t dtype);
+int cuhpx_grid_workspace_init(int grid, int nlat, int nlon, int lmax, int mmax, int batch, cuhpx_dtype_t dtype,
+                              void* d_workspace, size_t workspace_bytes, cuhpx_stream_t stream);
+int cuhpx_grid_alm2map(int grid, int nlat, int nlon, int lmax, int mmax, int batch, cuhpx_dtype_t dtype, const void* d_alm,
+                       void* d_map, void* d_workspace, size_t workspace_bytes, cuhpx_stream_t stream);
+int cuhpx_grid_map2alm(int grid, int nlat, int nlon, int lmax, int mmax, int batch, cuhpx_dtype_t dtype, const void* d_map,
+                       void* d_alm, const double* d_ring_weights, void* d_workspace, size_t workspace_bytes,
+                       cuhpx_stream_t stream);
+int cuhpx_grid_alm2map_adjoint(int grid, int nlat, int nlon, int lmax, int mmax, int batch, cuhpx_dtype_t dtype,
+                               const void* d_gmap, void* d_galm, void* d_workspace, size_t workspace_bytes,
+                               cuhpx_stream_t stream);
+int cuhpx_grid_map2alm_adjoint(int grid, int nlat, int nlon, int lmax, int mmax, int batch, cuhpx_dtype_t dtype,
+                               const void* d_galm, void* d_gmap, const double* d_ring_weights, void* d_workspace,
+                               size_t workspace_bytes, cuhpx_stream_t stream);
 
 /* ---- the two stages of each direction, individually, for per-stage
  * measurement and stage-level parity tests; same conventions and checks as the operators.  The ring spectra live

@@ -24,9 +24,12 @@ EXPORTS = [
     "cuhpx_alm2map_adjoint", "cuhpx_map2alm_adjoint", "cuhpx_spectra_stride", "cuhpx_spectra_offset",
     "cuhpx_plan_mcut", "cuhpx_analysis_fft_stage", "cuhpx_analysis_legendre_stage",
     "cuhpx_synthesis_legendre_stage", "cuhpx_synthesis_fft_stage", "cuhpx_fma_peak_probe", "cuhpx_plan_stats",
+    "cuhpx_grid_npix", "cuhpx_grid_ring_info", "cuhpx_grid_workspace_bytes", "cuhpx_grid_workspace_init",
+    "cuhpx_grid_alm2map", "cuhpx_grid_map2alm", "cuhpx_grid_alm2map_adjoint", "cuhpx_grid_map2alm_adjoint",
     "cuhpx_map2alm_iter", "cuhpx_ring_weights_workspace_bytes", "cuhpx_ring_weights", "cuhpx_reorder", "cuhpx_nest2ring_index", "cuhpx_alm_resize",
 ]
 CUHPX_NEST2RING, CUHPX_RING2NEST = 0, 1
+CUHPX_GRID_HEALPIX, CUHPX_GRID_GAUSS_LEGENDRE, CUHPX_GRID_EQUIANGULAR = 0, 1, 2
 
 
 class CuhpxError(RuntimeError):
@@ -63,6 +66,16 @@ def _load() -> ctypes.CDLL:
     lib.cuhpx_map2alm_adjoint.argtypes = [i, i, i, i, i, vp, vp, vp, vp, sz, vp]
     lib.cuhpx_map2alm_iter.argtypes = [i, i, i, i, i, vp, vp, vp, i, vp, vp, vp, sz, vp]
     lib.cuhpx_reorder.argtypes = [i, i, i, i, vp, vp, vp]
+    lib.cuhpx_grid_npix.argtypes = [i, i, i]
+    lib.cuhpx_grid_npix.restype = sz
+    lib.cuhpx_grid_ring_info.argtypes = [i, i, i, i, vp, vp]
+    lib.cuhpx_grid_workspace_bytes.argtypes = [i, i, i, i, i, i, i]
+    lib.cuhpx_grid_workspace_bytes.restype = sz
+    lib.cuhpx_grid_workspace_init.argtypes = [i, i, i, i, i, i, i, vp, sz, vp]
+    lib.cuhpx_grid_alm2map.argtypes = [i, i, i, i, i, i, i, vp, vp, vp, sz, vp]
+    lib.cuhpx_grid_map2alm.argtypes = [i, i, i, i, i, i, i, vp, vp, vp, vp, sz, vp]
+    lib.cuhpx_grid_alm2map_adjoint.argtypes = [i, i, i, i, i, i, i, vp, vp, vp, sz, vp]
+    lib.cuhpx_grid_map2alm_adjoint.argtypes = [i, i, i, i, i, i, i, vp, vp, vp, vp, sz, vp]
     lib.cuhpx_ring_weights_workspace_bytes.argtypes = [i, i]
     lib.cuhpx_ring_weights_workspace_bytes.restype = sz
     lib.cuhpx_ring_weights.argtypes = [i, i, vp, vp, sz, vp]
@@ -399,3 +412,64 @@ class Transform:
         gmap = torch.empty(self.batch, self.npix, dtype=self.rdtype, device=self.device) if out is None else out
         cuhpx_map2alm_adjoint(*self._args(), galm, gmap, self.ring_weights, self.workspace)
         return gmap
+
+
+# ---------------------------------------------------------------- iso-latitude grids
+def cuhpx_grid_npix(grid: int, nlat: int, nlon: int) -> int:
+    return int(_lib.cuhpx_grid_npix(grid, nlat, nlon))
+
+
+def cuhpx_grid_ring_info(grid: int, nlat: int, nlon: int, ring: int):
+    c, w = ctypes.c_double(), ctypes.c_double()
+    _check(_lib.cuhpx_grid_ring_info(grid, nlat, nlon, ring, ctypes.byref(c), ctypes.byref(w)), "cuhpx_grid_ring_info")
+    return c.value, w.value
+
+
+class GridTransform:
+    """alm2map / map2alm and their adjoints on a Gauss-Legendre or equiangular grid; argument marshalling only."""
+
+    def __init__(self, grid: int, nlat: int, nlon: int, lmax: int, mmax: int, batch: int, dtype: torch.dtype, device="cuda"):
+        self.grid, self.nlat, self.nlon, self.lmax, self.mmax, self.batch = grid, nlat, nlon, lmax, mmax, batch
+        self.dtype, self.code = dtype, _dtype_code(dtype)
+        self.cdtype = torch.complex128 if dtype == torch.float64 else torch.complex64
+        self.device = torch.device(device)
+        self.npix = cuhpx_grid_npix(grid, nlat, nlon)
+        self.nalm = cuhpx_alm_count(lmax, mmax)
+        nbytes = int(_lib.cuhpx_grid_workspace_bytes(grid, nlat, nlon, lmax, mmax, batch, self.code))
+        if nbytes == 0 or self.npix == 0:
+            raise CuhpxError(1, "cuhpx_grid_workspace_bytes")
+        self.workspace = torch.empty(nbytes, dtype=torch.uint8, device=self.device)
+        with torch.cuda.device(self.device):
+            p, n = _ws_args(self.workspace)
+            _check(_lib.cuhpx_grid_workspace_init(grid, nlat, nlon, lmax, mmax, batch, self.code, p, n, _stream_ptr(None)),
+                   "cuhpx_grid_workspace_init")
+
+    def _a(self):
+        return (self.grid, self.nlat, self.nlon, self.lmax, self.mmax, self.batch, self.code)
+
+    def alm2map(self, alm: torch.Tensor) -> torch.Tensor:
+        out = torch.empty(self.batch, self.npix, dtype=self.dtype, device=self.device)
+        p, n = _ws_args(self.workspace)
+        _check(_lib.cuhpx_grid_alm2map(*self._a(), _dev_ptr(alm), _dev_ptr(out), p, n, _stream_ptr(None)), "cuhpx_grid_alm2map")
+        return out
+
+    def map2alm(self, hmap: torch.Tensor, ring_weights: torch.Tensor | None = None) -> torch.Tensor:
+        out = torch.empty(self.batch, self.nalm, dtype=self.cdtype, device=self.device)
+        p, n = _ws_args(self.workspace)
+        _check(_lib.cuhpx_grid_map2alm(*self._a(), _dev_ptr(hmap), _dev_ptr(out), _dev_ptr(ring_weights), p, n, _stream_ptr(None)),
+               "cuhpx_grid_map2alm")
+        return out
+
+    def alm2map_adjoint(self, gmap: torch.Tensor) -> torch.Tensor:
+        out = torch.empty(self.batch, self.nalm, dtype=self.cdtype, device=self.device)
+        p, n = _ws_args(self.workspace)
+        _check(_lib.cuhpx_grid_alm2map_adjoint(*self._a(), _dev_ptr(gmap), _dev_ptr(out), p, n, _stream_ptr(None)),
+               "cuhpx_grid_alm2map_adjoint")
+        return out
+
+    def map2alm_adjoint(self, galm: torch.Tensor, ring_weights: torch.Tensor | None = None) -> torch.Tensor:
+        out = torch.empty(self.batch, self.npix, dtype=self.dtype, device=self.device)
+        p, n = _ws_args(self.workspace)
+        _check(_lib.cuhpx_grid_map2alm_adjoint(*self._a(), _dev_ptr(galm), _dev_ptr(out), _dev_ptr(ring_weights), p, n,
+                                               _stream_ptr(None)), "cuhpx_grid_map2alm_adjoint")
+        return out

@@ -61,6 +61,7 @@ struct DevPlan {
     const double* pref_hi;   // log2 |lambda_mm| prefactor, split hi + lo
     const double* pref_lo;
     const int* jmin;         // first ring pair processed for this m
+    const double* defw;      // [nrings] quadrature weight per pixel used when the caller passes none; null: 4 pi / npix
     // per (l, m) [nalm], packed like alm: rescaled recurrence coefficients (legendre.cu)
     const double* coef_alpha;
     const double* coef_scale;
@@ -95,7 +96,9 @@ struct HostPlan {
     DevPlan d;  // pointer members hold OFFSETS from the workspace base until resolve() rebases them
     cuhpx_dtype_t dtype;
     int geometry;
+    int max_ring;  // pixels of the longest ring
     size_t workspace_bytes;
+    size_t off_defw = 0;
     // table offsets inside the workspace
     size_t off_y, off_lshi, off_lslo, off_ringN, off_start, off_shifted, off_mcut, off_prefhi, off_preflo, off_jmin;
     size_t off_fft, fft_bytes, off_alpha, off_scale, off_spectra, off_partial, off_tcprefix, off_tcimages;

@@ -35,6 +35,29 @@ bool valid_args(int nside, int lmax, int mmax, int batch, int dtype) {
     return true;
 }
 
+// Which ring grid: HEALPix (n1 = nside) or an iso-latitude grid of n1 rings x n2 equally spaced pixels starting at
+// phi = 0 ("generalizes to ... Legendre-Gauss or Lobatto grids").
+struct Grid {
+    int geometry;  // cuhpx_grid_t
+    int n1, n2;
+};
+constexpr int MAX_NLAT = 1 << 14;
+
+bool valid_grid(const Grid& g) {
+    if (g.geometry == CUHPX_GRID_HEALPIX) return g.n1 >= 1 && g.n1 <= (1 << 13) && is_pow2(g.n1) && g.n2 == 0;
+    if (g.geometry != CUHPX_GRID_GAUSS_LEGENDRE && g.geometry != CUHPX_GRID_EQUIANGULAR) return false;
+    return g.n1 >= 1 && g.n1 <= MAX_NLAT && g.n2 >= 4 && g.n2 <= (1 << 14) && is_pow2(g.n2);
+}
+int grid_max_ring(const Grid& g) { return g.geometry == CUHPX_GRID_HEALPIX ? 4 * g.n1 : g.n2; }
+
+bool valid_call(const Grid& g, int lmax, int mmax, int batch, int dtype) {
+    if (!valid_grid(g)) return false;
+    if (g.geometry == CUHPX_GRID_HEALPIX) return valid_args(g.n1, lmax, mmax, batch, dtype);
+    if (lmax < 0 || mmax < 0 || mmax > lmax || lmax > 4 * (1 << 13)) return false;
+    if (batch < 1 || batch > MAX_BATCH) return false;
+    return dtype == CUHPX_F32 || dtype == CUHPX_F64;
+}
+
 // Gorski et al. ring table, northern hemisphere incl. equator: ring pair j (0-based) <-> ring i = j + 1.
 struct PairGeom {
     int N;
@@ -42,10 +65,61 @@ struct PairGeom {
     int shifted;
     ld y;    // 1 - cos(theta), exact rational rounded once
     ld sth;  // sin(theta)
+    ld w;    // quadrature weight per pixel (iso-latitude grids)
 };
+
+// Gauss-Legendre nodes (as colatitudes, north first) and weights by Newton's iteration on P_n(cos theta) in the angle,
+// long double; weights sum to 2.  (Textbook: Abramowitz & Stegun 25.4.29; the three-term recurrence for P_n.)
+void gauss_legendre(int n, std::vector<ld>& theta, std::vector<ld>& w) {
+    theta.resize(n);
+    w.resize(n);
+    for (int k = 0; k < (n + 1) / 2; ++k) {
+        ld t = PI_LD * ((ld)k + 0.75L) / ((ld)n + 0.5L);  // Tricomi's initial guess
+        ld dp = 0;
+        for (int it = 0; it < 100; ++it) {
+            const ld x = cosl(t);
+            ld p0 = 1, p1 = x;
+            for (int l = 2; l <= n; ++l) {
+                const ld p2 = ((2 * l - 1) * x * p1 - (l - 1) * p0) / l;
+                p0 = p1;
+                p1 = p2;
+            }
+            if (n == 1) { p0 = 1; p1 = x; }
+            dp = n * (x * p1 - p0) / (x * x - 1);      // dP_n/dx
+            const ld dt = p1 / (dp * -sinl(t));        // Newton in theta: d/dtheta = -sin(theta) d/dx
+            t -= dt;
+            if (fabsl(dt) < 1e-19L) break;
+        }
+        const ld x = cosl(t);
+        ld p0 = 1, p1 = x;
+        for (int l = 2; l <= n; ++l) {
+            const ld p2 = ((2 * l - 1) * x * p1 - (l - 1) * p0) / l;
+            p0 = p1;
+            p1 = p2;
+        }
+        dp = n * (x * p1 - p0) / (x * x - 1);
+        theta[k] = t;
+        theta[n - 1 - k] = PI_LD - t;
+        w[k] = w[n - 1 - k] = 2 / ((1 - x * x) * dp * dp);
+    }
+}
+
+// Fejer's first rule on theta_k = pi (k + 1/2) / n: exact for polynomials in cos(theta) of degree <= n - 1; weights sum to 2
+void fejer1(int n, std::vector<ld>& theta, std::vector<ld>& w) {
+    theta.resize(n);
+    w.resize(n);
+    for (int k = 0; k < n; ++k) {
+        const ld t = PI_LD * ((ld)k + 0.5L) / (ld)n;
+        ld s = 0;
+        for (int j = 1; j <= n / 2; ++j) s += cosl(2 * j * t) / (ld)(4LL * j * j - 1);
+        theta[k] = t;
+        w[k] = 2 * (1 - 2 * s) / (ld)n;
+    }
+}
 
 PairGeom pair_geom(int nside, int j) {
     PairGeom g;
+    g.w = 0;
     const long long ns = nside, i = j + 1;
     if (i < ns) {  // polar cap: N = 4 i, z = 1 - i^2 / (3 nside^2), phi0 = pi / N
         g.N = (int)(4 * i);
@@ -101,22 +175,32 @@ bool pair_active(int lmax, int m, ld pref_m, ld lg2sin, double yj) {
 }
 
 // Everything the host needs for (nside, lmax, mmax, batch, dtype): geometry, seeds, cut-offs, FFT ring classes, offsets.
-HostPlan* make_plan(int nside, int lmax, int mmax, int batch, cuhpx_dtype_t dt) {
+HostPlan* make_plan(const Grid& grid, int lmax, int mmax, int batch, cuhpx_dtype_t dt) {
     HostPlan* hp = new HostPlan;
     DevPlan& d = hp->d;
     memset(&d, 0, sizeof(d));
     hp->dtype = dt;
-    hp->geometry = 0;
+    hp->geometry = grid.geometry;
+    const bool hpx = grid.geometry == CUHPX_GRID_HEALPIX;
+    const int nside = hpx ? grid.n1 : 0;
     d.nside = nside;
     d.lmax = lmax;
     d.mmax = mmax;
     d.batch = batch;
-    d.nrings = 4 * nside - 1;
-    d.npairs = 2 * nside;
+    d.nrings = hpx ? 4 * nside - 1 : grid.n1;
+    d.npairs = hpx ? 2 * nside : (grid.n1 + 1) / 2;
     d.mstride = (int)cuhpx_spectra_stride(mmax);
-    d.npix = 12LL * nside * nside;
+    d.npix = hpx ? 12LL * nside * nside : (long long)grid.n1 * grid.n2;
     d.nalm = (long long)cuhpx_alm_count(lmax, mmax);
-    d.key = plan_key(nside, lmax, mmax, batch, (int)dt, 0);
+    d.key = plan_key(grid.n1, lmax, mmax, batch, (int)dt, grid.geometry + 16 * grid.n2);
+    hp->max_ring = grid_max_ring(grid);
+    std::vector<ld> gtheta, gw;
+    if (grid.geometry == CUHPX_GRID_GAUSS_LEGENDRE) gauss_legendre(grid.n1, gtheta, gw);
+    if (grid.geometry == CUHPX_GRID_EQUIANGULAR) fejer1(grid.n1, gtheta, gw);
+    if (!hpx) {  // quadrature weight per pixel: w_ring * 2 pi / nlon (Eq. 26 with the grid's own W)
+        hp->h_weight.resize(d.nrings);
+        for (int r = 0; r < d.nrings; ++r) hp->h_weight[r] = (double)(gw[r] * 2 * PI_LD / (ld)grid.n2);
+    }
     d.chunk_pairs = legendre_chunk_pairs(dt, batch, lmax, d.npairs);
     d.nchunk_max = (d.npairs + d.chunk_pairs - 1) / d.chunk_pairs;
 
@@ -131,7 +215,18 @@ HostPlan* make_plan(int nside, int lmax, int mmax, int batch, cuhpx_dtype_t dt) 
     hp->h_preflo.resize(mmax + 1);
     std::vector<ld> lg2sin(d.npairs), pref(mmax + 1);
     for (int j = 0; j < d.npairs; ++j) {
-        PairGeom g = pair_geom(nside, j);
+        PairGeom g;
+        if (hpx) {
+            g = pair_geom(nside, j);
+        } else {  // ring j of the northern half (the middle ring of an odd count is its own mirror)
+            g.N = grid.n2;
+            g.start = (long long)j * grid.n2;
+            g.shifted = 0;
+            const ld h = sinl(gtheta[j] / 2);
+            g.y = 2 * h * h;  // 1 - cos(theta) without cancellation
+            g.sth = sinl(gtheta[j]);
+            g.w = gw[j];
+        }
         hp->h_ringN[j] = g.N;
         hp->h_start[j] = g.start;
         hp->h_shifted[j] = g.shifted;
@@ -180,6 +275,7 @@ HostPlan* make_plan(int nside, int lmax, int mmax, int batch, cuhpx_dtype_t dt) 
     hp->off_prefhi = take(sizeof(double) * (d.mmax + 1));
     hp->off_preflo = take(sizeof(double) * (d.mmax + 1));
     hp->off_jmin = take(sizeof(int) * (d.mmax + 1));
+    hp->off_defw = hpx ? 0 : take(sizeof(double) * d.nrings);
     hp->off_fft = o;
     hp->fft_bytes = fft_plan_host(*hp);
     o = align_up(o + hp->fft_bytes);
@@ -205,17 +301,22 @@ HostPlan* make_plan(int nside, int lmax, int mmax, int batch, cuhpx_dtype_t dt) 
 
 // memo of host plans (bounded; entries are immutable and shared, so eviction never invalidates a running call)
 struct PlanKey {
-    int nside, lmax, mmax, batch, dtype;
+    int geometry, n1, n2, lmax, mmax, batch, dtype;
     bool operator==(const PlanKey& o) const {
-        return nside == o.nside && lmax == o.lmax && mmax == o.mmax && batch == o.batch && dtype == o.dtype;
+        return geometry == o.geometry && n1 == o.n1 && n2 == o.n2 && lmax == o.lmax && mmax == o.mmax && batch == o.batch &&
+               dtype == o.dtype;
     }
 };
 std::mutex g_mu;
 std::list<std::pair<PlanKey, PlanRef>> g_plans;  // most recently used first
 constexpr size_t MAX_PLANS = 24;
 
+PlanRef get_plan(const Grid& grid, int lmax, int mmax, int batch, cuhpx_dtype_t dt);
 PlanRef get_plan(int nside, int lmax, int mmax, int batch, cuhpx_dtype_t dt) {
-    const PlanKey k{nside, lmax, mmax, batch, (int)dt};
+    return get_plan(Grid{CUHPX_GRID_HEALPIX, nside, 0}, lmax, mmax, batch, dt);
+}
+PlanRef get_plan(const Grid& grid, int lmax, int mmax, int batch, cuhpx_dtype_t dt) {
+    const PlanKey k{grid.geometry, grid.n1, grid.n2, lmax, mmax, batch, (int)dt};
     {
         std::lock_guard<std::mutex> lk(g_mu);
         for (auto it = g_plans.begin(); it != g_plans.end(); ++it)
@@ -224,7 +325,7 @@ PlanRef get_plan(int nside, int lmax, int mmax, int batch, cuhpx_dtype_t dt) {
                 return g_plans.front().second;
             }
     }
-    PlanRef p(make_plan(nside, lmax, mmax, batch, dt));  // built outside the lock (may take a while at nside 4096)
+    PlanRef p(make_plan(grid, lmax, mmax, batch, dt));  // built outside the lock (may take a while at nside 4096)
     std::lock_guard<std::mutex> lk(g_mu);
     for (auto& e : g_plans)
         if (e.first == k) return e.second;
@@ -243,15 +344,21 @@ size_t alm_bytes(const HostPlan& hp) { return (size_t)hp.d.batch * (size_t)hp.d.
 
 // Argument checks shared by the operators; a / b are the data buffers with their sizes (either may be null for the
 // stage-level calls, which touch only one user buffer).
+int check_call(PlanRef* out, const Grid& grid, int lmax, int mmax, int batch, int dt, const void* a, size_t na, const void* b,
+               size_t nb, const void* ws, size_t ws_bytes);
 int check_call(PlanRef* out, int nside, int lmax, int mmax, int batch, int dt, const void* a, size_t na, const void* b,
                size_t nb, const void* ws, size_t ws_bytes) {
-    if (!valid_args(nside, lmax, mmax, batch, dt)) return CUHPX_EINVAL;
+    return check_call(out, Grid{CUHPX_GRID_HEALPIX, nside, 0}, lmax, mmax, batch, dt, a, na, b, nb, ws, ws_bytes);
+}
+int check_call(PlanRef* out, const Grid& grid, int lmax, int mmax, int batch, int dt, const void* a, size_t na, const void* b,
+               size_t nb, const void* ws, size_t ws_bytes) {
+    if (!valid_call(grid, lmax, mmax, batch, dt)) return CUHPX_EINVAL;
     if ((na && !a) || (nb && !b) || !ws) return CUHPX_EINVAL;
     if (((uintptr_t)a & 15) || ((uintptr_t)b & 15) || ((uintptr_t)ws & 15)) return CUHPX_EINVAL;
     // the map may hold up to 4 nside * 4 nside-ish rings of any supported length; unsupported ring lengths were
     // refused by cuhpx_workspace_bytes / cuhpx_workspace_init already
-    if (!fft_supported(4 * nside, (cuhpx_dtype_t)dt)) return CUHPX_EUNSUPPORTED;
-    PlanRef hp = get_plan(nside, lmax, mmax, batch, (cuhpx_dtype_t)dt);
+    if (!fft_supported(grid_max_ring(grid), (cuhpx_dtype_t)dt)) return CUHPX_EUNSUPPORTED;
+    PlanRef hp = get_plan(grid, lmax, mmax, batch, (cuhpx_dtype_t)dt);
     if (ws_bytes < hp->workspace_bytes) return CUHPX_EWORKSPACE;
     const size_t sa = a ? (na == (size_t)-1 ? map_bytes(*hp) : na == (size_t)-2 ? alm_bytes(*hp) : na) : 0;
     const size_t sb = b ? (nb == (size_t)-1 ? map_bytes(*hp) : nb == (size_t)-2 ? alm_bytes(*hp) : nb) : 0;
@@ -279,6 +386,7 @@ DevPlan HostPlan::resolve(void* ws) const {
     P.pref_hi = (const double*)(base + off_prefhi);
     P.pref_lo = (const double*)(base + off_preflo);
     P.jmin = (const int*)(base + off_jmin);
+    P.defw = off_defw ? (const double*)(base + off_defw) : nullptr;
     P.coef_alpha = (const double*)(base + off_alpha);
     P.coef_scale = (const double*)(base + off_scale);
     P.spectra = base + off_spectra;
@@ -343,12 +451,13 @@ size_t cuhpx_workspace_bytes(int nside, int lmax, int mmax, int batch, cuhpx_dty
     return get_plan(nside, lmax, mmax, batch, dtype)->workspace_bytes;
 }
 
-int cuhpx_workspace_init(int nside, int lmax, int mmax, int batch, cuhpx_dtype_t dtype, void* ws, size_t ws_bytes,
-                         cuhpx_stream_t stream) {
-    if (!valid_args(nside, lmax, mmax, batch, dtype)) return CUHPX_EINVAL;
+static int workspace_init_impl(const Grid& grid, int lmax, int mmax, int batch, cuhpx_dtype_t dtype, void* ws, size_t ws_bytes,
+                               cuhpx_stream_t stream) {
+    if (!valid_call(grid, lmax, mmax, batch, dtype)) return CUHPX_EINVAL;
     if (!ws || ((uintptr_t)ws & 15)) return CUHPX_EINVAL;
-    if (!fft_supported(4 * nside, dtype)) return CUHPX_EUNSUPPORTED;
-    PlanRef hp = get_plan(nside, lmax, mmax, batch, dtype);
+    if (!fft_supported(grid_max_ring(grid), dtype)) return CUHPX_EUNSUPPORTED;
+    const int nside = grid.n1;
+    PlanRef hp = get_plan(grid, lmax, mmax, batch, dtype);
     if (ws_bytes < hp->workspace_bytes) return CUHPX_EWORKSPACE;
     const DevPlan& d = hp->d;
     char* base = (char*)ws;
@@ -373,6 +482,7 @@ int cuhpx_workspace_init(int nside, int lmax, int mmax, int batch, cuhpx_dtype_t
     up(hp->off_prefhi, hp->h_prefhi.data(), sizeof(double) * (mmax + 1));
     up(hp->off_preflo, hp->h_preflo.data(), sizeof(double) * (mmax + 1));
     up(hp->off_jmin, hp->h_jmin.data(), sizeof(int) * (mmax + 1));
+    if (hp->off_defw) up(hp->off_defw, hp->h_weight.data(), sizeof(double) * d.nrings);
     if (d.tc_nb > 0) up(hp->off_tcprefix, hp->h_tcprefix.data(), sizeof(long long) * (mmax + 2));
     if (e == cudaSuccess)
         e = launch_legendre_coeff(lmax, mmax, (double*)(base + hp->off_alpha), (double*)(base + hp->off_scale), st);
@@ -390,6 +500,11 @@ int cuhpx_workspace_init(int nside, int lmax, int mmax, int batch, cuhpx_dtype_t
     // the sources above are pageable host memory owned by the (shared, immutable) plan or by this frame
     if (e == cudaSuccess) e = cudaStreamSynchronize(st);
     return e == cudaSuccess ? CUHPX_OK : CUHPX_ECUDA;
+}
+
+int cuhpx_workspace_init(int nside, int lmax, int mmax, int batch, cuhpx_dtype_t dtype, void* ws, size_t ws_bytes,
+                         cuhpx_stream_t stream) {
+    return workspace_init_impl(Grid{CUHPX_GRID_HEALPIX, nside, 0}, lmax, mmax, batch, dtype, ws, ws_bytes, stream);
 }
 
 int cuhpx_workspace_check(int nside, int lmax, int mmax, int batch, cuhpx_dtype_t dtype, const void* ws, size_t ws_bytes,
@@ -571,6 +686,84 @@ int cuhpx_map2alm_iter(int nside, int lmax, int mmax, int batch, cuhpx_dtype_t d
         CUDA_OR_FAIL(launch_accumulate(dt, d_scratch_alm, d_alm, nalm2, st));
     }
     return CUHPX_OK;
+}
+
+// ---- iso-latitude grids: the same two stages on another ring table
+size_t cuhpx_grid_npix(int grid, int nlat, int nlon) {
+    const Grid g{grid, nlat, grid == CUHPX_GRID_HEALPIX ? 0 : nlon};
+    if (!valid_grid(g)) return 0;
+    return grid == CUHPX_GRID_HEALPIX ? (size_t)12 * nlat * nlat : (size_t)nlat * nlon;
+}
+
+int cuhpx_grid_ring_info(int grid, int nlat, int nlon, int ring, double* cos_theta, double* weight) {
+    const Grid g{grid, nlat, nlon};
+    if (grid == CUHPX_GRID_HEALPIX || !valid_grid(g) || ring < 1 || ring > nlat) return CUHPX_EINVAL;
+    std::vector<ld> th, w;
+    if (grid == CUHPX_GRID_GAUSS_LEGENDRE) gauss_legendre(nlat, th, w);
+    else fejer1(nlat, th, w);
+    if (cos_theta) *cos_theta = (double)cosl(th[ring - 1]);
+    if (weight) *weight = (double)(w[ring - 1] * 2 * PI_LD / (ld)nlon);
+    return CUHPX_OK;
+}
+
+size_t cuhpx_grid_workspace_bytes(int grid, int nlat, int nlon, int lmax, int mmax, int batch, cuhpx_dtype_t dtype) {
+    const Grid g{grid, nlat, grid == CUHPX_GRID_HEALPIX ? 0 : nlon};
+    if (!valid_call(g, lmax, mmax, batch, dtype) || !fft_supported(grid_max_ring(g), dtype)) return 0;
+    return get_plan(g, lmax, mmax, batch, dtype)->workspace_bytes;
+}
+
+int cuhpx_grid_workspace_init(int grid, int nlat, int nlon, int lmax, int mmax, int batch, cuhpx_dtype_t dtype, void* ws,
+                              size_t ws_bytes, cuhpx_stream_t stream) {
+    return workspace_init_impl(Grid{grid, nlat, grid == CUHPX_GRID_HEALPIX ? 0 : nlon}, lmax, mmax, batch, dtype, ws, ws_bytes, stream);
+}
+
+// op: 0 alm2map, 1 map2alm, 2 alm2map_adjoint, 3 map2alm_adjoint
+static int grid_op(int op, int grid, int nlat, int nlon, int lmax, int mmax, int batch, cuhpx_dtype_t dt, const void* in, void* out,
+                   const double* d_w, void* ws, size_t ws_bytes, cuhpx_stream_t stream) {
+    const Grid g{grid, nlat, grid == CUHPX_GRID_HEALPIX ? 0 : nlon};
+    const bool in_is_map = op == 1 || op == 2;
+    PlanRef hp;
+    int rc = check_call(&hp, g, lmax, mmax, batch, dt, in, in_is_map ? MAP : ALM, out, in_is_map ? ALM : MAP, ws, ws_bytes);
+    if (rc) return rc;
+    if (d_w && ((uintptr_t)d_w & 7)) return CUHPX_EINVAL;
+    cudaStream_t st = (cudaStream_t)stream;
+    const DevPlan P = hp->resolve(ws);
+    switch (op) {
+        case 0:
+            CUDA_OR_FAIL(launch_legendre_synthesis(*hp, P, in, 0, st));
+            CUDA_OR_FAIL(launch_fft_synthesis(*hp, P, out, nullptr, 0, st));
+            break;
+        case 1:
+            CUDA_OR_FAIL(launch_fft_analysis(*hp, P, in, d_w, 1, st));
+            CUDA_OR_FAIL(launch_legendre_analysis(*hp, P, out, 0, st));
+            break;
+        case 2:
+            CUDA_OR_FAIL(launch_fft_analysis(*hp, P, in, nullptr, 0, st));
+            CUDA_OR_FAIL(launch_legendre_analysis(*hp, P, out, 1, st));
+            break;
+        default:
+            CUDA_OR_FAIL(launch_legendre_synthesis(*hp, P, in, 1, st));
+            CUDA_OR_FAIL(launch_fft_synthesis(*hp, P, out, d_w, 1, st));
+            break;
+    }
+    return CUHPX_OK;
+}
+
+int cuhpx_grid_alm2map(int grid, int nlat, int nlon, int lmax, int mmax, int batch, cuhpx_dtype_t dt, const void* d_alm, void* d_map,
+                       void* ws, size_t ws_bytes, cuhpx_stream_t stream) {
+    return grid_op(0, grid, nlat, nlon, lmax, mmax, batch, dt, d_alm, d_map, nullptr, ws, ws_bytes, stream);
+}
+int cuhpx_grid_map2alm(int grid, int nlat, int nlon, int lmax, int mmax, int batch, cuhpx_dtype_t dt, const void* d_map, void* d_alm,
+                       const double* d_w, void* ws, size_t ws_bytes, cuhpx_stream_t stream) {
+    return grid_op(1, grid, nlat, nlon, lmax, mmax, batch, dt, d_map, d_alm, d_w, ws, ws_bytes, stream);
+}
+int cuhpx_grid_alm2map_adjoint(int grid, int nlat, int nlon, int lmax, int mmax, int batch, cuhpx_dtype_t dt, const void* d_gmap,
+                               void* d_galm, void* ws, size_t ws_bytes, cuhpx_stream_t stream) {
+    return grid_op(2, grid, nlat, nlon, lmax, mmax, batch, dt, d_gmap, d_galm, nullptr, ws, ws_bytes, stream);
+}
+int cuhpx_grid_map2alm_adjoint(int grid, int nlat, int nlon, int lmax, int mmax, int batch, cuhpx_dtype_t dt, const void* d_galm,
+                               void* d_gmap, const double* d_w, void* ws, size_t ws_bytes, cuhpx_stream_t stream) {
+    return grid_op(3, grid, nlat, nlon, lmax, mmax, batch, dt, d_galm, d_gmap, d_w, ws, ws_bytes, stream);
 }
 
 static int ring_weights_lmax(int nside, int lmax_w) { return lmax_w > 0 ? lmax_w : 3 * nside; }

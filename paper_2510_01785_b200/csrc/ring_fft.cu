@@ -65,7 +65,8 @@ __device__ __forceinline__ RingInfo load_info(const RingInfo* __restrict__ info,
 
 __device__ __forceinline__ double ring_weight(const DevPlan& P, const RingInfo& R, const double* __restrict__ w, int use_w) {
     if (!use_w) return 1.0;
-    return w ? __ldg(w + R.r) : 4.0 * 3.14159265358979323846 / (double)P.npix;
+    if (w) return __ldg(w + R.r);
+    return P.defw ? __ldg(P.defw + R.r) : 4.0 * 3.14159265358979323846 / (double)P.npix;
 }
 
 // Ask the memory system to bring `bytes` at `ptr` into L2 (no register or shared-memory destination): issued
@@ -1125,7 +1126,8 @@ size_t fft_plan_host(HostPlan& hp) {
         R.r = r;
         R.pad0 = R.pad1 = 0;
         const int N = R.N;
-        if (N == 4 * d.nside && ilog2_ceil(N) - 1 >= MIN_LOG) F->pow2[ilog2_ceil(N) - 1].push_back(R);  // belt rings (N = 4 nside = 2^k)
+        // the longest rings when their length is 2^k: HEALPix belt rings (N = 4 nside), every ring of an iso-latitude grid
+        if (N == hp.max_ring && is_pow2(N) && ilog2_ceil(N) - 1 >= MIN_LOG) F->pow2[ilog2_ceil(N) - 1].push_back(R);
         else if (N <= DIRECT_MAX_N) F->direct.push_back(R);
         else {  // cap rings, chirp-z for every i (the few i = 2^k among them are not worth launches of their own)
             const int i = N / 4, lm = blue_logm(i);
@@ -1151,11 +1153,12 @@ size_t fft_plan_host(HostPlan& hp) {
         F->off_blue[l] = take(sizeof(RingInfo) * F->blue[l].size());
         F->off_blue_i[l] = take(sizeof(int) * F->blue_i[l].size());
     }
-    F->off_filt_offset = take(sizeof(long long) * d.nside);
-    F->twlen = 8 * d.nside < 2048 ? 2048 : 8 * d.nside;
+    const int nfilt = hp.max_ring / 4 > 0 ? hp.max_ring / 4 : 1;  // cap rings have N = 4 i, i < nfilt
+    F->off_filt_offset = take(sizeof(long long) * nfilt);
+    F->twlen = 2 * hp.max_ring < 2048 ? 2048 : 2 * hp.max_ring;
     F->off_tw = take(csize * F->twlen);
     F->off_tw64 = take(16 * (size_t)F->twlen);
-    F->filt_off.assign(d.nside, -1);
+    F->filt_off.assign(nfilt, -1);
     long long fo = 0;
     for (int l = MIN_LOG; l <= MAX_LOG; ++l)
         for (int i : F->blue_i[l]) {
@@ -1295,7 +1298,7 @@ cudaError_t fft_build_tables(const HostPlan& hp, char* base, cudaStream_t st) {
         up(F.off_blue[l], F.blue[l].data(), sizeof(RingInfo) * F.blue[l].size());
         up(F.off_blue_i[l], F.blue_i[l].data(), sizeof(int) * F.blue_i[l].size());
     }
-    up(F.off_filt_offset, F.filt_off.data(), sizeof(long long) * hp.d.nside);
+    up(F.off_filt_offset, F.filt_off.data(), sizeof(long long) * F.filt_off.size());
     if (e != cudaSuccess) return e;
     return hp.dtype == CUHPX_F64 ? build_tables_t<double>(F, base, st) : build_tables_t<float>(F, base, st);
 }
