@@ -142,6 +142,23 @@ int cuhpx_ring_weights(int nside, int lmax_w, double* d_weights, void* d_workspa
 typedef enum { CUHPX_NEST2RING = 0, CUHPX_RING2NEST = 1 } cuhpx_reorder_t;
 int cuhpx_reorder(int nside, int batch, cuhpx_dtype_t dtype, int direction, const void* d_in, void* d_out,
                   cuhpx_stream_t stream);
+/* The three layouts of P:108-110 through the (x, y, f) intermediate of P:118-123.  Layout codes:
+ *   CUHPX_LAYOUT_RING = 0, CUHPX_LAYOUT_NESTED = 1, CUHPX_LAYOUT_FLAT(corner, sense) = 2 + 2 corner + sense:
+ * "flat" (Fig. 3C: "indexing requires both an orientation (clockwise or counterclockwise) and a reference point")
+ * stores every base face as a row-major nside x nside image, index = f nside^2 + row nside + col, ready for 2-D
+ * convolution kernels; the image origin is the face's corner `corner` (0 south, 1 east, 2 north, 3 west), the fast
+ * axis leaves the origin counter-clockwise (sense 0; seen from outside the sphere, S -> E -> N -> W) or clockwise (sense
+ * 1) around the face, the slow axis the other way.  Fig. 3C's "counterclockwise from the south" is FLAT(0, 0) (col = x,
+ * row = y of the NESTED face coordinates), "clockwise from the east" is FLAT(1, 1) (reading R12; the paper
+ * gives no formula).  Same argument conventions as cuhpx_reorder; RING <-> NESTED takes the tiled kernels of
+ * cuhpx_reorder, every pair involving a flat layout one generic pass (reads or writes coalesced on the non-RING side). */
+#define CUHPX_LAYOUT_RING 0
+#define CUHPX_LAYOUT_NESTED 1
+#define CUHPX_LAYOUT_FLAT(corner, sense) (2 + 2 * (corner) + (sense))
+int cuhpx_reorder_layout(int nside, int batch, cuhpx_dtype_t dtype, int src_layout, int dst_layout, const void* d_in,
+                         void* d_out, cuhpx_stream_t stream);
+/* host helper: index in dst_layout of the pixel with index ip_src in src_layout (src_layout must not be RING); -1 on bad arguments */
+long long cuhpx_layout_index(int nside, int src_layout, int dst_layout, long long ip_src);
 /* host helper: RING index of NESTED pixel ipnest; -1 on bad arguments */
 long long cuhpx_nest2ring_index(int nside, long long ipnest);
 

@@ -57,6 +57,74 @@ def nested_centres(nside: int):
     return z, np.mod(phi, 2.0 * np.pi)
 
 
+def _plane_to_sphere(X, Y, col):
+    """HEALPix projection plane -> (z, phi); col = column of the face (its meridian in the polar zones)."""
+    z = np.empty(X.shape)
+    phi = np.empty(X.shape)
+    eq = np.abs(Y) <= 1.0
+    z[eq] = 2.0 * Y[eq] / 3.0
+    phi[eq] = X[eq] * (np.pi / 4.0)
+    po = ~eq
+    sigma = 2.0 - np.abs(Y[po])
+    z[po] = np.sign(Y[po]) * (1.0 - sigma * sigma / 3.0)
+    xm = 2.0 * col[po] + 1.0
+    phi[po] = (xm + (X[po] - xm) / sigma) * (np.pi / 4.0)
+    return z, np.mod(phi, 2.0 * np.pi)
+
+
+def flat_centres(nside: int, corner: int, sense: int):
+    """(z, phi) of the centre of every pixel of the flat layout (Fig. 3C; reading R12): face f is a
+    row-major nside x nside image whose origin is the face's corner `corner` (0 S, 1 E, 2 N, 3 W) and whose fast axis
+    runs along the face edge towards the counter-clockwise (sense 0: S -> E -> N -> W) or clockwise (sense 1) neighbour
+    corner, the slow axis along the other edge.  Written with the corners of the face diamond in the projection plane,
+    not with (x, y) index arithmetic."""
+    npix = 12 * nside * nside
+    ip = np.arange(npix, dtype=np.int64)
+    f = ip // (nside * nside)
+    r = ip % (nside * nside)
+    row_i = r // nside
+    col_i = r % nside
+    frow = f // 4
+    fcol = f % 4
+    cx = np.where(frow == 1, 2.0 * fcol, 2.0 * fcol + 1.0)
+    cy = -frow.astype(np.float64)
+    corners = [(cx, cy), (cx + 1.0, cy + 1.0), (cx, cy + 2.0), (cx - 1.0, cy + 1.0)]  # S, E, N, W: counter-clockwise
+    O = corners[corner]
+    ccw = corners[(corner + 1) % 4]
+    cw = corners[(corner - 1) % 4]
+    A, B = (ccw, cw) if sense == 0 else (cw, ccw)  # fast edge, slow edge
+    s = (col_i + 0.5) / nside
+    t = (row_i + 0.5) / nside
+    X = O[0] + s * (A[0] - O[0]) + t * (B[0] - O[0])
+    Y = O[1] + s * (A[1] - O[1]) + t * (B[1] - O[1])
+    return _plane_to_sphere(X, Y, fcol)
+
+
+def _lookup_ring_index(nside: int, z, phi) -> np.ndarray:
+    """RING index of the pixels with centres (z, phi), by matching against the (pinned) ring table."""
+    nrings = 4 * nside - 1
+    N = np.empty(nrings, dtype=np.int64)
+    start = np.empty(nrings, dtype=np.int64)
+    zr = np.empty(nrings)
+    phi0 = np.empty(nrings)
+    for r in range(nrings):
+        n, st, c, _s, p0 = ring_geometry(nside, r + 1)
+        N[r], start[r], zr[r], phi0[r] = n, st, c, p0
+    pos = np.clip(np.searchsorted(-zr, -z), 1, nrings - 1)
+    ring = np.where(np.abs(zr[pos - 1] - z) < np.abs(zr[pos] - z), pos - 1, pos)
+    assert np.abs(zr[ring] - z).max() < 1e-12, "a pixel centre is not on any ring"
+    t = (phi - phi0[ring]) * N[ring] / (2.0 * np.pi)
+    k = np.rint(t)
+    assert np.abs(t - k).max() < 1e-9, "a pixel centre is not a RING pixel centre"
+    return start[ring] + np.mod(k.astype(np.int64), N[ring])
+
+
+def flat2ring_table(nside: int, corner: int, sense: int) -> np.ndarray:
+    """ring_index[ipflat] for the flat layout (corner, sense)."""
+    z, phi = flat_centres(nside, corner, sense)
+    return _lookup_ring_index(nside, z, phi)
+
+
 def nest2ring_table(nside: int) -> np.ndarray:
     """ring_index[ipnest] for all 12 nside^2 pixels, by matching pixel centres against the ring table."""
     nrings = 4 * nside - 1

@@ -26,6 +26,7 @@ EXPORTS = [
     "cuhpx_synthesis_legendre_stage", "cuhpx_synthesis_fft_stage", "cuhpx_fma_peak_probe", "cuhpx_plan_stats",
     "cuhpx_grid_npix", "cuhpx_grid_ring_info", "cuhpx_grid_workspace_bytes", "cuhpx_grid_workspace_init",
     "cuhpx_grid_alm2map", "cuhpx_grid_map2alm", "cuhpx_grid_alm2map_adjoint", "cuhpx_grid_map2alm_adjoint",
+    "cuhpx_reorder_layout", "cuhpx_layout_index",
     "cuhpx_map2alm_iter", "cuhpx_ring_weights_workspace_bytes", "cuhpx_ring_weights", "cuhpx_reorder", "cuhpx_nest2ring_index", "cuhpx_alm_resize",
 ]
 CUHPX_NEST2RING, CUHPX_RING2NEST = 0, 1
@@ -76,6 +77,9 @@ def _load() -> ctypes.CDLL:
     lib.cuhpx_grid_map2alm.argtypes = [i, i, i, i, i, i, i, vp, vp, vp, vp, sz, vp]
     lib.cuhpx_grid_alm2map_adjoint.argtypes = [i, i, i, i, i, i, i, vp, vp, vp, sz, vp]
     lib.cuhpx_grid_map2alm_adjoint.argtypes = [i, i, i, i, i, i, i, vp, vp, vp, vp, sz, vp]
+    lib.cuhpx_reorder_layout.argtypes = [i, i, i, i, i, vp, vp, vp]
+    lib.cuhpx_layout_index.argtypes = [i, i, i, ctypes.c_longlong]
+    lib.cuhpx_layout_index.restype = ctypes.c_longlong
     lib.cuhpx_ring_weights_workspace_bytes.argtypes = [i, i]
     lib.cuhpx_ring_weights_workspace_bytes.restype = sz
     lib.cuhpx_ring_weights.argtypes = [i, i, vp, vp, sz, vp]
@@ -240,6 +244,29 @@ def ring_weights(nside: int, lmax_w: int = 0, device="cuda") -> torch.Tensor:
 def cuhpx_reorder(nside, batch, dtype, direction, d_in, d_out, stream=None) -> None:
     _check(_lib.cuhpx_reorder(nside, batch, dtype, int(direction), _dev_ptr(d_in), _dev_ptr(d_out), _stream_ptr(stream)),
            "cuhpx_reorder")
+
+
+CUHPX_LAYOUT_RING, CUHPX_LAYOUT_NESTED = 0, 1
+
+
+def CUHPX_LAYOUT_FLAT(corner: int, sense: int) -> int:
+    return 2 + 2 * corner + sense
+
+
+def cuhpx_reorder_layout(nside, batch, dtype, src_layout, dst_layout, d_in, d_out, stream=None) -> None:
+    _check(_lib.cuhpx_reorder_layout(nside, batch, dtype, int(src_layout), int(dst_layout), _dev_ptr(d_in), _dev_ptr(d_out),
+                                     _stream_ptr(stream)), "cuhpx_reorder_layout")
+
+
+def cuhpx_layout_index(nside: int, src_layout: int, dst_layout: int, ip_src: int) -> int:
+    return int(_lib.cuhpx_layout_index(nside, src_layout, dst_layout, ip_src))
+
+
+def reorder_layout(hmap: torch.Tensor, nside: int, src_layout: int, dst_layout: int) -> torch.Tensor:
+    """[batch, npix] between RING / NESTED / flat layouts."""
+    out = torch.empty_like(hmap)
+    cuhpx_reorder_layout(nside, hmap.shape[0], _dtype_code(hmap.dtype), src_layout, dst_layout, hmap, out)
+    return out
 
 
 def cuhpx_alm_resize(lmax_in, mmax_in, lmax_out, mmax_out, batch, dtype, d_in, d_out, stream=None) -> None:

@@ -151,6 +151,9 @@ cudaError_t launch_accumulate(cuhpx_dtype_t dt, const void* d, void* a, size_t n
 // layout reordering (reorder.cu)
 cudaError_t launch_reorder(int nside, int batch, cuhpx_dtype_t dt, int to_ring, const void* in, void* out, cudaStream_t st);
 long long nest_to_ring_index(int nside, long long ipnest);
+// generic layout conversion (0 RING, 1 NESTED, 2..9 flat variants); layout_index: src must not be RING
+cudaError_t launch_layout(int nside, int batch, cuhpx_dtype_t dt, int src, int dst, const void* in, void* out, cudaStream_t st);
+long long layout_index(int nside, int src_layout, int dst_layout, long long ip_src);
 cudaError_t launch_alm_resize(int lmax_in, int mmax_in, int lmax_out, int mmax_out, int batch, cuhpx_dtype_t dt,
                               const void* in, void* out, cudaStream_t st);
 

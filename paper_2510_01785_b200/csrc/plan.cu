@@ -804,6 +804,24 @@ int cuhpx_reorder(int nside, int batch, cuhpx_dtype_t dt, int direction, const v
     return CUHPX_OK;
 }
 
+int cuhpx_reorder_layout(int nside, int batch, cuhpx_dtype_t dt, int src_layout, int dst_layout, const void* d_in, void* d_out,
+                         cuhpx_stream_t stream) {
+    if (nside < 1 || !is_pow2(nside) || nside > (1 << 13) || batch < 1 || batch > MAX_BATCH || (dt != CUHPX_F32 && dt != CUHPX_F64))
+        return CUHPX_EINVAL;
+    if (src_layout < 0 || src_layout > 9 || dst_layout < 0 || dst_layout > 9) return CUHPX_EINVAL;
+    if (!d_in || !d_out || ((uintptr_t)d_in & 15) || ((uintptr_t)d_out & 15)) return CUHPX_EINVAL;
+    const size_t nb = (size_t)batch * 12 * nside * nside * (dt == CUHPX_F64 ? 8 : 4);
+    if (overlap(d_in, nb, d_out, nb)) return CUHPX_EINVAL;
+    CUDA_OR_FAIL(launch_layout(nside, batch, dt, src_layout, dst_layout, d_in, d_out, (cudaStream_t)stream));
+    return CUHPX_OK;
+}
+
+long long cuhpx_layout_index(int nside, int src_layout, int dst_layout, long long ip_src) {
+    if (nside < 1 || !is_pow2(nside) || nside > (1 << 13) || ip_src < 0 || ip_src >= 12LL * nside * nside) return -1;
+    if (src_layout < 1 || src_layout > 9 || dst_layout < 0 || dst_layout > 9) return -1;
+    return layout_index(nside, src_layout, dst_layout, ip_src);
+}
+
 int cuhpx_alm_resize(int lmax_in, int mmax_in, int lmax_out, int mmax_out, int batch, cuhpx_dtype_t dt,
                      const void* d_in, void* d_out, cuhpx_stream_t stream) {
     if (lmax_in < 0 || mmax_in < 0 || mmax_in > lmax_in || lmax_out < 0 || mmax_out < 0 || mmax_out > lmax_out) return CUHPX_EINVAL;

@@ -227,6 +227,107 @@ cudaError_t launch_reorder(int nside, int batch, cuhpx_dtype_t dt, int to_ring, 
                            : run_reorder<uint32_t>(nside, batch, to_ring, in, out, st);
 }
 
+// ------------------------------------------------------------------ generic layout conversion through (x, y, f)
+// "Source -> xyf, xyf -> Target".  Layout codes (include/cuhpx.h): 0 RING, 1 NESTED, 2 + 2 corner + sense
+// = flat: every face a row-major nside x nside image, index = f nside^2 + row nside + col, whose origin is the face's
+// corner S, E, N, W (corner 0..3) and whose fast axis leaves the origin counter-clockwise (sense 0) or clockwise (1)
+// around the face; the slow axis leaves it the other way (reading R12 of P:110 / Fig. 3C).
+// With the face coordinates of NESTED (x north-east, y north-west from the southern corner; corners S (0,0), E (n-1,0),
+// N (n-1,n-1), W (0,n-1), counter-clockwise S -> E -> N -> W):
+//   corner S: (u, v) = (x, y)   E: (y, n-1-x)   N: (n-1-x, n-1-y)   W: (n-1-y, x)   = steps along the two edges leaving
+//   the origin, u towards the counter-clockwise neighbour;  (col, row) = (u, v) for sense 0, (v, u) for sense 1.
+__host__ __device__ __forceinline__ void flat_to_xy(int n, int corner, int sense, int row, int col, int& x, int& y) {
+    const int u = sense ? row : col, v = sense ? col : row;
+    switch (corner) {
+        case 0: x = u; y = v; break;
+        case 1: x = n - 1 - v; y = u; break;
+        case 2: x = n - 1 - u; y = n - 1 - v; break;
+        default: x = v; y = n - 1 - u; break;
+    }
+}
+__host__ __device__ __forceinline__ void xy_to_flat(int n, int corner, int sense, int x, int y, int& row, int& col) {
+    int u, v;
+    switch (corner) {
+        case 0: u = x; v = y; break;
+        case 1: u = y; v = n - 1 - x; break;
+        case 2: u = n - 1 - x; v = n - 1 - y; break;
+        default: u = n - 1 - y; v = x; break;
+    }
+    col = sense ? v : u;
+    row = sense ? u : v;
+}
+__host__ __device__ __forceinline__ unsigned long long spread_bits(unsigned v) {  // bit b -> bit 2 b
+    unsigned long long r = v;
+    r = (r | (r << 16)) & 0x0000ffff0000ffffULL;
+    r = (r | (r << 8)) & 0x00ff00ff00ff00ffULL;
+    r = (r | (r << 4)) & 0x0f0f0f0f0f0f0f0fULL;
+    r = (r | (r << 2)) & 0x3333333333333333ULL;
+    r = (r | (r << 1)) & 0x5555555555555555ULL;
+    return r;
+}
+// non-RING layouts: index <-> (x, y, f)
+__host__ __device__ __forceinline__ void index_to_xyf(int n, int layout, long long ip, int& x, int& y, int& f) {
+    const long long n2 = (long long)n * n;
+    f = (int)(ip / n2);
+    const long long r = ip - (long long)f * n2;
+    if (layout == 1) {
+        x = (int)compact_bits((unsigned long long)r);
+        y = (int)compact_bits((unsigned long long)r >> 1);
+    } else {
+        flat_to_xy(n, (layout - 2) >> 1, (layout - 2) & 1, (int)(r / n), (int)(r % n), x, y);
+    }
+}
+__host__ __device__ __forceinline__ long long xyf_to_index(int n, int layout, int x, int y, int f) {
+    if (layout == 0) return xyf_to_ring(n, x, y, f);
+    const long long n2 = (long long)n * n;
+    if (layout == 1) return f * n2 + (long long)(spread_bits((unsigned)x) | (spread_bits((unsigned)y) << 1));
+    int row, col;
+    xy_to_flat(n, (layout - 2) >> 1, (layout - 2) & 1, x, y, row, col);
+    return f * n2 + (long long)row * n + col;
+}
+
+// `walk` is a non-RING layout: thread i handles the pixel with index i in that layout (coalesced on that side);
+// GATHER: out[i] = in[other(i)] (walk = destination);  otherwise out[other(i)] = in[i] (walk = source).
+template <typename W, bool GATHER>
+__global__ void __launch_bounds__(256) layout_kernel(int nside, long long npix, int walk, int other, const W* __restrict__ in,
+                                                     W* __restrict__ out) {
+    const long long i = (long long)blockIdx.x * 256 + threadIdx.x;
+    if (i >= npix) return;
+    int x, y, f;
+    index_to_xyf(nside, walk, i, x, y, f);
+    const long long j = xyf_to_index(nside, other, x, y, f);
+    const size_t b = (size_t)blockIdx.y * (size_t)npix;
+    if (GATHER) out[b + i] = in[b + j];
+    else out[b + j] = in[b + i];
+}
+
+long long layout_index(int nside, int src_layout, int dst_layout, long long ip_src) {
+    // only used by the host helper: RING as a source has no closed form here -> search is the caller's business
+    int x, y, f;
+    index_to_xyf(nside, src_layout, ip_src, x, y, f);
+    return xyf_to_index(nside, dst_layout, x, y, f);
+}
+
+cudaError_t launch_layout(int nside, int batch, cuhpx_dtype_t dt, int src, int dst, const void* in, void* out, cudaStream_t st) {
+    if (src == dst) {
+        const size_t bytes = (size_t)batch * 12 * nside * nside * (dt == CUHPX_F64 ? 8 : 4);
+        return cudaMemcpyAsync(out, in, bytes, cudaMemcpyDeviceToDevice, st);
+    }
+    if ((src == 0 && dst == 1) || (src == 1 && dst == 0)) return launch_reorder(nside, batch, dt, dst == 0, in, out, st);
+    const long long npix = 12LL * nside * nside;
+    const dim3 grid((unsigned)((npix + 255) / 256), (unsigned)batch);
+    const bool gather = src == 0 || dst != 0;  // walk the destination unless the destination is RING
+    const int walk = gather ? dst : src, other = gather ? src : dst;
+    if (dt == CUHPX_F64) {
+        if (gather) layout_kernel<uint64_t, true><<<grid, 256, 0, st>>>(nside, npix, walk, other, (const uint64_t*)in, (uint64_t*)out);
+        else layout_kernel<uint64_t, false><<<grid, 256, 0, st>>>(nside, npix, walk, other, (const uint64_t*)in, (uint64_t*)out);
+    } else {
+        if (gather) layout_kernel<uint32_t, true><<<grid, 256, 0, st>>>(nside, npix, walk, other, (const uint32_t*)in, (uint32_t*)out);
+        else layout_kernel<uint32_t, false><<<grid, 256, 0, st>>>(nside, npix, walk, other, (const uint32_t*)in, (uint32_t*)out);
+    }
+    return cudaGetLastError();
+}
+
 // ------------------------------------------------------------------ spectral resampling
 // "upsampling and downsampling of HEALPix data by truncating or extending spherical harmonic coefficients before
 // applying the iSHT": out(l, m) = in(l, m) where the input has that coefficient, else 0.  W = one complex value.
