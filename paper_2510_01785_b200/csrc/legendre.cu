@@ -1257,7 +1257,9 @@ static cudaError_t run_synthesis_f32x2(const HostPlan& hp, const DevPlan& P, con
 }
 
 cudaError_t launch_legendre_synthesis(const HostPlan& hp, const DevPlan& P, const void* d_alm, int adjoint, cudaStream_t st) {
-    if (hp.dtype == CUHPX_F64) return run_synthesis_cfg<double, 1, 4, 128>(hp, P, d_alm, adjoint, st);
+    // fp64: 2-warp CTAs of 6 ring pairs per thread (r2 sweep over NT 64..128, R 3..8: 60.9 ms at nside 4096 against 63.7 ms
+    // for the r1 shape 128 x 4)
+    if (hp.dtype == CUHPX_F64) return run_synthesis_cfg<double, 1, 6, 64>(hp, P, d_alm, adjoint, st);
     if (P.batch >= 8) {
         // tensor-core kernel (legendre_tc.cu): lambda goes to tensor memory, the contraction to tcgen05.mma
         const cudaError_t e = launch_legendre_synthesis_tc(hp, P, d_alm, adjoint, st);
