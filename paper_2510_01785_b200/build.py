@@ -65,6 +65,24 @@ def build(force: bool = False, verbose: bool = False) -> str:
     return LIB
 
 
+PROBE = os.path.join(HERE, "tcgen05_probe")
+
+
+def build_probe() -> str:
+    """Compile the tcgen05 micro-benchmark (csrc/tcgen05_probe.cu, a measurement tool: profiles/r2_tcgen05_probe.md)."""
+    nvcc = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
+    cmd = [nvcc, "-O3", "-std=c++17", "-gencode", "arch=compute_100a,code=sm_100a", "-o", PROBE,
+           os.path.join(CSRC, "tcgen05_probe.cu")]
+    res = subprocess.run(cmd, capture_output=True, text=True)
+    if res.returncode != 0:
+        sys.stderr.write(res.stdout + res.stderr)
+        raise RuntimeError("nvcc failed building tcgen05_probe")
+    return PROBE
+
+
 if __name__ == "__main__":
-    build(force="--force" in sys.argv, verbose=True)
-    print(LIB)
+    if "--probe" in sys.argv:
+        print(build_probe())
+    else:
+        build(force="--force" in sys.argv, verbose=True)
+        print(LIB)

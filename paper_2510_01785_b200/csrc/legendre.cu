@@ -1236,7 +1236,14 @@ cudaError_t launch_legendre_analysis(const HostPlan& hp, const DevPlan& P, void*
     // in-place accumulation over ring chunks (SEQ): cfg5 88.3 -> 87.0 ms, 3.7 GB of partial writes and 4.3 GB of workspace gone
     // fp64: 2-warp CTAs of 7 ring pairs per thread (r2 sweep over NT 32..128, R 5..8, resident CTAs: 80.9 ms at nside 4096
     // against 87.0 ms for the r1 shape 128 x 8; a software-pipelined butterfly was tried and was slower, 86-91 ms)
-    if (hp.dtype == CUHPX_F64) return run_analysis_cfg<double, 1, 7, 8, 64, 64, true>(hp, P, d_alm, adjoint, st);
+    // (small transforms keep the r1 shape: fewer, larger CTAs finish a launch-bound grid sooner -- nside 256: 0.090 vs 0.108 ms).
+    // The price of the narrow chunks is DRAM traffic: the a_lm row of an order is read, added to and written back once per
+    // chunk of 448 ring pairs (18 visits at nside 4096: 24.6 GB per call against 7.3 GB for 1024-pair chunks; L2 evict_last /
+    // evict_first cache policies on the row / the spectra were tried and changed nothing) -- 0.3 TB/s, 5 % of HBM, under a
+    // kernel that is bound by the FP64 pipe.
+    if (hp.dtype == CUHPX_F64)
+        return P.npairs >= 2048 ? run_analysis_cfg<double, 1, 7, 8, 64, 64, true>(hp, P, d_alm, adjoint, st)
+                                : run_analysis_cfg<double, 1, 8, 8, 128, 64, true>(hp, P, d_alm, adjoint, st);
     if (P.batch >= 5) return run_analysis_gemm(hp, P, d_alm, adjoint, st);
     if (P.batch >= 4) return run_analysis<float, 4>(hp, P, d_alm, adjoint, st);
     return run_analysis<float, 1>(hp, P, d_alm, adjoint, st);
@@ -1259,7 +1266,9 @@ static cudaError_t run_synthesis_f32x2(const HostPlan& hp, const DevPlan& P, con
 cudaError_t launch_legendre_synthesis(const HostPlan& hp, const DevPlan& P, const void* d_alm, int adjoint, cudaStream_t st) {
     // fp64: 2-warp CTAs of 6 ring pairs per thread (r2 sweep over NT 64..128, R 3..8: 60.9 ms at nside 4096 against 63.7 ms
     // for the r1 shape 128 x 4)
-    if (hp.dtype == CUHPX_F64) return run_synthesis_cfg<double, 1, 6, 64>(hp, P, d_alm, adjoint, st);
+    if (hp.dtype == CUHPX_F64)
+        return P.npairs >= 2048 ? run_synthesis_cfg<double, 1, 6, 64>(hp, P, d_alm, adjoint, st)
+                                : run_synthesis_cfg<double, 1, 4, 128>(hp, P, d_alm, adjoint, st);
     if (P.batch >= 8) {
         // tensor-core kernel (legendre_tc.cu): lambda goes to tensor memory, the contraction to tcgen05.mma
         const cudaError_t e = launch_legendre_synthesis_tc(hp, P, d_alm, adjoint, st);

@@ -109,6 +109,22 @@ __device__ __forceinline__ RingInfo begin_item(const DevPlan& P, const RingInfo*
     return R;
 }
 
+// Bluestein kernels: the filter spectrum of the ring size the SM will see `pf` items ahead, brought into L2 as well (it is
+// first touched in the middle of a work item, between the forward and the inverse transform, where every warp of the CTA
+// waits for it; north and south ring of one size are neighbours in the work list, so every other item finds it anyway)
+template <typename T>
+__device__ __forceinline__ void prefetch_filter(const RingInfo* __restrict__ info, const FftTables& tabs, int m_len) {
+    if (threadIdx.x < 32 && tabs.pf > 0) {
+        const long long lin = (long long)blockIdx.y * gridDim.x + blockIdx.x + tabs.pf;
+        if (lin < (long long)gridDim.x * gridDim.y) {
+            const RingInfo Rn = load_info(info, (int)(lin % gridDim.x));
+            using T2 = typename V2<T>::type;
+            const T2* f = reinterpret_cast<const T2*>(tabs.filt) + __ldg(tabs.filt_offset + (Rn.N >> 2));
+            prefetch_l2(f, (unsigned)(m_len * sizeof(T2)));
+        }
+    }
+}
+
 // ------------------------------------------------------------------ direct kernels (short rings)
 template <typename T>
 __global__ void __launch_bounds__(FFT_THREADS) ring_direct_analysis_kernel(DevPlan P, const RingInfo* __restrict__ info,
@@ -773,6 +789,7 @@ __global__ void __launch_bounds__(FftPlan<LOGM>::NT, MinBlocks<T, LOGM>::blue) r
     const int tid = threadIdx.x;
     const int ch = blockIdx.y;
     const RingInfo R = begin_item<T, true>(P, info, map, tabs.pf);
+    prefetch_filter<T>(info, tabs, M);
     const int N = R.N, i = N >> 2, n = N >> 1, Q = 2 * N;
     const T2* src = reinterpret_cast<const T2*>(map + (size_t)ch * P.npix + R.start);
     const T2* filt = reinterpret_cast<const T2*>(tabs.filt) + __ldg(tabs.filt_offset + i);
@@ -925,6 +942,7 @@ __global__ void __launch_bounds__(FftPlan<LOGM>::NT, MinBlocks<T, LOGM>::blue) r
     const int tid = threadIdx.x;
     const int ch = blockIdx.y;
     const RingInfo R = begin_item<T, false>(P, info, map, tabs.pf);
+    prefetch_filter<T>(info, tabs, M);
     const int N = R.N, i = N >> 2, n = N >> 1, Q = 2 * N;
     const T2* filt = reinterpret_cast<const T2*>(tabs.filt) + __ldg(tabs.filt_offset + i);
     fill_roots_any<T>(rq, Q, tid, NT);
