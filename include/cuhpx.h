@@ -47,6 +47,8 @@
  *     thrown across the ABI.  After CUHPX_ECUDA, cudaGetLastError() describes the launch failure.
  *   - batch <= 65535 (channels index a grid dimension).
  *   - There is no CPU fallback: on a machine without a CUDA device every compute call returns CUHPX_ECUDA.
+ *   - One environment switch, read once per process, for A/B measurements only: CUHPX_LEGENDRE_TC=0 runs batched fp32
+ *     Legendre synthesis (batch >= 8) on the CUDA-core kernels instead of the tcgen05 / tensor-memory kernel.
  */
 #ifndef CUHPX_H_
 #define CUHPX_H_

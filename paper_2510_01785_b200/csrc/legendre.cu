@@ -10,15 +10,12 @@
 // registers.  cos(theta) enters as x p = p - y p with y = 1 - cos(theta) (R3).
 #include <cuda_runtime.h>
 #include <math.h>
-#include <stdlib.h>
 
 #include "cuhpx_internal.h"
 #include "legendre_common.cuh"
 
 namespace cuhpx {
 
-constexpr int LEG_THREADS = 256;
-constexpr int LEG_WARPS = LEG_THREADS / 32;
 constexpr int CT = 64;  // recurrence-coefficient tile (l values per __syncthreads)
 
 // ------------------------------------------------------------------ recurrence coefficients (built once per plan)
@@ -1231,7 +1228,7 @@ static cudaError_t run_analysis_gemm(const HostPlan& hp, const DevPlan& P, void*
     return e;
 }
 
-// Configurations below are the winners of sweeps on B200 (profiles/r1_legendre_tuning.md).
+// Configurations below are the winners of sweeps on B200.
 cudaError_t launch_legendre_analysis(const HostPlan& hp, const DevPlan& P, void* d_alm, int adjoint, cudaStream_t st) {
     // in-place accumulation over ring chunks (SEQ): cfg5 88.3 -> 87.0 ms, 3.7 GB of partial writes and 4.3 GB of workspace gone
     // fp64: 2-warp CTAs of 7 ring pairs per thread (r2 sweep over NT 32..128, R 5..8, resident CTAs: 80.9 ms at nside 4096
