@@ -177,6 +177,9 @@ def test_map2alm_iter_matches_oracle(nside, lmax, batch, dtype, n_iter, weighted
     # fp32 with few channels at sizes where the exponent-scaled seeds matter (sc < 0 on polar rings) and the
     # analysis walks several ring chunks: legendre_analysis_kernel<float, 1 / 4>, legendre_synthesis_kernel<float, 1 / 4>
     (256, 600, 600, 1, "f32"), (512, 700, 700, 4, "f32"),
+    # tensor-core synthesis (batch >= 8): 16-channel groups with a ragged second group and mmax < lmax; a last stage of
+    # one degree (lmax - m + 1 = 1 mod 32); more than one 128-ring tile per order with late-starting polar rings
+    (32, 64, 40, 20, "f32"), (16, 32, 32, 8, "f32"), (128, 300, 300, 8, "f32"),
 ])
 def test_small_and_ragged_cases(nside, lmax, mmax, batch, dtype):
     """mmax < lmax, lmax far above 2 nside (every polar ring aliases), batch not a multiple of the channel

@@ -96,6 +96,10 @@ GPU_CASES = [
     ("eq", 2, 64, 256, 31, 31, 1, "f64"),
     ("gl", 1, 64, 256, 63, 63, 8, "f32"),       # batched fp32: tensor-core synthesis, contraction analysis
     ("eq", 2, 48, 128, 40, 40, 3, "f32"),
+    ("gl", 1, 1, 4, 0, 0, 1, "f64"),            # degenerate: one ring on the equator
+    ("gl", 1, 2, 4, 1, 1, 1, "f64"),
+    ("eq", 2, 3, 8, 2, 2, 2, "f64"),
+    ("gl", 1, 40, 64, 60, 60, 1, "f64"),        # lmax beyond the ring Nyquist frequency: the alias fold on a uniform grid
 ]
 
 
@@ -137,6 +141,18 @@ def test_gpu_grid_transforms_match_oracle(kind, code, nlat, nlon, lmax, mmax, ba
             else:
                 err = np.linalg.norm(got[name][b] - ref[name]) / np.linalg.norm(ref[name])
                 assert err <= 2e-5, (name, b, err)    # north_star: relative L2 <= 2e-5 for fp32
+
+
+def test_grid_argument_errors():
+    from paper_2510_01785_b200 import binding as B
+
+    assert B.cuhpx_grid_npix(B.CUHPX_GRID_GAUSS_LEGENDRE, 8, 12) == 0         # nlon must be a power of two
+    assert B.cuhpx_grid_npix(B.CUHPX_GRID_GAUSS_LEGENDRE, 0, 16) == 0
+    assert B.cuhpx_grid_npix(7, 8, 16) == 0                                    # unknown grid
+    assert B.cuhpx_grid_npix(B.CUHPX_GRID_HEALPIX, 4, 0) == 12 * 16
+    assert int(B._lib.cuhpx_grid_workspace_bytes(B.CUHPX_GRID_EQUIANGULAR, 8, 16, 4, 5, 1, 1)) == 0   # mmax > lmax
+    c, w = B.cuhpx_grid_ring_info(B.CUHPX_GRID_GAUSS_LEGENDRE, 5, 8, 3)
+    assert abs(c) < 1e-15 and w > 0                                            # the middle node of an odd rule is the equator
 
 
 @pytest.mark.gpu
