@@ -6,13 +6,23 @@
 //   M = 128 ring pairs (one per thread = one tensor-memory lane), K = degrees l of one parity, N = columns c.
 //   Every thread walks the fp64 recurrence of its ring pairs and writes lambda -- split in two TF32 terms,
 //   lambda = hi + lo -- straight into tensor memory as the A operand (tcgen05.st: lane = ring, column = degree):
-//   lambda never touches shared memory.  The B operand (s_l a_lm, also split hi + lo, K-major [hi | lo] columns)
-//   is a small shared-memory tile built by the CTA.  Per 8 degrees of one parity two instructions
+//   lambda never touches shared memory.  The B operand (s_l a_lm, also split hi + lo, K-major [hi | lo] columns) is
+//   laid out once per call by a small pre-pass kernel (synthesis_images_kernel) as ready-to-use "images" in the
+//   workspace -- per (channel group, order m, stage of 32 degrees): the 32 recurrence coefficients alpha and four
+//   K = 8 tiles [parity][K block] -- which the main kernel fetches with one bulk asynchronous copy (TMA, mbarrier
+//   complete_tx) per stage, three in flight.  Per 8 degrees of one parity two instructions
 //       D(128 x 4 NB) += A_hi (TMEM) x [a_hi | a_lo],      D(128 x 2 NB) += A_lo (TMEM) x [a_hi]
 //   give hi hi + hi lo + lo hi (the dropped lo lo term is 2^-22 relative); the accumulators E (even l - m) and
 //   O (odd) live in tensor memory and come back once, at the end: G(N) = E + O, G(S) = E - O.
-//   A stage = 16 degrees; the lambda buffers and the a_lm tiles are double buffered, tcgen05.commit -> mbarrier tells
-//   the producers when a buffer may be overwritten.
+//   CTA = 4 producer warps (one 128-ring tile) + one warp that requests the images and issues the tcgen05.mma of a
+//   stage when the producers have parked it (mbarrier `ready`), committing to the mbarrier (`bar`) the producers wait
+//   on before they overwrite the lambda buffer; the next stage is generated into registers meanwhile.  128 columns of
+//   tensor memory per CTA at NB = 8: four CTAs per SM.
+//   Variants measured and dropped (cfg4, 2.37 ms as built): two tiles per CTA 2.58 ms; lambda double-buffered by
+//   half-stages of 16 degrees 2.59 ms; two ring pairs per producer thread 2.66 ms; two producer threads per ring pair
+//   (one per parity, duplicated recurrence) 3.61 ms.  With an empty pipeline (no recurrence, no MMA) the kernel takes
+//   0.86 ms: 0.48 ms per-CTA fixed cost (seeds, first image, the strided 8-byte epilogue stores) + 0.38 ms of per-stage
+//   synchronisation.
 #include <cuda_runtime.h>
 #include <math.h>
 #include <stdlib.h>
