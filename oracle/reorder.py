@@ -77,7 +77,8 @@ def flat_centres(nside: int, corner: int, sense: int):
     row-major nside x nside image whose origin is the face's corner `corner` (0 S, 1 E, 2 N, 3 W) and whose fast axis
     runs along the face edge towards the counter-clockwise (sense 0: S -> E -> N -> W) or clockwise (sense 1) neighbour
     corner, the slow axis along the other edge.  Written with the corners of the face diamond in the projection plane,
-    not with (x, y) index arithmetic."""
+    not with (x, y) index arithmetic.  The paper defines the layout only by Fig. 3C: that this reading matches the figure's
+    face orientation is PARITY UNPINNED (R12); the stated geometry itself is pinned in tests/test_reorder.py."""
     npix = 12 * nside * nside
     ip = np.arange(npix, dtype=np.int64)
     f = ip // (nside * nside)

@@ -9,6 +9,8 @@ quadrature of Eq. 26 is exact,
 Written out as the textbook minimum-norm solution of a linear system, dense, in long double:
         M[l][i] = sqrt(N_i) lambda_l0(theta_i),   r = sqrt(4 pi) e_0 - M sqrt(N) w0,
         w = w0 + N^-1/2 M^T (M M^T)^+ r
+Whether these weights equal the values HEALPix tabulates is PARITY UNPINNED (the files are not available; DESIGN.md R11);
+everything the definition above states is pinned in tests/test_ring_weights.py.
 lambda_l0 comes from the oracle's own recurrence (oracle/sht_oracle.c, pinned in tests/test_oracle_pins.py); the solve is
 numpy's (a library primitive serving as a step).
 """
