@@ -65,24 +65,28 @@ def build(force: bool = False, verbose: bool = False) -> str:
     return LIB
 
 
-PROBE = os.path.join(HERE, "tcgen05_probe")
+PROBES = {"tcgen05_probe": "tcgen05_probe.cu", "dfma_probe": "dfma_probe.cu"}
 
 
-def build_probe() -> str:
-    """Compile the tcgen05 micro-benchmark (csrc/tcgen05_probe.cu, a measurement tool: profiles/r2_tcgen05_probe.md)."""
+def build_probe() -> list:
+    """Compile the micro-benchmarks (measurement tools outside libcuhpx.so): csrc/tcgen05_probe.cu
+    (profiles/r2_tcgen05_probe.md) and csrc/dfma_probe.cu (profiles/r2_dfma_probe.md)."""
     nvcc = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
-    cmd = [nvcc, "-O3", "-std=c++17", "-gencode", "arch=compute_100a,code=sm_100a", "-o", PROBE,
-           os.path.join(CSRC, "tcgen05_probe.cu")]
-    res = subprocess.run(cmd, capture_output=True, text=True)
-    if res.returncode != 0:
-        sys.stderr.write(res.stdout + res.stderr)
-        raise RuntimeError("nvcc failed building tcgen05_probe")
-    return PROBE
+    built = []
+    for exe, src in PROBES.items():
+        out = os.path.join(HERE, exe)
+        cmd = [nvcc, "-O3", "-std=c++17", "-gencode", "arch=compute_100a,code=sm_100a", "-o", out, os.path.join(CSRC, src)]
+        res = subprocess.run(cmd, capture_output=True, text=True)
+        if res.returncode != 0:
+            sys.stderr.write(res.stdout + res.stderr)
+            raise RuntimeError(f"nvcc failed building {exe}")
+        built.append(out)
+    return built
 
 
 if __name__ == "__main__":
     if "--probe" in sys.argv:
-        print(build_probe())
+        print("\n".join(build_probe()))
     else:
         build(force="--force" in sys.argv, verbose=True)
         print(LIB)
