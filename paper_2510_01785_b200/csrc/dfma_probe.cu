@@ -1,10 +1,10 @@
-// DFMA operand-bandwidth micro-benchmark (a measurement tool outside libcuhpx.so; profiles/r2_dfma_probe.md).
+// Register-operand bandwidth micro-benchmark (a measurement tool outside libcuhpx.so; profiles/r2_dfma_probe.md).
 // Question: why do the fp64 Legendre kernels (legendre.cu), whose inner loops are dense DFMA streams with stall
 // count 2 on every instruction, stop at 62 % (analysis) and 78 % (synthesis) of the FP64 pipe?
 // Part 1 times DFMA streams that differ only in how many source registers are fresh per instruction (not served by
 // the operand reuse cache): the pipe issues one warp-DFMA every 2 clk only when at most two 64-bit registers are
 // read; a third fresh register costs a third clock.  Part 2 times the inner loops of the two kernels in isolation
-// (same arithmetic, nothing else) in the instruction order ptxas chooses.
+// (same arithmetic, nothing else) in the instruction order ptxas chooses.  Part 3 repeats part 1 for FFMA / FFMA2.
 //   build: python -m paper_2510_01785_b200.build --probe        run: ./paper_2510_01785_b200/dfma_probe
 #include <cstdio>
 #include <cuda_runtime.h>
@@ -105,6 +105,47 @@ __global__ void __launch_bounds__(64, 6) loop_kernel(const double* __restrict__ 
     out[blockIdx.x * blockDim.x + threadIdx.x] = s;
 }
 
+// ---- part 3: the same operand patterns for FFMA and the packed FFMA2 (fma.rn.f32x2) of the fp32 kernels
+__device__ __forceinline__ float2 fma2(float2 a, float2 b, float2 c) {
+    float2 d;
+    asm("{\n\t.reg .b64 ra, rb, rc, rd;\n\tmov.b64 ra, {%2, %3};\n\tmov.b64 rb, {%4, %5};\n\tmov.b64 rc, {%6, %7};\n\t"
+        "fma.rn.f32x2 rd, ra, rb, rc;\n\tmov.b64 {%0, %1}, rd;\n\t}"
+        : "=f"(d.x), "=f"(d.y)
+        : "f"(a.x), "f"(a.y), "f"(b.x), "f"(b.y), "f"(c.x), "f"(c.y));
+    return d;
+}
+__device__ __forceinline__ float fmaT(float a, float b, float c) { return fmaf(a, b, c); }
+__device__ __forceinline__ float2 fmaT(float2 a, float2 b, float2 c) { return fma2(a, b, c); }
+__device__ __forceinline__ float sumT(float a) { return a; }
+__device__ __forceinline__ float sumT(float2 a) { return a.x + a.y; }
+
+template <typename V, int T>
+__global__ void __launch_bounds__(128, 4) operand32_kernel(const V* __restrict__ in, float* __restrict__ out, int n) {
+    V a[16], b[16], acc[16];
+#pragma unroll
+    for (int i = 0; i < 16; ++i) {
+        a[i] = in[i + threadIdx.x];
+        b[i] = in[32 + i + threadIdx.x];
+        acc[i] = in[64 + i];
+    }
+#pragma unroll 1
+    for (int t = 0; t < n; ++t) {
+#pragma unroll
+        for (int u = 0; u < 4; ++u)
+#pragma unroll
+            for (int i = 0; i < 16; ++i) {
+                if (T == 2) acc[i] = fmaT(a[i], b[0], acc[i]);
+                if (T == 3) acc[i] = fmaT(a[i], b[i], acc[i]);
+                if (T == 4) acc[i] = fmaT(a[i], a[i], acc[i]);
+                if (T == 5) acc[i] = fmaT(a[i / 2], b[i], acc[i]);
+            }
+    }
+    float s = 0;
+#pragma unroll
+    for (int i = 0; i < 16; ++i) s += sumT(acc[i]);
+    out[blockIdx.x * blockDim.x + threadIdx.x] = s;
+}
+
 template <typename K>
 static float time_ms(K launch) {
     launch();
@@ -139,6 +180,16 @@ static void run_loop(const char* what, const double* in, double* out) {
            2.0 * PEAK_TFLOPS / tf);
 }
 
+template <typename V, int T>
+static void run_operand32(const char* what, const double* in, double* out) {
+    const int n = 8000, grid = 148 * 16;
+    const float ms = time_ms([&] { operand32_kernel<V, T><<<grid, 128>>>(reinterpret_cast<const V*>(in), reinterpret_cast<float*>(out), n); });
+    const double lanes = sizeof(V) / 4;  // FMAs per lane and instruction
+    const double tf = 2.0 * lanes * 64 * n * (double)grid * 128 / ms * 1e-9;
+    printf("%-44s %6.2f TFLOP/s  %5.1f %% of the FMA pipe   -> %.2f clk per warp-instruction\n", what, tf, 100 * tf / (2 * PEAK_TFLOPS),
+           lanes * 2.0 * PEAK_TFLOPS / tf);
+}
+
 int main() {
     double *in, *out;
     cudaMalloc(&in, 8192);
@@ -157,6 +208,14 @@ int main() {
     run_loop<6, 0>("analysis loop, 6 ring pairs, 8 degrees", in, out);
     run_loop<6, 1>("synthesis loop, 6 ring pairs", in, out);
     run_loop<4, 1>("synthesis loop, 4 ring pairs", in, out);
+    printf("-- part 3: FFMA / FFMA2 (fp32 peak %.1f TFLOP/s: one FFMA per clk, one FFMA2 per 2 clk and sub-partition)\n", 2 * PEAK_TFLOPS);
+    run_operand32<float, 2>("FFMA  fma(a_k, b, acc_k)       2 fresh", in, out);
+    run_operand32<float, 5>("FFMA  fma(a_(k/2), b_k, acc_k) 3 then 2 fresh", in, out);
+    run_operand32<float, 3>("FFMA  fma(a_k, b_k, acc_k)     3 fresh", in, out);
+    run_operand32<float2, 2>("FFMA2 fma(a_k, b, acc_k)       2 fresh pairs", in, out);
+    run_operand32<float2, 4>("FFMA2 fma(a_k, a_k, acc_k)     2 distinct pairs", in, out);
+    run_operand32<float2, 5>("FFMA2 fma(a_(k/2), b_k, acc_k) 3 then 2 fresh", in, out);
+    run_operand32<float2, 3>("FFMA2 fma(a_k, b_k, acc_k)     3 fresh pairs", in, out);
     const cudaError_t e = cudaDeviceSynchronize();
     printf("%s\n", cudaGetErrorString(e));
     return e != cudaSuccess;
