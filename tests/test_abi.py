@@ -84,3 +84,16 @@ def test_workspace_bytes_and_argument_validation():
     assert len(B.cuhpx_plan_mcut((4, 8, 8, 1, 1))) == 15
     st = B.cuhpx_plan_stats((32, 64, 64, 1, 1))
     assert st["legendre_terms_full"] == 2145 * 64 and 0 < st["legendre_terms_executed"] <= st["legendre_terms_full"]
+
+
+def test_measurement_probes_compile_for_sm100a():
+    """csrc/tcgen05_probe.cu and csrc/dfma_probe.cu (profiles/r2_tcgen05_probe.md, r2_dfma_probe.md) are measurement tools
+    outside the library; they must keep building with the library's toolchain (nvcc cross-compiles without a GPU)."""
+    import shutil
+
+    from paper_2510_01785_b200 import build as builder
+
+    if shutil.which(os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")) is None:
+        pytest.skip("nvcc not available")
+    for exe in builder.build_probe():
+        assert os.path.getsize(exe) > 0
