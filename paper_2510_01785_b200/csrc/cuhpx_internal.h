@@ -74,6 +74,15 @@ struct DevPlan {
     int tc_nb;                   // channels per group (0: tensor-core path not planned)
     int nchunk_max;          // ring-pair chunks per m in the Legendre analysis grid
     int chunk_pairs;         // ring pairs per chunk
+    // late-start tables of the fp64 Legendre kernels ([0] analysis, [1] synthesis; legendre.cu "late start"): per order
+    // and ring chunk the first 64-degree tile in which a ring pair of the chunk becomes significant, and the recurrence
+    // state of every ring pair at the start of that tile.  st_chunk = 0: not planned.
+    const double* st_cur[2];   // [mmax + 1][npairs]
+    const double* st_prev[2];  // [mmax + 1][npairs]
+    const int* st_sc[2];       // [mmax + 1][npairs] exponent window of the stored state
+    const int* st_l0[2];       // [mmax + 1][st_nchunk] l - m of the first tile to run
+    int st_chunk[2];           // ring pairs per chunk the tables were built for
+    int st_nchunk[2];
 };
 
 // true if the workspace behind P was initialised for the parameters of this call (one 16-byte load per CTA)
@@ -102,6 +111,7 @@ struct HostPlan {
     // table offsets inside the workspace
     size_t off_y, off_lshi, off_lslo, off_ringN, off_start, off_shifted, off_mcut, off_prefhi, off_preflo, off_jmin;
     size_t off_fft, fft_bytes, off_alpha, off_scale, off_spectra, off_partial, off_tcprefix, off_tcimages;
+    size_t off_st[2][4] = {{0, 0, 0, 0}, {0, 0, 0, 0}};  // late-start tables: cur, prev, sc, l0
     std::vector<long long> h_tcprefix;
     std::vector<int> h_ringN, h_mcut, h_jmin, h_shifted;
     std::vector<long long> h_start;

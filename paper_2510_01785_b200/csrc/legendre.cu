@@ -10,6 +10,7 @@
 // registers.  cos(theta) enters as x p = p - y p with y = 1 - cos(theta) (R3).
 #include <cuda_runtime.h>
 #include <math.h>
+#include <stdlib.h>
 
 #include "cuhpx_internal.h"
 #include "legendre_common.cuh"
@@ -235,6 +236,29 @@ __global__ void __launch_bounds__(NT, MINB) legendre_analysis_kernel(LegArgs a) 
     if (a.to_partial) out += (size_t)chunk * P.batch * P.nalm * 2;
 
     const int nl = P.lmax - m + 1;  // l values of this m
+    // late start (tables built by legendre_start_kernel): no ring pair of this chunk is significant before degree
+    // m + tstart, so the walk begins there with the recurrence state the skipped steps would have produced
+    int tstart = 0;
+    if (SEQ && P.st_chunk[0] == NT * R) {
+        tstart = P.st_l0[0][(size_t)m * P.st_nchunk[0] + chunk];
+        if (tstart > 0) {
+#pragma unroll
+            for (int r = 0; r < R; ++r) {
+                const int j = jbase + tid + NT * r;
+                if (j < P.npairs) {
+                    const size_t e = (size_t)m * P.npairs + j;
+                    cur[r] = P.st_cur[0][e];
+                    prev[r] = P.st_prev[0][e];
+                    sc[r] = P.st_sc[0][e];
+                }
+            }
+            if (chunk == 0) {  // the first chunk initialises a_lm: zeros where nothing is significant yet
+                const int ch = ch0;  // BT == 1 on this path
+                if (ch < P.batch)
+                    for (int e = tid; e < 2 * tstart; e += NT) out[((size_t)ch * P.nalm + abase + m) * 2 + e] = 0;
+            }
+        }
+    }
     bool warp_active = __any_sync(0xffffffffu, nact > 0);
     // alpha of the steps that produce degrees l = m + t0 + 1 + i; the next tile is fetched into a register while
     // the current one is consumed, so no global-load latency sits between two tiles
@@ -243,10 +267,10 @@ __global__ void __launch_bounds__(NT, MINB) legendre_analysis_kernel(LegArgs a) 
 #pragma unroll
     for (int q = 0; q < APT; ++q) {
         const int i = tid + q * NT;
-        nextA[q] = (i < CT && 1 + i < nl) ? P.coef_alpha[abase + m + 1 + i] : 0.0;
+        nextA[q] = (i < CT && tstart + 1 + i < nl) ? P.coef_alpha[abase + m + tstart + 1 + i] : 0.0;
     }
     constexpr int NOUT = (TPG * NV + NT - 1) / NT;  // output elements per thread and group (cross-warp sums)
-    for (int t0 = 0; t0 < nl; t0 += CT) {
+    for (int t0 = tstart; t0 < nl; t0 += CT) {
         const int cb = (t0 / CT) & 1;
 #pragma unroll
         for (int q = 0; q < APT; ++q) {
@@ -823,9 +847,25 @@ __global__ void __launch_bounds__(NT) legendre_synthesis_kernel(LegArgs a) {
             nAlm[q] = ok ? alm[((size_t)ch * P.nalm + abase + m + k) * 2 + ri] : (T)0;
         }
     };
-    fetch(0);
+    int tstart = 0;  // late start, as in legendre_analysis_kernel
+    if (P.st_chunk[1] == NT * R) {
+        tstart = P.st_l0[1][(size_t)m * P.st_nchunk[1] + chunk];
+        if (tstart > 0) {
+#pragma unroll
+            for (int r = 0; r < R; ++r) {
+                const int j = jbase + tid + NT * r;
+                if (j < P.npairs) {
+                    const size_t e = (size_t)m * P.npairs + j;
+                    cur[r] = P.st_cur[1][e];
+                    prev[r] = P.st_prev[1][e];
+                    sc[r] = P.st_sc[1][e];
+                }
+            }
+        }
+    }
+    fetch(tstart);
     bool all_on = false;  // every ring pair of this warp is active (sc == 0)
-    for (int t0 = 0; t0 < nl; t0 += CT) {
+    for (int t0 = tstart; t0 < nl; t0 += CT) {
         __syncthreads();  // previous tile fully consumed
         if (tid < CT) sA[tid] = nA;
 #pragma unroll
@@ -1115,6 +1155,114 @@ template <> struct LegCfg<float, 4> { static constexpr int NT = 128, R = 4, LT =
 // batched fp32 analysis: contraction kernels.  Long degree ranges use the 64-degree tiles with in-place accumulation
 // over the ring chunks (one "chunk" as far as the plan is concerned: no partial arrays); short ones (a few tiles per
 // order, latency-bound) the 32-degree tiles with one CTA per ring chunk.
+// ------------------------------------------------------------------ late start of the fp64 kernels
+// For small m every ring pair is significant from l = m on; for large m the polar-most chunks walk hundreds of degrees
+// with every lambda below the exponent window (recurrence only, nothing accumulated).  Those steps do not depend on the
+// data: at workspace set-up this kernel walks them once per (m, chunk) exactly as the transform kernels would (same
+// seeds, same two FMAs, same rescale checks every CHECK_EVERY degrees) and stores, for the first 64-degree tile in
+// which a ring pair of the chunk crosses the window, the tile's first degree and every ring pair's state (value,
+// previous value, exponent window) at that degree.  The transform kernels start there: results are bit-identical.
+template <int R, int NT>
+__global__ void __launch_bounds__(NT) legendre_start_kernel(DevPlan P, int which) {
+    const int m = blockIdx.x, chunk = blockIdx.y, tid = threadIdx.x;
+    const int jbase = P.jmin[m] + chunk * (NT * R);
+    int* l0 = const_cast<int*>(P.st_l0[which]) + (size_t)m * P.st_nchunk[which] + chunk;
+    if (jbase >= P.npairs) {
+        if (tid == 0) *l0 = 0;
+        return;
+    }
+    double cur[R], prev[R], y[R], scur[R], sprev[R];
+    int sc[R], ssc[R];
+    const double pref_hi = P.pref_hi[m], pref_lo = P.pref_lo[m];
+#pragma unroll
+    for (int r = 0; r < R; ++r) {
+        const int j = jbase + tid + NT * r;
+        if (j < P.npairs) {
+            y[r] = P.y[j];
+            lambda_seed<double>(m, pref_hi, pref_lo, P.ls_hi[j], P.ls_lo[j], cur[r], sc[r]);
+            prev[r] = 0.0;
+        } else {
+            y[r] = 1.0;
+            cur[r] = 0.0;
+            prev[r] = 0.0;
+            sc[r] = -1;
+        }
+    }
+    const long long abase = (long long)m * (2LL * P.lmax + 1 - m) / 2;
+    const int nl = P.lmax - m + 1;
+    int t0 = 0;
+    for (;; t0 += CT) {
+#pragma unroll
+        for (int r = 0; r < R; ++r) {
+            scur[r] = cur[r];
+            sprev[r] = prev[r];
+            ssc[r] = sc[r];
+        }
+        if (t0 + CT >= nl) break;  // the last tile is always run by the transform kernels
+        bool act = false;
+        const int tend = min(CT, nl - t0);
+        for (int s0 = 0; s0 < tend && !act; s0 += CHECK_EVERY) {
+#pragma unroll
+            for (int r = 0; r < R; ++r) {
+                if (sc[r] < 0 && fabs(cur[r]) > pow2c(ScaleCfg<double>::THR)) {
+                    cur[r] *= pow2c(-ScaleCfg<double>::K);
+                    prev[r] *= pow2c(-ScaleCfg<double>::K);
+                    ++sc[r];
+                }
+                act |= (sc[r] == 0);
+            }
+            act = __syncthreads_or(act);
+            if (act) break;
+            for (int i = 0; i < CHECK_EVERY; ++i) {
+                const int k = t0 + s0 + i;  // step producing degree m + k + 1
+                const double A = (k + 1 < nl) ? P.coef_alpha[abase + m + k + 1] : 0.0;
+#pragma unroll
+                for (int r = 0; r < R; ++r) {
+                    const double xl = fma(-y[r], cur[r], cur[r]);
+                    const double nx = fma(A, xl, -prev[r]);
+                    prev[r] = cur[r];
+                    cur[r] = nx;
+                }
+            }
+        }
+        if (act) break;
+    }
+    if (tid == 0) *l0 = t0;
+#pragma unroll
+    for (int r = 0; r < R; ++r) {
+        const int j = jbase + tid + NT * r;
+        if (j < P.npairs) {
+            const size_t e = (size_t)m * P.npairs + j;
+            const_cast<double*>(P.st_cur[which])[e] = scur[r];
+            const_cast<double*>(P.st_prev[which])[e] = sprev[r];
+            const_cast<int*>(P.st_sc[which])[e] = ssc[r];
+        }
+    }
+}
+
+// chunk sizes of the two fp64 kernels (must agree with launch_legendre_analysis / launch_legendre_synthesis below)
+constexpr int ST_R_ANA = 7, ST_R_SYN = 6, ST_NT = 64;
+void legendre_start_chunks(cuhpx_dtype_t dt, int npairs, int chunk[2]) {
+    const char* sw = getenv("CUHPX_LATE_START");  // "0": walk every order from l = m (A/B measurements)
+    const bool on = dt == CUHPX_F64 && npairs >= 2048 && !(sw && sw[0] == '0');
+    chunk[0] = on ? ST_R_ANA * ST_NT : 0;
+    chunk[1] = on ? ST_R_SYN * ST_NT : 0;
+}
+
+cudaError_t launch_legendre_start_tables(const DevPlan& P, cudaStream_t st) {
+    if (P.st_chunk[0] > 0) {
+        legendre_start_kernel<ST_R_ANA, ST_NT><<<dim3(P.mmax + 1, P.st_nchunk[0]), ST_NT, 0, st>>>(P, 0);
+        cudaError_t e = cudaGetLastError();
+        if (e != cudaSuccess) return e;
+    }
+    if (P.st_chunk[1] > 0) {
+        legendre_start_kernel<ST_R_SYN, ST_NT><<<dim3(P.mmax + 1, P.st_nchunk[1]), ST_NT, 0, st>>>(P, 1);
+        cudaError_t e = cudaGetLastError();
+        if (e != cudaSuccess) return e;
+    }
+    return cudaSuccess;
+}
+
 static bool use_gemm64(int lmax) { return lmax >= 512; }
 
 int legendre_chunk_pairs(cuhpx_dtype_t dt, int batch, int lmax, int npairs) {

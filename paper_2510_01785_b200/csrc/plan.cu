@@ -19,6 +19,8 @@
 namespace cuhpx {
 
 int legendre_chunk_pairs(cuhpx_dtype_t dt, int batch, int lmax, int npairs);  // legendre.cu
+void legendre_start_chunks(cuhpx_dtype_t dt, int npairs, int chunk[2]);            // legendre.cu
+cudaError_t launch_legendre_start_tables(const DevPlan& P, cudaStream_t st);         // legendre.cu
 
 namespace {
 
@@ -295,6 +297,18 @@ HostPlan* make_plan(const Grid& grid, int lmax, int mmax, int batch, cuhpx_dtype
         const size_t groups = (size_t)(batch + d.tc_nb - 1) / d.tc_nb;
         hp->off_tcimages = take(groups * (size_t)hp->h_tcprefix[mmax + 1] * legendre_tc_image_bytes(d.tc_nb));
     }
+    // late-start tables of the fp64 Legendre kernels (legendre.cu)
+    legendre_start_chunks(dt, d.npairs, d.st_chunk);
+    for (int k = 0; k < 2; ++k) {
+        d.st_nchunk[k] = 0;
+        if (d.st_chunk[k] <= 0) continue;
+        d.st_nchunk[k] = (d.npairs + d.st_chunk[k] - 1) / d.st_chunk[k];
+        const size_t n = (size_t)(mmax + 1) * d.npairs;
+        hp->off_st[k][0] = take(sizeof(double) * n);
+        hp->off_st[k][1] = take(sizeof(double) * n);
+        hp->off_st[k][2] = take(sizeof(int) * n);
+        hp->off_st[k][3] = take(sizeof(int) * (size_t)(mmax + 1) * d.st_nchunk[k]);
+    }
     hp->workspace_bytes = o;
     return hp;
 }
@@ -393,6 +407,13 @@ DevPlan HostPlan::resolve(void* ws) const {
     P.partial = d.nchunk_max > 1 ? base + off_partial : nullptr;
     P.tc_prefix = d.tc_nb > 0 ? (const long long*)(base + off_tcprefix) : nullptr;
     P.tc_images = d.tc_nb > 0 ? base + off_tcimages : nullptr;
+    for (int k = 0; k < 2; ++k) {
+        const bool on = d.st_chunk[k] > 0;
+        P.st_cur[k] = on ? (const double*)(base + off_st[k][0]) : nullptr;
+        P.st_prev[k] = on ? (const double*)(base + off_st[k][1]) : nullptr;
+        P.st_sc[k] = on ? (const int*)(base + off_st[k][2]) : nullptr;
+        P.st_l0[k] = on ? (const int*)(base + off_st[k][3]) : nullptr;
+    }
     return P;
 }
 
@@ -487,6 +508,7 @@ static int workspace_init_impl(const Grid& grid, int lmax, int mmax, int batch, 
     if (e == cudaSuccess)
         e = launch_legendre_coeff(lmax, mmax, (double*)(base + hp->off_alpha), (double*)(base + hp->off_scale), st);
     if (e == cudaSuccess) e = fft_build_tables(*hp, base + hp->off_fft, st);
+    if (e == cudaSuccess) e = launch_legendre_start_tables(hp->resolve(ws), st);
     hdr.magic = WS_MAGIC;
     hdr.key = d.key;
     hdr.nside = nside;
