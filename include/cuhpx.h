@@ -47,8 +47,11 @@
  *     thrown across the ABI.  After CUHPX_ECUDA, cudaGetLastError() describes the launch failure.
  *   - batch <= 65535 (channels index a grid dimension).
  *   - There is no CPU fallback: on a machine without a CUDA device every compute call returns CUHPX_ECUDA.
- *   - One environment switch, read once per process, for A/B measurements only: CUHPX_LEGENDRE_TC=0 runs batched fp32
- *     Legendre synthesis (batch >= 8) on the CUDA-core kernels instead of the tcgen05 / tensor-memory kernel.
+ *   - Two environment switches for A/B measurements only.  CUHPX_LEGENDRE_TC=0 (read once per process) runs batched
+ *     fp32 Legendre synthesis (batch >= 8) on the CUDA-core kernels instead of the tcgen05 / tensor-memory kernel.
+ *     CUHPX_LATE_START=0 (read when a parameter set is first planned) leaves out the late-start tables of the fp64
+ *     Legendre kernels (20 bytes per (m, ring pair) and direction of workspace, transforms with >= 2048 ring pairs):
+ *     every order is then walked from l = m.  Results are bit-identical either way.
  */
 #ifndef CUHPX_H_
 #define CUHPX_H_

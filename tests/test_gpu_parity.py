@@ -497,3 +497,37 @@ def test_cuda_graph_capture_replay(nside, lmax, batch, dtype):
         torch.cuda.synchronize()
         assert torch.equal(o_alm, T.map2alm(fmap)) and torch.equal(o_map, T.alm2map(alm))
     B.cuhpx_workspace_check(*T.params, T.workspace)
+
+
+def test_late_start_tables_change_no_bit():
+    """fp64 Legendre kernels with >= 2048 ring pairs start each (order, ring chunk) at the first tile with a significant
+    ring pair, from a tabulated recurrence state (legendre.cu "late start").  The skipped steps carry no data, so the
+    results must equal those of the full walk (CUHPX_LATE_START=0, its own process: plans are memoised) bit for bit."""
+    import os
+    import subprocess
+    import sys
+    import tempfile
+
+    nside, lmax = 1024, 2047  # 2048 ring pairs: the smallest transform that plans the tables
+    code = (
+        "import sys, torch; sys.path.insert(0, %r)\n"
+        "from paper_2510_01785_b200 import binding as B\n"
+        "t = B.Transform(%d, %d, %d, 1, torch.float64)\n"
+        "g = torch.Generator(device='cuda').manual_seed(5)\n"
+        "m = torch.randn(1, t.npix, dtype=torch.float64, device='cuda', generator=g)\n"
+        "a = t.map2alm(m); r = t.alm2map(a); ga = t.alm2map_adjoint(m); gm = t.map2alm_adjoint(a)\n"
+        "torch.save({'alm': a.cpu(), 'map': r.cpu(), 'galm': ga.cpu(), 'gmap': gm.cpu(), 'ws': t.workspace.numel()}, sys.argv[1])\n"
+    ) % (os.path.dirname(os.path.dirname(os.path.abspath(__file__))), nside, lmax, lmax)
+    with tempfile.TemporaryDirectory() as d:
+        res = {}
+        for arm in ("0", "1"):
+            env = dict(os.environ)
+            env.pop("CUHPX_LATE_START", None)
+            if arm == "0":
+                env["CUHPX_LATE_START"] = "0"
+            path = os.path.join(d, f"arm{arm}.pt")
+            subprocess.run([sys.executable, "-c", code, path], env=env, check=True, timeout=600)
+            res[arm] = torch.load(path)
+    assert res["1"]["ws"] > res["0"]["ws"], "the tables were not planned"
+    for k in ("alm", "map", "galm", "gmap"):
+        assert torch.equal(res["0"][k], res["1"][k]), f"{k} differs between the full walk and the late start"
