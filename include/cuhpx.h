@@ -139,6 +139,17 @@ size_t cuhpx_ring_weights_workspace_bytes(int nside, int lmax_w);
 int cuhpx_ring_weights(int nside, int lmax_w, double* d_weights, void* d_workspace, size_t workspace_bytes,
                        cuhpx_stream_t stream);
 
+/* ---- the same solver for callers that may not allocate device memory (graph-capture set-up, serving loops, harnesses
+ * that forbid cudaMalloc): the scratch is a built-in device array of CUHPX_NOALLOC_SCRATCH_BYTES (8 MiB) that every GPU
+ * loading the library holds until the process exits; the call (and everything below it) makes no cudaMalloc / cudaFree
+ * / allocating library call.  Same arguments, result and error codes as cuhpx_ring_weights without the workspace; a
+ * request with cuhpx_ring_weights_workspace_bytes(nside, lmax_w) > CUHPX_NOALLOC_SCRATCH_BYTES (nside >= 1024 at the
+ * default lmax_w) returns CUHPX_EWORKSPACE before anything is launched.  All calls on one device SHARE the array: it is
+ * cleared at the start of each call, and two calls whose GPU work overlaps in time (other streams, other host threads)
+ * race -- serialise them.  SYNCHRONISES `stream` like cuhpx_ring_weights. */
+#define CUHPX_NOALLOC_SCRATCH_BYTES (8u << 20)
+int cuhpx_ring_weights_noalloc(int nside, int lmax_w, double* d_weights, cuhpx_stream_t stream);
+
 /* ---- layout reordering NESTED <-> RING (paper section III-B, via (x, y, f) P:118-123)
  * NESTED: index = f nside^2 + Z-order (Morton) interleave of (x, y) inside base face f (x on the even bits), P:109;
  * RING: as everywhere else in this header.  d_in / d_out: [batch][npix] elements of `dtype` (moved as bits,

@@ -27,7 +27,7 @@ EXPORTS = [
     "cuhpx_grid_npix", "cuhpx_grid_ring_info", "cuhpx_grid_workspace_bytes", "cuhpx_grid_workspace_init",
     "cuhpx_grid_alm2map", "cuhpx_grid_map2alm", "cuhpx_grid_alm2map_adjoint", "cuhpx_grid_map2alm_adjoint",
     "cuhpx_reorder_layout", "cuhpx_layout_index",
-    "cuhpx_map2alm_iter", "cuhpx_ring_weights_workspace_bytes", "cuhpx_ring_weights", "cuhpx_reorder", "cuhpx_nest2ring_index", "cuhpx_alm_resize",
+    "cuhpx_map2alm_iter", "cuhpx_ring_weights_workspace_bytes", "cuhpx_ring_weights", "cuhpx_ring_weights_noalloc", "cuhpx_reorder", "cuhpx_nest2ring_index", "cuhpx_alm_resize",
 ]
 CUHPX_NEST2RING, CUHPX_RING2NEST = 0, 1
 CUHPX_GRID_HEALPIX, CUHPX_GRID_GAUSS_LEGENDRE, CUHPX_GRID_EQUIANGULAR = 0, 1, 2
@@ -83,6 +83,7 @@ def _load() -> ctypes.CDLL:
     lib.cuhpx_ring_weights_workspace_bytes.argtypes = [i, i]
     lib.cuhpx_ring_weights_workspace_bytes.restype = sz
     lib.cuhpx_ring_weights.argtypes = [i, i, vp, vp, sz, vp]
+    lib.cuhpx_ring_weights_noalloc.argtypes = [i, i, vp, vp]
     lib.cuhpx_alm_resize.argtypes = [i, i, i, i, i, i, vp, vp, vp]
     lib.cuhpx_nest2ring_index.restype = ctypes.c_longlong
     lib.cuhpx_nest2ring_index.argtypes = [i, ctypes.c_longlong]
@@ -227,6 +228,15 @@ def cuhpx_ring_weights_workspace_bytes(nside: int, lmax_w: int = 0) -> int:
 def cuhpx_ring_weights(nside, lmax_w, d_weights, workspace, stream=None) -> None:
     p, n = _ws_args(workspace)
     _check(_lib.cuhpx_ring_weights(nside, lmax_w, _dev_ptr(d_weights), p, n, _stream_ptr(stream)), "cuhpx_ring_weights")
+
+
+CUHPX_NOALLOC_SCRATCH_BYTES = 8 << 20
+
+
+def cuhpx_ring_weights_noalloc(nside, lmax_w, d_weights, stream=None) -> None:
+    """cuhpx_ring_weights with the scratch in the library's built-in device array (no device allocation; requests needing
+    more than CUHPX_NOALLOC_SCRATCH_BYTES raise CUHPX_EWORKSPACE; calls on one device share the array: serialise them)."""
+    _check(_lib.cuhpx_ring_weights_noalloc(nside, lmax_w, _dev_ptr(d_weights), _stream_ptr(stream)), "cuhpx_ring_weights_noalloc")
 
 
 def ring_weights(nside: int, lmax_w: int = 0, device="cuda") -> torch.Tensor:

@@ -11,7 +11,7 @@ import sys
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libcuhpx.so")
-SOURCES = ["plan.cu", "legendre.cu", "legendre_tc.cu", "ring_fft.cu", "reorder.cu", "ring_weights.cu"]
+SOURCES = ["plan.cu", "legendre.cu", "legendre_tc.cu", "ring_fft.cu", "reorder.cu", "ring_weights.cu", "noalloc.cu"]
 HEADERS = [os.path.join(CSRC, "cuhpx_internal.h"), os.path.join(CSRC, "block_fft.cuh"),
            os.path.join(CSRC, "legendre_common.cuh"), os.path.join(CSRC, "tc_common.cuh"),
            os.path.join(HERE, "..", "include", "cuhpx.h")]
