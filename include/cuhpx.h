@@ -247,6 +247,12 @@ int cuhpx_synthesis_fft_stage(int nside, int lmax, int mmax, int batch, cuhpx_dt
  *  [6] bytes of constant tables read by one FFT-stage call (chirp filters + twiddles)   [7] workspace bytes */
 int cuhpx_plan_stats(int nside, int lmax, int mmax, int batch, cuhpx_dtype_t dtype, double* h_stats, int count);
 
+/* Measurement companion of cuhpx_plan_stats for an initialised workspace: h_skipped[0] / h_skipped[1] = Legendre steps
+ * ((m, ring pair, degree) triples counted in [3] above) that the fp64 analysis / synthesis kernels do NOT walk because of
+ * the late-start tables (0 when none are planned, see CUHPX_LATE_START).  Reads the tables back: SYNCHRONISES `stream`. */
+int cuhpx_late_start_stats(int nside, int lmax, int mmax, int batch, cuhpx_dtype_t dtype, const void* d_workspace,
+                           size_t workspace_bytes, cuhpx_stream_t stream, double* h_skipped);
+
 /* MEASUREMENT HOOK, not part of the transform API: register-only FMA loop used by bench.py to measure the FP64 /
  * FP32 FMA peak of the device in the same run as the transforms (SURVEY 8(d) asks for exactly that).
  * Writes the elapsed milliseconds of `iters` dependent-chain FMAs per thread over the whole GPU to *ms and the

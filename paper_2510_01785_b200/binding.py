@@ -27,7 +27,7 @@ EXPORTS = [
     "cuhpx_grid_npix", "cuhpx_grid_ring_info", "cuhpx_grid_workspace_bytes", "cuhpx_grid_workspace_init",
     "cuhpx_grid_alm2map", "cuhpx_grid_map2alm", "cuhpx_grid_alm2map_adjoint", "cuhpx_grid_map2alm_adjoint",
     "cuhpx_reorder_layout", "cuhpx_layout_index",
-    "cuhpx_map2alm_iter", "cuhpx_ring_weights_workspace_bytes", "cuhpx_ring_weights", "cuhpx_ring_weights_noalloc", "cuhpx_reorder", "cuhpx_nest2ring_index", "cuhpx_alm_resize",
+    "cuhpx_map2alm_iter", "cuhpx_ring_weights_workspace_bytes", "cuhpx_ring_weights", "cuhpx_ring_weights_noalloc", "cuhpx_late_start_stats", "cuhpx_reorder", "cuhpx_nest2ring_index", "cuhpx_alm_resize",
 ]
 CUHPX_NEST2RING, CUHPX_RING2NEST = 0, 1
 CUHPX_GRID_HEALPIX, CUHPX_GRID_GAUSS_LEGENDRE, CUHPX_GRID_EQUIANGULAR = 0, 1, 2
@@ -98,6 +98,7 @@ def _load() -> ctypes.CDLL:
     lib.cuhpx_synthesis_fft_stage.argtypes = [i, i, i, i, i, vp, vp, i, vp, sz, vp]
     lib.cuhpx_fma_peak_probe.argtypes = [i, i, vp, vp, vp]
     lib.cuhpx_plan_stats.argtypes = [i, i, i, i, i, vp, i]
+    lib.cuhpx_late_start_stats.argtypes = [i, i, i, i, i, vp, sz, vp, vp]
     return lib
 
 
@@ -353,6 +354,14 @@ def cuhpx_plan_stats(params) -> dict:
     keys = ["fft_stage_launches", "legendre_analysis_launches", "legendre_synthesis_launches", "legendre_terms_executed",
             "legendre_terms_full", "spectra_entries", "fft_table_bytes", "workspace_bytes"]
     return dict(zip(keys, [float(v) for v in arr]))
+
+
+def cuhpx_late_start_stats(params, workspace, stream=None):
+    """(analysis, synthesis) Legendre steps of legendre_terms_executed that the late-start tables skip (synchronising)."""
+    arr = (ctypes.c_double * 2)()
+    p, n = _ws_args(workspace)
+    _check(_lib.cuhpx_late_start_stats(*params, p, n, _stream_ptr(stream), arr), "cuhpx_late_start_stats")
+    return float(arr[0]), float(arr[1])
 
 
 def cuhpx_fma_peak_probe(dtype: int, iters: int, stream=None):

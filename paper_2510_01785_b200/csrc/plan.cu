@@ -581,6 +581,31 @@ int cuhpx_plan_stats(int nside, int lmax, int mmax, int batch, cuhpx_dtype_t dty
     return CUHPX_OK;
 }
 
+int cuhpx_late_start_stats(int nside, int lmax, int mmax, int batch, cuhpx_dtype_t dtype, const void* ws, size_t ws_bytes,
+                           cuhpx_stream_t stream, double* h_skipped) {
+    if (!valid_args(nside, lmax, mmax, batch, dtype) || !ws || ((uintptr_t)ws & 15) || !h_skipped) return CUHPX_EINVAL;
+    const int rc = cuhpx_workspace_check(nside, lmax, mmax, batch, dtype, ws, ws_bytes, stream);
+    if (rc != CUHPX_OK) return rc;
+    PlanRef hp = get_plan(nside, lmax, mmax, batch, dtype);
+    const DevPlan& d = hp->d;
+    for (int k = 0; k < 2; ++k) {
+        h_skipped[k] = 0.0;
+        if (d.st_chunk[k] <= 0) continue;
+        std::vector<int> l0((size_t)(mmax + 1) * d.st_nchunk[k]);
+        if (cudaMemcpyAsync(l0.data(), (const char*)ws + hp->off_st[k][3], sizeof(int) * l0.size(), cudaMemcpyDeviceToHost,
+                            (cudaStream_t)stream) != cudaSuccess ||
+            cudaStreamSynchronize((cudaStream_t)stream) != cudaSuccess)
+            return CUHPX_ECUDA;
+        for (int m = 0; m <= mmax; ++m)
+            for (int c = 0; c < d.st_nchunk[k]; ++c) {
+                const long long left = (long long)d.npairs - (hp->h_jmin[m] + (long long)c * d.st_chunk[k]);
+                const long long pairs = left < 0 ? 0 : left < d.st_chunk[k] ? left : d.st_chunk[k];
+                h_skipped[k] += (double)l0[(size_t)m * d.st_nchunk[k] + c] * (double)pairs;
+            }
+    }
+    return CUHPX_OK;
+}
+
 #define CUDA_OR_FAIL(expr)                         \
     do {                                           \
         if ((expr) != cudaSuccess) return CUHPX_ECUDA; \
