@@ -156,13 +156,14 @@ def test_grid_argument_errors():
 
 
 @pytest.mark.gpu
-def test_gpu_gauss_legendre_round_trip_large():
-    """nlat 1024 x nlon 2048, lmax 1023: beyond the dense oracle; the exactness of Gauss-Legendre quadrature is the check."""
+@pytest.mark.parametrize("nlat,nlon,lmax", [(1024, 2048, 1023), (4096, 8192, 4095)])
+def test_gpu_gauss_legendre_round_trip_large(nlat, nlon, lmax):
+    """Beyond the dense oracle: the exactness of Gauss-Legendre quadrature is the check.  nlat 4096 has 2048 ring pairs, the
+    smallest fp64 transform whose Legendre kernels use the late-start tables -- here on a geometry other than HEALPix."""
     import torch
 
     from paper_2510_01785_b200 import binding as B
 
-    nlat, nlon, lmax = 1024, 2048, 1023
     T = B.GridTransform(B.CUHPX_GRID_GAUSS_LEGENDRE, nlat, nlon, lmax, lmax, 1, torch.float64)
     alm = synth.powerlaw_alm(31, lmax, lmax, 1)
     z0 = [oracle.alm_index(lmax, l, 0) for l in range(lmax + 1)]
