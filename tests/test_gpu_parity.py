@@ -413,36 +413,38 @@ def test_nside1024_fp32_few_channels(batch):
 
 
 @pytest.mark.slow
-def test_cfg5_nside4096_fp64():
+@pytest.mark.parametrize("nside,lmax,mmax,seed", [(4096, 8191, 8191, 505), (2048, 4095, 4095, 506), (2048, 5000, 3777, 507)],
+                         ids=["cfg5", "nside2048", "nside2048-ragged"])
+def test_cfg5_nside4096_fp64(nside, lmax, mmax, seed):
     """configs[4]: nside 4096, lmax = mmax = 8191, fp64: alm -> alm2map -> map2alm.  Oracle checked on a seeded
     subset of 512+ (l, m) and 64+ rings; the analysis is checked on the GPU's own map so both
-    sides see identical input."""
-    nside, lmax = 4096, 8191
-    T = make_transform(nside, lmax, lmax, 1, "f64")
-    alm = synth.powerlaw_alm(505, lmax, lmax, 1)
-    rings = _subset_rings(505, nside, 60)
-    sl, sm = _subset_lm(505, lmax, lmax, 60, 9)
+    sides see identical input.  The nside 2048 cases run the same late-start Legendre kernels with other chunk counts,
+    lmax > 2 nside and mmax < lmax."""
+    T = make_transform(nside, lmax, mmax, 1, "f64")
+    alm = synth.powerlaw_alm(seed, lmax, mmax, 1)
+    rings = _subset_rings(seed, nside, 60)
+    sl, sm = _subset_lm(seed, lmax, mmax, 60, 9)
     assert len(sl) >= 512 and len(rings) >= 64
     sl_idx = [oracle.alm_index(lmax, l, m) for l, m in zip(sl, sm)]
     slices = _ring_slices(nside, rings)
     dmap = T.alm2map(to_dev(alm, "f64", True))
     got_map = dmap.cpu().numpy()[0]
-    ref = oracle.alm2map_rings(nside, lmax, lmax, alm[0], rings)
+    ref = oracle.alm2map_rings(nside, lmax, mmax, alm[0], rings)
     got = np.concatenate([got_map[s] for s in slices])
     e_syn = np.abs(got - ref).max() / np.abs(ref).max()  # oracle-side maximum (of the sampled rings)
     assert e_syn <= TOL64, f"alm2map {e_syn:.3e}"
     galm = T.map2alm(dmap).cpu().numpy()[0]
-    ref = oracle.map2alm_subset(nside, lmax, lmax, got_map, sl, sm)
+    ref = oracle.map2alm_subset(nside, lmax, mmax, got_map, sl, sm)
     e_ana = np.abs(galm[sl_idx] - ref).max() / np.abs(ref).max()  # the sample holds (0, 0), the largest coefficient
     assert e_ana <= TOL64, f"map2alm {e_ana:.3e}"
     assert np.all(galm[: lmax + 1].imag == 0.0)
     # adjoints on the same subset
     gst = T.alm2map_adjoint(dmap).cpu().numpy()[0]
-    ref = oracle.alm2map_adjoint_subset(nside, lmax, lmax, got_map, sl, sm)
+    ref = oracle.alm2map_adjoint_subset(nside, lmax, mmax, got_map, sl, sm)
     e_st = np.abs(gst[sl_idx] - ref).max() / np.abs(ref).max()
     assert e_st <= TOL64, f"alm2map_adjoint {e_st:.3e}"
     gat = T.map2alm_adjoint(to_dev(alm, "f64", True)).cpu().numpy()[0]
-    ref = oracle.map2alm_adjoint_rings(nside, lmax, lmax, alm[0], rings)
+    ref = oracle.map2alm_adjoint_rings(nside, lmax, mmax, alm[0], rings)
     got = np.concatenate([gat[s] for s in slices])
     e_at = np.abs(got - ref).max() / np.abs(ref).max()
     assert e_at <= TOL64, f"map2alm_adjoint {e_at:.3e}"
