@@ -5,6 +5,7 @@
 // the operand reuse cache): the pipe issues one warp-DFMA every 2 clk only when at most two 64-bit registers are
 // read; a third fresh register costs a third clock.  Part 2 times the inner loops of the two kernels in isolation
 // (same arithmetic, nothing else) in the instruction order ptxas chooses.  Part 3 repeats part 1 for FFMA / FFMA2.
+// Part 4 runs a DFMA stream and an FFMA2 stream side by side on every sub-partition.
 //   build: python -m paper_2510_01785_b200.build --probe        run: ./paper_2510_01785_b200/dfma_probe
 #include <cstdio>
 #include <cuda_runtime.h>
@@ -146,6 +147,52 @@ __global__ void __launch_bounds__(128, 4) operand32_kernel(const V* __restrict__
     out[blockIdx.x * blockDim.x + threadIdx.x] = s;
 }
 
+// ---- part 4: do a DFMA stream and an FFMA2 stream on the SAME sub-partition overlap?  One CTA of 8 warps per SM: warps
+// 0-3 (one per sub-partition) run DFMAs, warps 4-7 FFMA2s, each with two fresh operands per instruction (full rate
+// alone).  MODE 1: only the DFMA warps work, 2: only the FFMA2 warps, 3: both.
+template <int MODE>
+__global__ void __launch_bounds__(256, 1) coissue_kernel(const double* __restrict__ in, double* __restrict__ out, int n) {
+    const int warp = threadIdx.x >> 5;
+    double s = 0;
+    if (warp < 4) {
+        if (MODE & 1) {
+            double a[16], acc[16];
+            const double b = in[threadIdx.x];
+#pragma unroll
+            for (int i = 0; i < 16; ++i) {
+                a[i] = in[i + threadIdx.x];
+                acc[i] = in[64 + i];
+            }
+#pragma unroll 1
+            for (int t = 0; t < n; ++t)
+#pragma unroll
+                for (int u = 0; u < 4; ++u)
+#pragma unroll
+                    for (int i = 0; i < 16; ++i) acc[i] = fma(a[i], b, acc[i]);
+#pragma unroll
+            for (int i = 0; i < 16; ++i) s += acc[i];
+        }
+    } else if (MODE & 2) {
+        const float2* fin = reinterpret_cast<const float2*>(in);
+        float2 a[16], acc[16];
+        const float2 b = fin[threadIdx.x];
+#pragma unroll
+        for (int i = 0; i < 16; ++i) {
+            a[i] = fin[i + threadIdx.x];
+            acc[i] = fin[64 + i];
+        }
+#pragma unroll 1
+        for (int t = 0; t < n; ++t)
+#pragma unroll
+            for (int u = 0; u < 4; ++u)
+#pragma unroll
+                for (int i = 0; i < 16; ++i) acc[i] = fma2(a[i], b, acc[i]);
+#pragma unroll
+        for (int i = 0; i < 16; ++i) s += acc[i].x + acc[i].y;
+    }
+    out[blockIdx.x * blockDim.x + threadIdx.x] = s;
+}
+
 template <typename K>
 static float time_ms(K launch) {
     launch();
@@ -216,6 +263,17 @@ int main() {
     run_operand32<float2, 4>("FFMA2 fma(a_k, a_k, acc_k)     2 distinct pairs", in, out);
     run_operand32<float2, 5>("FFMA2 fma(a_(k/2), b_k, acc_k) 3 then 2 fresh", in, out);
     run_operand32<float2, 3>("FFMA2 fma(a_k, b_k, acc_k)     3 fresh pairs", in, out);
+    printf("-- part 4: one DFMA warp and one FFMA2 warp per sub-partition (64 instructions x 20000 trips per warp)\n");
+    {
+        const int n = 20000;
+        const float t1 = time_ms([&] { coissue_kernel<1><<<148, 256>>>(in, out, n); });
+        const float t2 = time_ms([&] { coissue_kernel<2><<<148, 256>>>(in, out, n); });
+        const float t3 = time_ms([&] { coissue_kernel<3><<<148, 256>>>(in, out, n); });
+        const double clk = 1.965e6;  // clocks per ms
+        printf("DFMA warps alone  %.3f ms = %.2f clk per DFMA\n", t1, t1 * clk / (64.0 * n));
+        printf("FFMA2 warps alone %.3f ms = %.2f clk per FFMA2\n", t2, t2 * clk / (64.0 * n));
+        printf("both together     %.3f ms  (sum %.3f, max %.3f)\n", t3, t1 + t2, t1 > t2 ? t1 : t2);
+    }
     const cudaError_t e = cudaDeviceSynchronize();
     printf("%s\n", cudaGetErrorString(e));
     return e != cudaSuccess;
